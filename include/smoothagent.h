@@ -1,0 +1,184 @@
+/*
+ * smoothagent.h -- C ABI of the B200-native re-prefill hot path of SmoothAgent
+ * (arxiv/paper_2607_00151, "lookahead context engineering").
+ *
+ * What the path computes (PAPER.md = the paper text, line numbers Lnnn):
+ *   After a context transformation the transformed segment must be re-prefilled: its K/V are
+ *   built and its tokens attend causally to the retained prefix held in a paged KV cache plus
+ *   themselves (L37, L105-109, L168).  Lookahead re-prefill chunks are co-batched with
+ *   latency-critical decode rows (L392-398).  Per request j the batch carries q_j new query
+ *   tokens over prefix_j cached tokens; "the i-th query token attends to prefix_j + i + 1
+ *   tokens" (L311-313); a decode request is "a single query token that attends to its full KV
+ *   cache of length L_j" (L305).  The scheduler's latency model (Eq. 1) consumes
+ *   profiled attention costs: sa_latency_table measures them.
+ *
+ * Conventions
+ *   - Every call returns an int32_t status: SA_OK or a negative SA_ERR_*.  No exceptions, no
+ *     exit(), nothing is printed.  sa_status_string() names a status.
+ *   - "device" pointers are CUDA device pointers on the pool's device; "host" pointers are
+ *     ordinary host memory.  THE CALLER OWNS EVERY DEVICE BUFFER (pool storage, q/k/v inputs,
+ *     outputs, workspace); the library owns host metadata only.  Host arrays passed to a call
+ *     are copied before it returns and may be reused at once.
+ *   - Hot calls (sa_rope_kv_append, sa_mixed_attention) take a CUDA stream as void*
+ *     (cudaStream_t; NULL = the legacy default stream), only enqueue work, never allocate
+ *     device memory and never synchronise the device.  All hot calls on one pool must be
+ *     issued on one stream (or on streams the caller orders).  A pool is not thread-safe.
+ *   - A call that fails leaves the pool, its block tables and session lengths unchanged.
+ *   - All tensors are bf16 (raw 16-bit patterns), packed ragged: the tokens of request r are
+ *     rows [qo_indptr[r], qo_indptr[r+1]) of a [T, heads, head_dim] row-major array.
+ *   - There is no CPU fallback: without a CUDA device the hot calls return SA_ERR_CUDA.
+ *
+ * Supported shapes: head_dim in {64, 128}; page_size in {16, 64}; num_q_heads a multiple of
+ * num_kv_heads with group size G = Hq/Hkv in {1, 2, 4, 8, 16}.  Anything else:
+ * SA_ERR_UNSUPPORTED.
+ */
+#ifndef SMOOTHAGENT_H_
+#define SMOOTHAGENT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define SA_API __attribute__((visibility("default")))
+#else
+#define SA_API
+#endif
+
+#define SA_OK 0
+#define SA_ERR_INVALID_ARG (-1)
+#define SA_ERR_OUT_OF_PAGES (-2)
+#define SA_ERR_UNSUPPORTED (-3)
+#define SA_ERR_CUDA (-4)
+#define SA_ERR_WORKSPACE_TOO_SMALL (-5)
+#define SA_ERR_OUT_OF_SESSIONS (-6)
+
+typedef struct sa_kv_pool sa_kv_pool; /* opaque */
+
+typedef struct {
+    int32_t num_q_heads;        /* Hq */
+    int32_t num_kv_heads;       /* Hkv; q head h reads kv head h / (Hq/Hkv)  (GQA, L422) */
+    int32_t head_dim;           /* D */
+    int32_t page_size;          /* B: tokens per page */
+    int64_t num_pages;          /* pages in the pool */
+    int32_t max_sessions;       /* concurrently open sessions */
+    int32_t device;             /* CUDA device ordinal of dev_storage */
+    int64_t max_session_tokens; /* longest context one session may reach (sizes its block table) */
+    double rope_base;           /* theta_m = rope_base^(-2m/D); half-split pairing (m, m + D/2) */
+} sa_kv_pool_config;
+
+/* Where a slot lives, so a caller (or a test) can address any K/V element:
+ *   element (page p, kv head g, slot s, dim d) of K is  k_base[p*stride_page + g*stride_head
+ *   + s*stride_slot + d]  (strides in bf16 elements, d contiguous); same for v_base. */
+typedef struct {
+    void *k_base;
+    void *v_base;
+    int64_t stride_page;
+    int64_t stride_head;
+    int64_t stride_slot;
+} sa_kv_layout;
+
+SA_API const char *sa_status_string(int32_t status);
+
+/* ---- sa_kv_pool_create: the page pool and block tables -------------
+ * Bytes of device storage a pool of this configuration needs (K pages, V pages, the device
+ * mirror of the block tables, RoPE frequency table, per-call metadata ring). */
+SA_API int32_t sa_kv_pool_storage_bytes(const sa_kv_pool_config *cfg, size_t *out_bytes);
+
+/* Create a pool over caller-owned device storage (256-byte aligned, >= storage_bytes).
+ * free_page_order (host, nullable): a permutation of [0, num_pages); pages are handed out in
+ * this order (NULL = 0,1,2,...), which is how tests pick the physical page map.
+ * dev_storage == NULL creates a HOST-ONLY pool: session and page bookkeeping work (including
+ * the page allocation of sa_rope_kv_append, which then moves no data), sa_mixed_attention and
+ * sa_latency_table return SA_ERR_CUDA.  Used by the CPU tests of the allocator and planner.
+ * The storage is not cleared: page contents are whatever the caller left there. */
+SA_API int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_storage, size_t bytes,
+                          const int32_t *free_page_order, sa_kv_pool **out_pool);
+SA_API int32_t sa_kv_pool_destroy(sa_kv_pool *pool);
+SA_API int32_t sa_kv_pool_layout(const sa_kv_pool *pool, sa_kv_layout *out);
+SA_API int32_t sa_kv_pool_free_pages(const sa_kv_pool *pool, int64_t *out_free_pages);
+
+/* Sessions: one logical context = an ordered list of pages + a length in tokens. */
+SA_API int32_t sa_kv_session_open(sa_kv_pool *pool, int32_t *out_sid);
+SA_API int32_t sa_kv_session_close(sa_kv_pool *pool, int32_t sid); /* returns its pages to the pool */
+/* Keep the retained prefix [0, new_len), drop the invalidated tail (the context transformation
+ * "invalidates the existing KV cache" from the first changed token on, L37).  Pages wholly
+ * beyond new_len go back to the free list (most recently freed is reused first). */
+SA_API int32_t sa_kv_session_truncate(sa_kv_pool *pool, int32_t sid, int64_t new_len);
+/* len (nullable): tokens; pages (nullable, host): receives min(*n_pages, used) page ids;
+ * n_pages (nullable, in/out): capacity in, pages used out. */
+SA_API int32_t sa_kv_session_query(const sa_kv_pool *pool, int32_t sid, int64_t *len, int32_t *pages,
+                            int32_t *n_pages);
+
+/* ---- sa_rope_kv_append: fused RoPE + scatter of new K/V into pages (step a2) -------------
+ * Request r appends q_r = qo_indptr[r+1]-qo_indptr[r] tokens to session sids[r]; token i of
+ * request r sits at absolute position session_len(r) + i IN THE TRANSFORMED CONTEXT (the
+ * segment starts right after the retained prefix, L105-109).  K is rotated at that position
+ * (computed in fp32 with a split-precision angle, one round-to-nearest-even to bf16) and
+ * stored; V is copied bit for bit; q_inout (nullable) is rotated in place at the same
+ * positions.  Pages are allocated as needed; on SA_ERR_OUT_OF_PAGES nothing is changed.
+ * A session may appear at most once per call.  Slots not addressed by the call keep their bits.
+ *   sids, qo_indptr : host, n_req and n_req+1 entries, qo_indptr[0] == 0, non-decreasing
+ *   k, v            : device bf16 [T, Hkv, D], pre-RoPE
+ *   q_inout         : device bf16 [T, Hq, D], nullable */
+SA_API int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                          const int32_t *qo_indptr, const void *k, const void *v, void *q_inout,
+                          void *stream);
+
+/* ---- sa_mixed_attention: ragged batch of prefill chunks and decode rows (steps a3-a6) -----
+ * Request r has q_r query rows and attends to its session's cache of kv_r = session_len(r)
+ * tokens, WHICH ALREADY CONTAINS its own q_r tokens (append first, then attend; L305 "its full
+ * KV cache").  Row i of request r attends keys 0 .. kv_r - q_r + i (L311-313), softmax in fp32
+ * with scale sm_scale, GQA head mapping h -> h / G.  q_r == 1 is a decode row, q_r > 1 a
+ * prefill chunk, q_r == 0 a no-op; they may be mixed freely in one call.  The bits of a row's
+ * output depend only on that request (co-batching changes nothing) and not on which physical
+ * pages hold its cache.  Contents of page slots >= kv_r never influence a result, NaN included.
+ *   q    : device bf16 [T, Hq, D], already rotated (sa_rope_kv_append's q_inout)
+ *   out  : device bf16 [T, Hq, D]
+ *   lse  : device f32 [T, Hq], nullable; natural-log sum-exp of the scaled scores of the row
+ *   sm_scale <= 0 selects 1/sqrt(D)
+ *   workspace : device, >= sa_mixed_attention_workspace_bytes(...) for the same batch */
+SA_API int32_t sa_mixed_attention_workspace_bytes(const sa_kv_pool *pool, int32_t n_req,
+                                           const int32_t *sids, const int32_t *qo_indptr,
+                                           size_t *out_bytes);
+SA_API int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                           const int32_t *qo_indptr, const void *q, void *out, float *lse,
+                           float sm_scale, void *workspace, size_t workspace_bytes, void *stream);
+
+/* Host-side planner statistics of the batch sa_mixed_attention would run (no device work; works
+ * on host-only pools).  out_stats (host int64[8]) = { decode-like requests, prefill requests,
+ * decode CTAs, prefill CTAs, split partial rows, sum_j L_j over decode-like requests,
+ * sum_j A_j over prefill requests (A_j = q_j*prefix_j + q_j(q_j+1)/2, L313), 1 if prefill chunks
+ * run on the tcgen05 kernel else 0 }. */
+SA_API int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                const int32_t *qo_indptr, int64_t *out_stats);
+
+/* Number of kernel launches the last successful sa_mixed_attention / sa_rope_kv_append on this
+ * pool enqueued (for launch accounting in benchmarks). */
+SA_API int32_t sa_last_launch_count(const sa_kv_pool *pool, int32_t *out_launches);
+
+/* ---- sa_latency_table: device-level latency model input (step a7) -------------------------
+ * Measures the time of one sa_mixed_attention call for every (prefill_tokens[a],
+ * decode_batch[b]) pair: the profiled attention terms of Eq. 1 (L305-319, L349-353; "offline-
+ * profiled", L303).  Prefill tokens p are issued as ceil(p/2048) chunks of <= 2048 tokens, each
+ * over its own prefix of prefill_prefix_len tokens; decode rows have contexts drawn uniformly
+ * from [decode_ctx_lo, decode_ctx_hi] with a counter-based generator seeded by seed.
+ * NOT a hot call: it opens scratch sessions in the pool's free pages, allocates its own
+ * temporary device buffers (cudaMalloc), synchronises the stream, and closes the sessions
+ * before returning.  Between timed iterations it evicts L2 by writing a 256 MiB buffer.
+ *   out_ms : host float [n_p][n_d], median over iters of CUDA-event times on `stream`
+ *   out_sum_kv (nullable): host int64 [n_p][n_d][2] = {sum_j L_j of the decode rows,
+ *                          sum_j A_j of the prefill chunks} for fitting alpha_d, alpha_p */
+SA_API int32_t sa_latency_table(sa_kv_pool *pool, const int32_t *prefill_tokens, int32_t n_p,
+                         const int32_t *decode_batch, int32_t n_d, int64_t prefill_prefix_len,
+                         int64_t decode_ctx_lo, int64_t decode_ctx_hi, uint64_t seed,
+                         int32_t warmup, int32_t iters, float *out_ms, int64_t *out_sum_kv,
+                         void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SMOOTHAGENT_H_ */

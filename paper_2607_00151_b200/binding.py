@@ -1,0 +1,299 @@
+"""ctypes binding of libsmoothagent.so: the same names as include/smoothagent.h, argument
+marshalling only.  Every step of the path runs in the library's CUDA kernels; torch is used for
+device memory and streams.  There is no fallback: if the library is missing or a call fails, an
+exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsmoothagent.so")
+
+SA_OK = 0
+SA_ERR_INVALID_ARG = -1
+SA_ERR_OUT_OF_PAGES = -2
+SA_ERR_UNSUPPORTED = -3
+SA_ERR_CUDA = -4
+SA_ERR_WORKSPACE_TOO_SMALL = -5
+SA_ERR_OUT_OF_SESSIONS = -6
+
+
+class SAError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s failed: %s (%d)" % (where, sa_status_string(status), status))
+
+
+class sa_kv_pool_config(ctypes.Structure):
+    _fields_ = [
+        ("num_q_heads", ctypes.c_int32),
+        ("num_kv_heads", ctypes.c_int32),
+        ("head_dim", ctypes.c_int32),
+        ("page_size", ctypes.c_int32),
+        ("num_pages", ctypes.c_int64),
+        ("max_sessions", ctypes.c_int32),
+        ("device", ctypes.c_int32),
+        ("max_session_tokens", ctypes.c_int64),
+        ("rope_base", ctypes.c_double),
+    ]
+
+
+class sa_kv_layout(ctypes.Structure):
+    _fields_ = [
+        ("k_base", ctypes.c_void_p),
+        ("v_base", ctypes.c_void_p),
+        ("stride_page", ctypes.c_int64),
+        ("stride_head", ctypes.c_int64),
+        ("stride_slot", ctypes.c_int64),
+    ]
+
+
+_i32p = ctypes.POINTER(ctypes.c_int32)
+_i64p = ctypes.POINTER(ctypes.c_int64)
+_f32p = ctypes.POINTER(ctypes.c_float)
+_vp = ctypes.c_void_p
+
+# name -> (restype, argtypes); also the list the symbol test checks against the header
+PROTOTYPES = {
+    "sa_status_string": (ctypes.c_char_p, [ctypes.c_int32]),
+    "sa_kv_pool_storage_bytes": (ctypes.c_int32, [ctypes.POINTER(sa_kv_pool_config), ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_kv_pool_create": (ctypes.c_int32, [ctypes.POINTER(sa_kv_pool_config), _vp, ctypes.c_size_t, _i32p, ctypes.POINTER(_vp)]),
+    "sa_kv_pool_destroy": (ctypes.c_int32, [_vp]),
+    "sa_kv_pool_layout": (ctypes.c_int32, [_vp, ctypes.POINTER(sa_kv_layout)]),
+    "sa_kv_pool_free_pages": (ctypes.c_int32, [_vp, _i64p]),
+    "sa_kv_session_open": (ctypes.c_int32, [_vp, _i32p]),
+    "sa_kv_session_close": (ctypes.c_int32, [_vp, ctypes.c_int32]),
+    "sa_kv_session_truncate": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64]),
+    "sa_kv_session_query": (ctypes.c_int32, [_vp, ctypes.c_int32, _i64p, _i32p, _i32p]),
+    "sa_rope_kv_append": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _vp, _vp, _vp, _vp]),
+    "sa_mixed_attention_workspace_bytes": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_mixed_attention": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _vp, _vp, _vp, ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
+    "sa_mixed_attention_plan": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _i64p]),
+    "sa_last_launch_count": (ctypes.c_int32, [_vp, _i32p]),
+    "sa_latency_table": (ctypes.c_int32, [_vp, _i32p, ctypes.c_int32, _i32p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
+                                          ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32, ctypes.c_int32, _f32p, _i64p, _vp]),
+}
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Load the in-tree library; fail loudly if it has not been built (no fallback path exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                "%s is missing: build it with `python -m paper_2607_00151_b200.build` "
+                "(or __graft_entry__.build()); this package has no CPU or PyTorch fallback" % LIB_PATH)
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in PROTOTYPES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != SA_OK:
+        raise SAError(status, where)
+
+
+def _i32(a: Sequence[int]):
+    arr = np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+    return arr, arr.ctypes.data_as(_i32p)
+
+
+def _ptr(t) -> Optional[int]:
+    """Device (or host) pointer of a torch tensor / raw int / None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def sa_status_string(status: int) -> str:
+    return load_library().sa_status_string(int(status)).decode()
+
+
+@dataclass
+class PoolConfig:
+    num_q_heads: int
+    num_kv_heads: int
+    head_dim: int
+    page_size: int
+    num_pages: int
+    max_sessions: int
+    max_session_tokens: int
+    rope_base: float
+    device: int = 0
+
+    def to_c(self) -> sa_kv_pool_config:
+        return sa_kv_pool_config(self.num_q_heads, self.num_kv_heads, self.head_dim, self.page_size, self.num_pages,
+                                 self.max_sessions, self.device, self.max_session_tokens, self.rope_base)
+
+
+def sa_kv_pool_storage_bytes(cfg: PoolConfig) -> int:
+    out = ctypes.c_size_t(0)
+    c = cfg.to_c()
+    _check(load_library().sa_kv_pool_storage_bytes(ctypes.byref(c), ctypes.byref(out)), "sa_kv_pool_storage_bytes")
+    return int(out.value)
+
+
+class Pool:
+    """Handle of an sa_kv_pool plus the torch tensor that owns its device storage."""
+
+    def __init__(self, handle: int, cfg: PoolConfig, storage):
+        self.handle = handle
+        self.cfg = cfg
+        self.storage = storage
+
+    def __del__(self):
+        try:
+            if self.handle:
+                sa_kv_pool_destroy(self)
+        except Exception:
+            pass
+
+
+def sa_kv_pool_create(cfg: PoolConfig, storage=None, free_page_order=None, host_only: bool = False) -> Pool:
+    """storage: a uint8 CUDA tensor of >= sa_kv_pool_storage_bytes(cfg) bytes (allocated here with
+    torch.empty if None); host_only=True creates the metadata-only pool (no device needed)."""
+    lib = load_library()
+    c = cfg.to_c()
+    nbytes = sa_kv_pool_storage_bytes(cfg)
+    if host_only:
+        storage, sptr = None, None
+    else:
+        import torch
+        if storage is None:
+            storage = torch.empty(nbytes, dtype=torch.uint8, device="cuda:%d" % cfg.device)
+        assert storage.is_cuda and storage.numel() * storage.element_size() >= nbytes
+        sptr = storage.data_ptr()
+    order_keep, order_ptr = (None, None)
+    if free_page_order is not None:
+        order_keep, order_ptr = _i32(free_page_order)
+        assert order_keep.shape == (cfg.num_pages,)
+    out = _vp()
+    _check(lib.sa_kv_pool_create(ctypes.byref(c), sptr, nbytes if not host_only else 0, order_ptr, ctypes.byref(out)),
+           "sa_kv_pool_create")
+    return Pool(out.value, cfg, storage)
+
+
+def sa_kv_pool_destroy(pool: Pool) -> None:
+    h, pool.handle = pool.handle, None
+    if h:
+        _check(load_library().sa_kv_pool_destroy(h), "sa_kv_pool_destroy")
+
+
+def sa_kv_pool_layout(pool: Pool) -> sa_kv_layout:
+    out = sa_kv_layout()
+    _check(load_library().sa_kv_pool_layout(pool.handle, ctypes.byref(out)), "sa_kv_pool_layout")
+    return out
+
+
+def sa_kv_pool_free_pages(pool: Pool) -> int:
+    out = ctypes.c_int64(0)
+    _check(load_library().sa_kv_pool_free_pages(pool.handle, ctypes.byref(out)), "sa_kv_pool_free_pages")
+    return int(out.value)
+
+
+def sa_kv_session_open(pool: Pool) -> int:
+    out = ctypes.c_int32(-1)
+    _check(load_library().sa_kv_session_open(pool.handle, ctypes.byref(out)), "sa_kv_session_open")
+    return int(out.value)
+
+
+def sa_kv_session_close(pool: Pool, sid: int) -> None:
+    _check(load_library().sa_kv_session_close(pool.handle, sid), "sa_kv_session_close")
+
+
+def sa_kv_session_truncate(pool: Pool, sid: int, new_len: int) -> None:
+    _check(load_library().sa_kv_session_truncate(pool.handle, sid, new_len), "sa_kv_session_truncate")
+
+
+def sa_kv_session_query(pool: Pool, sid: int):
+    """-> (len, [page ids])"""
+    lib = load_library()
+    ln = ctypes.c_int64(0)
+    n = ctypes.c_int32(0)
+    _check(lib.sa_kv_session_query(pool.handle, sid, ctypes.byref(ln), None, ctypes.byref(n)), "sa_kv_session_query")
+    pages = np.zeros(max(int(n.value), 1), dtype=np.int32)
+    cap = ctypes.c_int32(int(n.value))
+    _check(lib.sa_kv_session_query(pool.handle, sid, None, pages.ctypes.data_as(_i32p), ctypes.byref(cap)), "sa_kv_session_query")
+    return int(ln.value), pages[: int(n.value)].tolist()
+
+
+def sa_rope_kv_append(pool: Pool, sids, qo_indptr, k, v, q_inout=None, stream=None) -> None:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    assert i_keep.shape[0] == s_keep.shape[0] + 1
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_rope_kv_append(pool.handle, s_keep.shape[0], s_ptr, i_ptr, _ptr(k), _ptr(v), _ptr(q_inout), sp),
+           "sa_rope_kv_append")
+
+
+def sa_mixed_attention_workspace_bytes(pool: Pool, sids, qo_indptr) -> int:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_mixed_attention_workspace_bytes(pool.handle, s_keep.shape[0], s_ptr, i_ptr, ctypes.byref(out)),
+           "sa_mixed_attention_workspace_bytes")
+    return int(out.value)
+
+
+def sa_mixed_attention(pool: Pool, sids, qo_indptr, q, out, lse=None, sm_scale: float = 0.0, workspace=None, stream=None) -> None:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    assert i_keep.shape[0] == s_keep.shape[0] + 1
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_mixed_attention(pool.handle, s_keep.shape[0], s_ptr, i_ptr, _ptr(q), _ptr(out), _ptr(lse),
+                                             float(sm_scale), _ptr(workspace), ws_bytes, sp), "sa_mixed_attention")
+
+
+def sa_mixed_attention_plan(pool: Pool, sids, qo_indptr) -> dict:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    st = np.zeros(8, dtype=np.int64)
+    _check(load_library().sa_mixed_attention_plan(pool.handle, s_keep.shape[0], s_ptr, i_ptr, st.ctypes.data_as(_i64p)),
+           "sa_mixed_attention_plan")
+    keys = ["decode_requests", "prefill_requests", "decode_ctas", "prefill_ctas", "partial_rows", "sum_decode_kv",
+            "sum_prefill_A", "tcgen05"]
+    return dict(zip(keys, (int(x) for x in st)))
+
+
+def sa_last_launch_count(pool: Pool) -> int:
+    out = ctypes.c_int32(0)
+    _check(load_library().sa_last_launch_count(pool.handle, ctypes.byref(out)), "sa_last_launch_count")
+    return int(out.value)
+
+
+def sa_latency_table(pool: Pool, prefill_tokens, decode_batch, prefill_prefix_len: int, decode_ctx_lo: int,
+                     decode_ctx_hi: int, seed: int = 0, warmup: int = 3, iters: int = 10, stream=None):
+    """-> (ms [n_p, n_d] float32, sums [n_p, n_d, 2] int64 = (sum L_j, sum A_j))"""
+    p_keep, p_ptr = _i32(prefill_tokens)
+    d_keep, d_ptr = _i32(decode_batch)
+    ms = np.zeros((p_keep.shape[0], d_keep.shape[0]), dtype=np.float32)
+    sums = np.zeros((p_keep.shape[0], d_keep.shape[0], 2), dtype=np.int64)
+    _check(load_library().sa_latency_table(pool.handle, p_ptr, p_keep.shape[0], d_ptr, d_keep.shape[0], prefill_prefix_len,
+                                           decode_ctx_lo, decode_ctx_hi, seed, warmup, iters, ms.ctypes.data_as(_f32p),
+                                           sums.ctypes.data_as(_i64p), _stream_ptr(stream)), "sa_latency_table")
+    return ms, sums

@@ -1,0 +1,273 @@
+// sa_append.cu -- sa_rope_kv_append: fused RoPE + scatter of new K/V into pool pages
+// ("KV cache construction that depends on the previously
+// transformed prefix").  HBM-bound: every byte is read once and written once, 128-bit accesses.
+#include <cuda_bf16.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "sa_internal.h"
+
+namespace sa {
+
+constexpr int kAppendTok = 4;       // tokens per CTA
+constexpr int kAppendThreads = 256;
+
+__device__ __forceinline__ void unpack8(const uint4 &u, float (&f)[8]) {
+    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        f[2 * i] = __uint_as_float(w[i] << 16);
+        f[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+    }
+}
+
+__device__ __forceinline__ uint4 pack8(const float (&f)[8]) {
+    uint32_t w[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        __nv_bfloat162 p = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);  // round-to-nearest-even
+        w[i] = *reinterpret_cast<uint32_t *>(&p);
+    }
+    return make_uint4(w[0], w[1], w[2], w[3]);
+}
+
+// New page ids of this call -> device block table.  One CTA per request that gained pages.
+__global__ void block_table_update_kernel(const ReqMeta *__restrict__ reqs, const int32_t *__restrict__ new_pages,
+                                          int32_t *__restrict__ block_table, int64_t mpps) {
+    const ReqMeta r = reqs[blockIdx.x];
+    int32_t *row = block_table + int64_t(r.sid) * mpps + r.part_begin;
+    for (int i = threadIdx.x; i < r.n_splits; i += blockDim.x) row[i] = new_pages[r.item_begin + i];
+}
+
+// Per token: (2*Hkv + Hq) heads, each D/16 "units" of two 16-byte vectors (dims [8j, 8j+8) and
+// [D/2+8j, D/2+8j+8)): K and Q units are rotated, V units are copied bit for bit.
+template <int D>
+__global__ void __launch_bounds__(kAppendThreads)
+rope_append_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t total_rows,
+                   const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
+                   __nv_bfloat16 *__restrict__ q, __nv_bfloat16 *__restrict__ k_base,
+                   __nv_bfloat16 *__restrict__ v_base, const int32_t *__restrict__ block_table, int64_t mpps,
+                   int32_t log2_page, int64_t stride_page, int64_t stride_head,
+                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
+    constexpr int HALF = D / 2;
+    constexpr int UPH = D / 16;  // units per head
+    __shared__ int64_t s_dst[kAppendTok];
+    __shared__ float2 s_cs[kAppendTok][HALF];
+    __shared__ int32_t s_pos[kAppendTok];
+
+    const int64_t t0 = int64_t(blockIdx.x) * kAppendTok;
+    const int n_tok = int(min(int64_t(kAppendTok), total_rows - t0));
+    const int tid = threadIdx.x;
+
+    if (tid < n_tok) {
+        const int64_t t = t0 + tid;
+        int lo = 0, hi = n_req - 1;  // last request with q_start <= t (empty requests never match last)
+        while (lo < hi) {
+            int mid = (lo + hi + 1) >> 1;
+            if (reqs[mid].q_start <= t) lo = mid; else hi = mid - 1;
+        }
+        const ReqMeta r = reqs[lo];
+        const int32_t pos = r.kv_len + int32_t(t - r.q_start);
+        const int32_t page = block_table[int64_t(r.sid) * mpps + (pos >> log2_page)];
+        const int32_t slot = pos & ((1 << log2_page) - 1);
+        s_pos[tid] = pos;
+        s_dst[tid] = int64_t(page) * stride_page + int64_t(slot) * D;
+    }
+    __syncthreads();
+    for (int e = tid; e < n_tok * HALF; e += kAppendThreads) {
+        const int tl = e / HALF, m = e % HALF;
+        const float2 u = rope_tab[m];
+        const float p = float(s_pos[tl]);          // exact: positions < 2^24
+        const float ph = p * u.x;
+        float pl = fmaf(p, u.x, -ph);              // exact error of the product
+        pl = fmaf(p, u.y, pl);
+        const float fr = (ph - rintf(ph)) + pl;    // turns, |fr| <= 0.5 (+ tiny)
+        float sn, cs;
+        sincospif(2.0f * fr, &sn, &cs);
+        s_cs[tl][m] = make_float2(cs, sn);
+    }
+    __syncthreads();
+
+    const int heads = 2 * Hkv + (q ? Hq : 0);
+    const int units_per_tok = heads * UPH;
+    const int total_units = n_tok * units_per_tok;
+    constexpr int U = 2;  // units in flight per thread
+    for (int base = tid; base < total_units; base += kAppendThreads * U) {
+        uint4 a[U], b[U];
+        __nv_bfloat16 *dst[U];
+        int tl_[U], j_[U];
+        bool rot[U], live[U];
+#pragma unroll
+        for (int i = 0; i < U; ++i) {
+            const int e = base + i * kAppendThreads;
+            live[i] = e < total_units;
+            if (!live[i]) continue;
+            const int tl = e / units_per_tok, u = e % units_per_tok;
+            const int hu = u / UPH, j = u % UPH;
+            const int64_t row = t0 + tl;
+            const __nv_bfloat16 *src;
+            if (hu < Hkv) {
+                src = k + (row * Hkv + hu) * D;
+                dst[i] = k_base + s_dst[tl] + int64_t(hu) * stride_head;
+                rot[i] = true;
+            } else if (hu < 2 * Hkv) {
+                src = v + (row * Hkv + (hu - Hkv)) * D;
+                dst[i] = v_base + s_dst[tl] + int64_t(hu - Hkv) * stride_head;
+                rot[i] = false;
+            } else {
+                __nv_bfloat16 *qp = q + (row * Hq + (hu - 2 * Hkv)) * D;
+                src = qp;
+                dst[i] = qp;
+                rot[i] = true;
+            }
+            tl_[i] = tl;
+            j_[i] = j;
+            a[i] = *reinterpret_cast<const uint4 *>(src + 8 * j);
+            b[i] = *reinterpret_cast<const uint4 *>(src + HALF + 8 * j);
+        }
+#pragma unroll
+        for (int i = 0; i < U; ++i) {
+            if (!live[i]) continue;
+            if (rot[i]) {
+                float x0[8], x1[8], y0[8], y1[8];
+                unpack8(a[i], x0);
+                unpack8(b[i], x1);
+#pragma unroll
+                for (int d = 0; d < 8; ++d) {
+                    const float2 c = s_cs[tl_[i]][8 * j_[i] + d];
+                    y0[d] = fmaf(x0[d], c.x, -(x1[d] * c.y));
+                    y1[d] = fmaf(x1[d], c.x, x0[d] * c.y);
+                }
+                a[i] = pack8(y0);
+                b[i] = pack8(y1);
+            }
+            *reinterpret_cast<uint4 *>(dst[i] + 8 * j_[i]) = a[i];
+            *reinterpret_cast<uint4 *>(dst[i] + HALF + 8 * j_[i]) = b[i];
+        }
+    }
+}
+
+cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
+                               int64_t total_rows, const void *k, const void *v, void *q,
+                               cudaStream_t stream, int32_t *launches) {
+    if (total_rows == 0) return cudaSuccess;
+    const unsigned grid = unsigned((total_rows + kAppendTok - 1) / kAppendTok);
+    auto kb = static_cast<__nv_bfloat16 *>(pool->k_base);
+    auto vb = static_cast<__nv_bfloat16 *>(pool->v_base);
+    if (pool->cfg.head_dim == 128)
+        rope_append_kernel<128><<<grid, kAppendThreads, 0, stream>>>(
+            reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
+            static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
+            pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
+            pool->cfg.num_kv_heads);
+    else
+        rope_append_kernel<64><<<grid, kAppendThreads, 0, stream>>>(
+            reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
+            static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
+            pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
+            pool->cfg.num_kv_heads);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+}  // namespace sa
+
+extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                     const int32_t *qo_indptr, const void *k, const void *v, void *q_inout,
+                                     void *stream_) {
+    using namespace sa;
+    if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
+    if (n_req == 0) {
+        pool->last_launches = 0;
+        return SA_OK;
+    }
+    if (!sids || !qo_indptr || qo_indptr[0] != 0 || n_req > pool->cfg.max_sessions) return SA_ERR_INVALID_ARG;
+    const int B = pool->cfg.page_size;
+    // ---- validate everything and size the page demand before touching any state
+    std::vector<char> seen(pool->sessions.size(), 0);
+    int64_t need_pages = 0;
+    for (int r = 0; r < n_req; ++r) {
+        const int32_t sid = sids[r];
+        if (sid < 0 || size_t(sid) >= pool->sessions.size() || !pool->sessions[size_t(sid)].open || seen[size_t(sid)])
+            return SA_ERR_INVALID_ARG;
+        seen[size_t(sid)] = 1;
+        const int64_t n = int64_t(qo_indptr[r + 1]) - qo_indptr[r];
+        if (n < 0) return SA_ERR_INVALID_ARG;
+        const Session &s = pool->sessions[size_t(sid)];
+        if (s.len + n > pool->cfg.max_session_tokens) return SA_ERR_INVALID_ARG;
+        need_pages += (s.len + n + B - 1) / B - int64_t(s.pages.size());
+    }
+    const int64_t total = qo_indptr[n_req];
+    if (need_pages > int64_t(pool->free_pages.size())) return SA_ERR_OUT_OF_PAGES;
+    if (!pool->host_only && total > 0 && (!k || !v)) return SA_ERR_INVALID_ARG;
+
+    char *mh = nullptr, *md = nullptr;
+    if (!pool->host_only) {
+        int32_t st = acquire_meta(pool, &mh, &md);
+        if (st != SA_OK) return st;
+    }
+    std::vector<ReqMeta> host_meta;  // host-only pools keep the same bookkeeping path
+    ReqMeta *meta = nullptr;
+    int32_t *page_list = nullptr;
+    std::vector<int32_t> host_pages;
+    if (pool->host_only) {
+        host_meta.resize(size_t(n_req));
+        host_pages.resize(size_t(need_pages) + 1);
+        meta = host_meta.data();
+        page_list = host_pages.data();
+    } else {
+        meta = reinterpret_cast<ReqMeta *>(mh);
+        page_list = reinterpret_cast<int32_t *>(mh + sizeof(ReqMeta) * size_t(n_req));
+    }
+    // ---- allocate pages (cannot fail any more) and build the metadata
+    int32_t n_list = 0, n_gain = 0;
+    std::vector<ReqMeta> gain;  // requests that gained pages, for the block-table update
+    for (int r = 0; r < n_req; ++r) {
+        Session &s = pool->sessions[size_t(sids[r])];
+        const int64_t n = int64_t(qo_indptr[r + 1]) - qo_indptr[r];
+        const int64_t want = (s.len + n + B - 1) / B;
+        ReqMeta m{};
+        m.sid = sids[r];
+        m.q_start = qo_indptr[r];
+        m.q_len = int32_t(n);
+        m.kv_len = int32_t(s.len);  // position of the request's first new token
+        m.item_begin = n_list;
+        m.part_begin = int32_t(s.pages.size());
+        while (int64_t(s.pages.size()) < want) {
+            const int32_t p = pool->free_pages.back();
+            pool->free_pages.pop_back();
+            s.pages.push_back(p);
+            page_list[n_list++] = p;
+        }
+        m.n_splits = n_list - m.item_begin;
+        meta[r] = m;
+        if (m.n_splits > 0) {
+            gain.push_back(m);
+            ++n_gain;
+        }
+        s.len += n;
+    }
+    pool->last_launches = 0;
+    if (pool->host_only) return SA_OK;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    // slab layout: [ReqMeta x n_req][new page ids x n_list][ReqMeta x n_gain]
+    size_t off_gain = sizeof(ReqMeta) * size_t(n_req) + sizeof(int32_t) * size_t(n_list);
+    off_gain = (off_gain + 15) / 16 * 16;
+    // (the slab is sized for 2 x max_sessions entries + num_pages ids, so this always fits)
+    if (n_gain > 0) memcpy(mh + off_gain, gain.data(), sizeof(ReqMeta) * size_t(n_gain));
+    const size_t bytes = n_gain > 0 ? off_gain + sizeof(ReqMeta) * size_t(n_gain) : off_gain;
+    if (commit_meta(pool, bytes, stream) != SA_OK) return SA_ERR_CUDA;
+    const ReqMeta *reqs_dev = reinterpret_cast<const ReqMeta *>(md);
+    const int32_t *pages_dev = reinterpret_cast<const int32_t *>(md + sizeof(ReqMeta) * size_t(n_req));
+    if (n_gain > 0) {
+        block_table_update_kernel<<<unsigned(n_gain), 128, 0, stream>>>(
+            reinterpret_cast<const ReqMeta *>(md + off_gain), pages_dev, pool->block_table, pool->max_pages_per_session);
+        ++pool->last_launches;
+    }
+    if (cudaGetLastError() != cudaSuccess) return SA_ERR_CUDA;
+    if (launch_rope_append(pool, reqs_dev, n_req, total, k, v, q_inout, stream, &pool->last_launches) != cudaSuccess)
+        return SA_ERR_CUDA;
+    return SA_OK;
+}

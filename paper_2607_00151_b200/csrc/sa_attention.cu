@@ -1,0 +1,163 @@
+// sa_attention.cu -- sa_mixed_attention: host-side batch planning and the
+// dispatch of a ragged batch of prefill chunks and decode rows to the kernels (steps a4-a6).
+// lookahead (BE) prefill chunks are co-batched with LC decode rows; L311-313
+// and L305 define what each row attends to.
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "sa_internal.h"
+
+namespace sa {
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct HostPlan {
+    AttnPlan plan;
+    std::vector<ReqMeta> dec, pre;
+    int64_t total_q = 0;
+    int64_t sum_decode_kv = 0;   // sum_j L_j over decode-like requests   (Eq. 1, alpha_d term)
+    int64_t sum_prefill_A = 0;   // sum_j A_j over prefill requests       (Eq. 1, alpha_p term)
+    bool use_tc5 = false;
+};
+
+// The split of a request depends only on that request (never on its batch), so co-batching
+// cannot change the bits of a row.
+int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
+                   HostPlan *hp) {
+    if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
+    if (n_req == 0) return SA_OK;
+    if (!sids || !qo_indptr || qo_indptr[0] != 0 || n_req > pool->cfg.max_sessions) return SA_ERR_INVALID_ARG;
+    const int G = pool->G, Hq = pool->cfg.num_q_heads, Hkv = pool->cfg.num_kv_heads;
+    hp->use_tc5 = tc5_supported(pool);
+    const int tile_m = hp->use_tc5 ? kTc5TileM : kLegacyTileM;
+    for (int r = 0; r < n_req; ++r) {
+        const int32_t sid = sids[r];
+        if (sid < 0 || size_t(sid) >= pool->sessions.size() || !pool->sessions[size_t(sid)].open) return SA_ERR_INVALID_ARG;
+        const int64_t n = int64_t(qo_indptr[r + 1]) - qo_indptr[r];
+        const int64_t kv = pool->sessions[size_t(sid)].len;
+        if (n < 0 || n > kv) return SA_ERR_INVALID_ARG;  // the request's own tokens must already be appended
+        if (n == 0) continue;
+        ReqMeta m{};
+        m.sid = sid;
+        m.q_start = qo_indptr[r];
+        m.q_len = int32_t(n);
+        m.kv_len = int32_t(kv);
+        if (n * G <= 16) {
+            m.n_splits = int32_t((kv + kDecodeSplitKeys - 1) / kDecodeSplitKeys);
+            hp->dec.push_back(m);
+            hp->sum_decode_kv += kv * n;
+        } else {
+            m.n_tiles = int32_t((n * G + tile_m - 1) / tile_m);
+            hp->pre.push_back(m);
+            hp->sum_prefill_A += n * (kv - n) + n * (n + 1) / 2;
+        }
+    }
+    hp->total_q = qo_indptr[n_req];
+    // prefill: longest context first (its tiles carry the most work)
+    std::stable_sort(hp->pre.begin(), hp->pre.end(),
+                     [](const ReqMeta &a, const ReqMeta &b) { return a.kv_len > b.kv_len; });
+    int64_t items = 0, parts = 0, rows = 0;
+    for (ReqMeta &m : hp->dec) {
+        m.item_begin = int32_t(items);
+        m.part_begin = int32_t(parts);
+        items += int64_t(Hkv) * m.n_splits;
+        parts += int64_t(m.n_splits) * m.q_len * Hq;
+        rows += int64_t(m.q_len) * Hq;
+    }
+    if (items > INT32_MAX || parts > INT32_MAX) return SA_ERR_UNSUPPORTED;
+    hp->plan.n_dec = int32_t(hp->dec.size());
+    hp->plan.dec_items = int32_t(items);
+    hp->plan.part_rows = parts;
+    hp->plan.dec_rows = rows;
+    items = 0;
+    for (ReqMeta &m : hp->pre) {
+        m.item_begin = int32_t(items);
+        items += int64_t(Hkv) * m.n_tiles;
+    }
+    if (items > INT32_MAX) return SA_ERR_UNSUPPORTED;
+    hp->plan.n_pre = int32_t(hp->pre.size());
+    hp->plan.pre_items = int32_t(items);
+    return SA_OK;
+}
+
+size_t workspace_need(const sa_kv_pool *pool, const HostPlan &hp) {
+    const size_t D = size_t(pool->cfg.head_dim);
+    return align_up(size_t(hp.plan.part_rows) * D * 4, 256) + align_up(size_t(hp.plan.part_rows) * 4, 256) + 256;
+}
+
+}  // namespace
+}  // namespace sa
+
+extern "C" int32_t sa_mixed_attention_workspace_bytes(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                                      const int32_t *qo_indptr, size_t *out_bytes) {
+    if (!out_bytes) return SA_ERR_INVALID_ARG;
+    sa::HostPlan hp;
+    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hp);
+    if (st != SA_OK) return st;
+    *out_bytes = sa::workspace_need(pool, hp);
+    return SA_OK;
+}
+
+extern "C" int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                           const int32_t *qo_indptr, int64_t *out_stats) {
+    if (!out_stats) return SA_ERR_INVALID_ARG;
+    sa::HostPlan hp;
+    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hp);
+    if (st != SA_OK) return st;
+    out_stats[0] = hp.plan.n_dec;
+    out_stats[1] = hp.plan.n_pre;
+    out_stats[2] = hp.plan.dec_items;
+    out_stats[3] = hp.plan.pre_items;
+    out_stats[4] = hp.plan.part_rows;
+    out_stats[5] = hp.sum_decode_kv;
+    out_stats[6] = hp.sum_prefill_A;
+    out_stats[7] = hp.use_tc5 ? 1 : 0;
+    return SA_OK;
+}
+
+extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
+                                      const void *q, void *out, float *lse, float sm_scale, void *workspace,
+                                      size_t workspace_bytes, void *stream_) {
+    using namespace sa;
+    HostPlan hp;
+    int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hp);
+    if (st != SA_OK) return st;
+    if (pool->host_only) return SA_ERR_CUDA;
+    pool->last_launches = 0;
+    if (hp.plan.n_dec + hp.plan.n_pre == 0) return SA_OK;
+    if (!q || !out) return SA_ERR_INVALID_ARG;
+    const size_t need = workspace_need(pool, hp);
+    if (hp.plan.part_rows > 0 && (!workspace || workspace_bytes < need)) return SA_ERR_WORKSPACE_TOO_SMALL;
+    if (!(sm_scale > 0.f)) sm_scale = 1.0f / sqrtf(float(pool->cfg.head_dim));
+
+    char *mh = nullptr, *md = nullptr;
+    st = acquire_meta(pool, &mh, &md);
+    if (st != SA_OK) return st;
+    const size_t dec_bytes = sizeof(ReqMeta) * hp.dec.size(), pre_bytes = sizeof(ReqMeta) * hp.pre.size();
+    if (dec_bytes) memcpy(mh, hp.dec.data(), dec_bytes);
+    if (pre_bytes) memcpy(mh + dec_bytes, hp.pre.data(), pre_bytes);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (commit_meta(pool, dec_bytes + pre_bytes, stream) != SA_OK) return SA_ERR_CUDA;
+    const ReqMeta *dec_dev = reinterpret_cast<const ReqMeta *>(md);
+    const ReqMeta *pre_dev = reinterpret_cast<const ReqMeta *>(md + dec_bytes);
+
+    // workspace carve-up: [partial O f32][partial lse f32]
+    uintptr_t w = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255);
+    float *part_o = reinterpret_cast<float *>(w);
+    float *part_lse = reinterpret_cast<float *>(w + align_up(size_t(hp.plan.part_rows) * size_t(pool->cfg.head_dim) * 4, 256));
+
+    // prefill first: it is the long pole; the decode kernel fills in behind it on the same stream
+    cudaError_t e;
+    if (hp.use_tc5)
+        e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.total_q, q, out, lse, sm_scale, stream, &pool->last_launches);
+    else
+        e = launch_flash_prefill_legacy(pool, pre_dev, hp.plan, q, out, lse, sm_scale, stream, &pool->last_launches);
+    if (e != cudaSuccess) return SA_ERR_CUDA;
+    e = launch_flash_decode(pool, dec_dev, hp.plan, q, out, lse, sm_scale, part_o, part_lse, stream, &pool->last_launches);
+    if (e != cudaSuccess) return SA_ERR_CUDA;
+    return SA_OK;
+}

@@ -1,0 +1,499 @@
+// sa_flash_mma.cu -- attention over paged KV on the warp-level tensor path (mma.sync m16n8k16):
+//   * decode-like rows (q_len * G <= 16): split-KV, HBM-bound.  One CTA per (request, kv head,
+//     1024-key split); the G query heads of the group are the M rows of the MMA so K/V are read
+//     once per group; 4 warps take 16 keys each of every 64-key tile; cp.async 3-stage ring of
+//     page-gathered tiles; deterministic merge of the splits ("a single query
+//     token that attends to its full KV cache of length L_j ... memory-bandwidth bound").
+//   * prefill chunks that the tcgen05 kernel does not take (head_dim 64, or no tcgen05 path):
+//     64 packed rows per CTA, flash-style online softmax.
+// Packed rows: row rho of a (request, kv head g) pair is (token rho / G, q head g*G + rho % G).
+#include <cuda_bf16.h>
+#include <math.h>
+
+#include "sa_internal.h"
+
+namespace sa {
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr int kBN = 64;      // keys per tile
+constexpr int kStages = 3;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void mma16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&p);
+}
+// byte offset of 16-byte chunk `chunk` of row `row` in a [rows][D] bf16 tile, XOR-swizzled
+template <int D>
+__device__ __forceinline__ uint32_t tile_off(int row, int chunk) {
+    return uint32_t(row * (D * 2) + ((chunk ^ (row & 7)) << 4));
+}
+
+struct KvView {
+    const __nv_bfloat16 *k_base, *v_base;
+    const int32_t *bt_row;  // block table row of the session
+    int64_t stride_page;
+    int64_t head_off;  // g * stride_head
+    int32_t log2_page;
+};
+
+// Gather one 64-key tile of K and V (logical keys kt .. kt+63) into swizzled smem; rows at or
+// beyond kv_len are zero-filled, so slots the session does not own never reach the math.
+template <int D>
+__device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_len, uint32_t sK, uint32_t sV, int tid) {
+    constexpr int CPR = D / 8;               // 16-byte chunks per row
+    constexpr int RPP = kThreads / CPR;      // rows per pass
+    const int chunk = tid % CPR;
+    const int r0 = tid / CPR;
+    const int pmask = (1 << kv.log2_page) - 1;
+#pragma unroll
+    for (int i = 0; i < kBN / RPP; ++i) {
+        const int row = r0 + i * RPP;
+        const int key = kt + row;
+        const bool valid = key < kv_len;
+        int64_t off = 0;
+        if (valid) {
+            const int32_t page = __ldg(kv.bt_row + (key >> kv.log2_page));
+            off = int64_t(page) * kv.stride_page + kv.head_off + int64_t(key & pmask) * D + chunk * 8;
+        }
+        const uint32_t so = tile_off<D>(row, chunk);
+        cp_async16(sK + so, kv.k_base + off, valid ? 16 : 0);
+        cp_async16(sV + so, kv.v_base + off, valid ? 16 : 0);
+    }
+}
+
+// One online-softmax step of a warp over NKG groups of 16 keys starting at tile row key_off.
+template <int D, int NKG>
+__device__ __forceinline__ void warp_step(const uint32_t (&qf)[D / 16][4], uint32_t sK, uint32_t sV, int key_off,
+                                          int kt_abs, int lim0, int lim1, bool need_mask, float scale_log2,
+                                          float (&o)[D / 8][4], float &m0, float &m1, float &l0, float &l1, int lane) {
+    float s[NKG * 2][4];
+#pragma unroll
+    for (int i = 0; i < NKG * 2; ++i) s[i][0] = s[i][1] = s[i][2] = s[i][3] = 0.f;
+    const int mi = lane >> 3, rr = lane & 7;
+#pragma unroll
+    for (int ks = 0; ks < D / 16; ++ks) {
+#pragma unroll
+        for (int kg = 0; kg < NKG; ++kg) {
+            const int krow = key_off + kg * 16 + (mi >> 1) * 8 + rr;
+            uint32_t b[4];
+            ldsm_x4(b, sK + tile_off<D>(krow, ks * 2 + (mi & 1)));
+            mma16816(s[kg * 2], qf[ks], b[0], b[1]);
+            mma16816(s[kg * 2 + 1], qf[ks], b[2], b[3]);
+        }
+    }
+    float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+    for (int nt = 0; nt < NKG * 2; ++nt) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            float v = s[nt][e] * scale_log2;
+            if (need_mask) {
+                const int pos = kt_abs + key_off + nt * 8 + 2 * (lane & 3) + (e & 1);
+                if (pos > (e < 2 ? lim0 : lim1)) v = -INFINITY;
+            }
+            s[nt][e] = v;
+            if (e < 2) mx0 = fmaxf(mx0, v); else mx1 = fmaxf(mx1, v);
+        }
+    }
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+    const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+    const float b0 = (mn0 == -INFINITY) ? 0.f : mn0, b1 = (mn1 == -INFINITY) ? 0.f : mn1;
+    const float c0 = exp2f(m0 - b0), c1 = exp2f(m1 - b1);
+    m0 = mn0;
+    m1 = mn1;
+    float rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < NKG * 2; ++nt) {
+        s[nt][0] = exp2f(s[nt][0] - b0);
+        s[nt][1] = exp2f(s[nt][1] - b0);
+        s[nt][2] = exp2f(s[nt][2] - b1);
+        s[nt][3] = exp2f(s[nt][3] - b1);
+        rs0 += s[nt][0] + s[nt][1];
+        rs1 += s[nt][2] + s[nt][3];
+    }
+    l0 = l0 * c0 + rs0;  // per-thread partial sums; reduced across the quad at the end
+    l1 = l1 * c1 + rs1;
+#pragma unroll
+    for (int nt = 0; nt < D / 8; ++nt) {
+        o[nt][0] *= c0;
+        o[nt][1] *= c0;
+        o[nt][2] *= c1;
+        o[nt][3] *= c1;
+    }
+#pragma unroll
+    for (int kg = 0; kg < NKG; ++kg) {
+        uint32_t a[4];
+        a[0] = pack_bf16(s[kg * 2][0], s[kg * 2][1]);
+        a[1] = pack_bf16(s[kg * 2][2], s[kg * 2][3]);
+        a[2] = pack_bf16(s[kg * 2 + 1][0], s[kg * 2 + 1][1]);
+        a[3] = pack_bf16(s[kg * 2 + 1][2], s[kg * 2 + 1][3]);
+        const int vrow = key_off + kg * 16 + (mi & 1) * 8 + rr;
+#pragma unroll
+        for (int np = 0; np < D / 16; ++np) {
+            uint32_t b[4];
+            ldsm_x4_t(b, sV + tile_off<D>(vrow, np * 2 + (mi >> 1)));
+            mma16816(o[np * 2], a, b[0], b[1]);
+            mma16816(o[np * 2 + 1], a, b[2], b[3]);
+        }
+    }
+}
+
+__device__ __forceinline__ int find_req(const ReqMeta *reqs, int n, int item) {
+    int lo = 0, hi = n - 1;  // last request with item_begin <= item (requests with no items never match last)
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (reqs[mid].item_begin <= item) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+struct AttnArgs {
+    const ReqMeta *reqs;
+    int32_t n_reqs;
+    const __nv_bfloat16 *q;
+    __nv_bfloat16 *out;
+    float *lse;
+    float *part_o;
+    float *part_lse;
+    const __nv_bfloat16 *k_base, *v_base;
+    const int32_t *block_table;
+    int64_t mpps, stride_page, stride_head;
+    int32_t log2_page, Hq, Hkv, log2G;
+    float scale_log2;
+};
+
+// Load BM packed rows of Q (row base rho0) into swizzled smem; rows beyond n_rows are zero.
+template <int D, int BM>
+__device__ __forceinline__ void load_q_tile(const AttnArgs &a, const ReqMeta &r, int g, int rho0, int n_rows,
+                                            uint32_t sQ, int tid) {
+    constexpr int CPR = D / 8;
+    for (int e = tid; e < BM * CPR; e += kThreads) {
+        const int row = e / CPR, chunk = e % CPR;
+        const int rho = rho0 + row;
+        uint4 val = make_uint4(0, 0, 0, 0);
+        if (rho < n_rows) {
+            const int tok = rho >> a.log2G, hq = (g << a.log2G) + (rho & ((1 << a.log2G) - 1));
+            val = *reinterpret_cast<const uint4 *>(a.q + (int64_t(r.q_start + tok) * a.Hq + hq) * D + chunk * 8);
+        }
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(sQ + tile_off<D>(row, chunk)), "r"(val.x),
+                     "r"(val.y), "r"(val.z), "r"(val.w) : "memory");
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// MODE 0: decode-like, split-KV, partials out.   MODE 1: prefill, 64 packed rows, direct out.
+template <int D, int MODE>
+__global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int BM = MODE == 0 ? 16 : kLegacyTileM;
+    constexpr int TILE_BYTES = kBN * D * 2;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t s_base = smem_u32(smem);
+    const uint32_t sQ = s_base + kStages * 2 * TILE_BYTES;
+
+    const int item = blockIdx.x;
+    const int ri = find_req(a.reqs, a.n_reqs, item);
+    const ReqMeta r = a.reqs[ri];
+    const int local = item - r.item_begin;
+    const int G = 1 << a.log2G;
+    const int n_rows = r.q_len * G;
+    int g, rho0, k_begin, k_end, split = 0;
+    if (MODE == 0) {
+        g = local / r.n_splits;
+        split = local % r.n_splits;
+        rho0 = 0;
+        k_begin = split * kDecodeSplitKeys;
+        k_end = min(r.kv_len, k_begin + kDecodeSplitKeys);
+    } else {
+        const int tile = r.n_tiles - 1 - local / a.Hkv;  // heavy (late) tiles first
+        g = local % a.Hkv;
+        rho0 = tile * BM;
+        k_begin = 0;
+        const int tok_max = min(r.q_len - 1, (rho0 + BM - 1) >> a.log2G);
+        k_end = r.kv_len - r.q_len + tok_max + 1;
+    }
+    KvView kv;
+    kv.k_base = a.k_base;
+    kv.v_base = a.v_base;
+    kv.bt_row = a.block_table + int64_t(r.sid) * a.mpps;
+    kv.stride_page = a.stride_page;
+    kv.head_off = int64_t(g) * a.stride_head;
+    kv.log2_page = a.log2_page;
+
+    const int n_tiles = (k_end - k_begin + kBN - 1) / kBN;
+    // prologue of the cp.async ring
+#pragma unroll
+    for (int s = 0; s < kStages - 1; ++s) {
+        if (s < n_tiles)
+            load_kv_tile<D>(kv, k_begin + s * kBN, r.kv_len, s_base + s * 2 * TILE_BYTES,
+                            s_base + s * 2 * TILE_BYTES + TILE_BYTES, tid);
+        cp_async_commit();
+    }
+    load_q_tile<D, BM>(a, r, g, rho0, n_rows, sQ, tid);
+    __syncthreads();
+    const int row_base = MODE == 0 ? 0 : warp * 16;
+    uint32_t qf[D / 16][4];
+    {
+        const int mi = lane >> 3, rr = lane & 7;
+#pragma unroll
+        for (int ks = 0; ks < D / 16; ++ks)
+            ldsm_x4(qf[ks], sQ + tile_off<D>(row_base + (mi & 1) * 8 + rr, ks * 2 + (mi >> 1)));
+    }
+    // causal limits (inclusive last key) of this thread's two rows
+    const int rA = rho0 + row_base + (lane >> 2), rB = rA + 8;
+    const int base_lim = r.kv_len - r.q_len;
+    const int lim0 = rA < n_rows ? base_lim + (rA >> a.log2G) : -1;
+    const int lim1 = rB < n_rows ? base_lim + (rB >> a.log2G) : -1;
+    // smallest limit among this warp's rows (warp-uniform): tiles entirely at or below it need no mask
+    const int warp_rows_lo = rho0 + row_base;
+    const int lim_min = (warp_rows_lo + 15 < n_rows) ? base_lim + (warp_rows_lo >> a.log2G) : -1;
+
+    float o[D / 8][4];
+#pragma unroll
+    for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+
+    for (int t = 0; t < n_tiles; ++t) {
+        cp_async_wait<kStages - 2>();
+        __syncthreads();
+        {
+            const int tn = t + kStages - 1;
+            if (tn < n_tiles) {
+                const int sn = tn % kStages;
+                load_kv_tile<D>(kv, k_begin + tn * kBN, r.kv_len, s_base + sn * 2 * TILE_BYTES,
+                                s_base + sn * 2 * TILE_BYTES + TILE_BYTES, tid);
+            }
+            cp_async_commit();
+        }
+        const int st = t % kStages;
+        const uint32_t sK = s_base + st * 2 * TILE_BYTES, sV = sK + TILE_BYTES;
+        const int kt = k_begin + t * kBN;
+        if (MODE == 0) {
+            const int key_off = warp * 16;
+            if (kt + key_off < k_end) {  // warp-uniform: this warp's 16 keys hold at least one live key
+                const bool need_mask = kt + key_off + 15 > lim_min;
+                warp_step<D, 1>(qf, sK, sV, key_off, kt, lim0, lim1, need_mask, a.scale_log2, o, m0, m1, l0, l1, lane);
+            }
+        } else {
+            const bool need_mask = kt + kBN - 1 > lim_min;
+            warp_step<D, 4>(qf, sK, sV, 0, kt, lim0, lim1, need_mask, a.scale_log2, o, m0, m1, l0, l1, lane);
+        }
+    }
+    cp_async_wait<0>();
+    l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+    l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+    l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+    l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+
+    if (MODE == 1) {
+        const float inv0 = l0 > 0.f ? 1.f / l0 : 0.f, inv1 = l1 > 0.f ? 1.f / l1 : 0.f;
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const int rho = half ? rB : rA;
+            if (rho >= n_rows) continue;
+            const int tok = rho >> a.log2G, hq = (g << a.log2G) + (rho & (G - 1));
+            const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+            __nv_bfloat16 *op = a.out + orow * D + 2 * (lane & 3);
+            const float inv = half ? inv1 : inv0;
+#pragma unroll
+            for (int nt = 0; nt < D / 8; ++nt)
+                *reinterpret_cast<uint32_t *>(op + nt * 8) = pack_bf16(o[nt][half * 2] * inv, o[nt][half * 2 + 1] * inv);
+            if (a.lse && (lane & 3) == 0) {
+                const float m = half ? m1 : m0, l = half ? l1 : l0;
+                a.lse[orow] = (m + log2f(l)) * 0.6931471805599453f;
+            }
+        }
+        return;
+    }
+
+    // ---- MODE 0: merge the four warps' states (each saw a disjoint quarter of every tile)
+    __syncthreads();  // everyone is done with the stage buffers
+    float *sO = reinterpret_cast<float *>(smem);             // [4][16][D]
+    float *sM = sO + 4 * 16 * D;                             // [4][16]
+    float *sL = sM + 4 * 16;                                 // [4][16]
+    {
+        const int r0 = lane >> 2, r1 = r0 + 8;
+        float *wo = sO + warp * 16 * D;
+#pragma unroll
+        for (int nt = 0; nt < D / 8; ++nt) {
+            const int col = nt * 8 + 2 * (lane & 3);
+            *reinterpret_cast<float2 *>(wo + r0 * D + col) = make_float2(o[nt][0], o[nt][1]);
+            *reinterpret_cast<float2 *>(wo + r1 * D + col) = make_float2(o[nt][2], o[nt][3]);
+        }
+        if ((lane & 3) == 0) {
+            sM[warp * 16 + r0] = m0;
+            sM[warp * 16 + r1] = m1;
+            sL[warp * 16 + r0] = l0;
+            sL[warp * 16 + r1] = l1;
+        }
+    }
+    __syncthreads();
+    for (int e = tid; e < n_rows * (D / 4); e += kThreads) {
+        const int row = e / (D / 4), c4 = e % (D / 4);
+        float M = -INFINITY;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) M = fmaxf(M, sM[w * 16 + row]);
+        const float Mb = (M == -INFINITY) ? 0.f : M;
+        float L = 0.f;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {  // fixed order: bit-reproducible
+            const float wgt = exp2f(sM[w * 16 + row] - Mb);
+            L += sL[w * 16 + row] * wgt;
+            const float4 ov = *reinterpret_cast<const float4 *>(sO + (w * 16 + row) * D + c4 * 4);
+            acc.x += ov.x * wgt;
+            acc.y += ov.y * wgt;
+            acc.z += ov.z * wgt;
+            acc.w += ov.w * wgt;
+        }
+        const float inv = L > 0.f ? 1.f / L : 0.f;
+        const int tok = row >> a.log2G, hq = (g << a.log2G) + (row & (G - 1));
+        const int64_t prow = int64_t(r.part_begin) + (int64_t(split) * r.q_len + tok) * a.Hq + hq;
+        *reinterpret_cast<float4 *>(a.part_o + prow * D + c4 * 4) = make_float4(acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv);
+        if (c4 == 0) a.part_lse[prow] = L > 0.f ? M + log2f(L) : -INFINITY;  // log2 domain
+    }
+}
+
+// Merge of the split partials, fixed split order.  grid = (decode-like requests, Hkv); each warp
+// takes packed rows of the group; lanes cover D with float4.
+template <int D>
+__global__ void __launch_bounds__(128) merge_splits_kernel(const AttnArgs a) {
+    const ReqMeta r = a.reqs[blockIdx.x];
+    const int g = blockIdx.y;
+    const int G = 1 << a.log2G;
+    const int n_rows = r.q_len * G;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int LANES = D / 4;
+    for (int row = warp; row < n_rows; row += 4) {
+        const int tok = row >> a.log2G, hq = (g << a.log2G) + (row & (G - 1));
+        const int64_t p0 = int64_t(r.part_begin) + int64_t(tok) * a.Hq + hq;
+        const int64_t pstride = int64_t(r.q_len) * a.Hq;
+        float M = -INFINITY;
+        for (int s = 0; s < r.n_splits; ++s) M = fmaxf(M, a.part_lse[p0 + s * pstride]);
+        const float Mb = (M == -INFINITY) ? 0.f : M;
+        float W = 0.f;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int s = 0; s < r.n_splits; ++s) {
+            const float w = exp2f(a.part_lse[p0 + s * pstride] - Mb);
+            W += w;
+            if (lane < LANES) {
+                const float4 ov = *reinterpret_cast<const float4 *>(a.part_o + (p0 + s * pstride) * D + lane * 4);
+                acc.x += ov.x * w;
+                acc.y += ov.y * w;
+                acc.z += ov.z * w;
+                acc.w += ov.w * w;
+            }
+        }
+        const float inv = W > 0.f ? 1.f / W : 0.f;
+        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+        if (lane < LANES) {
+            uint2 pk;
+            pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+            pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+            *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
+        }
+        if (a.lse && lane == 0) a.lse[orow] = (M + log2f(W)) * 0.6931471805599453f;
+    }
+}
+
+AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const void *q, void *out, float *lse,
+                   float sm_scale, float *part_o, float *part_lse) {
+    AttnArgs a;
+    a.reqs = reqs;
+    a.n_reqs = n;
+    a.q = static_cast<const __nv_bfloat16 *>(q);
+    a.out = static_cast<__nv_bfloat16 *>(out);
+    a.lse = lse;
+    a.part_o = part_o;
+    a.part_lse = part_lse;
+    a.k_base = static_cast<const __nv_bfloat16 *>(pool->k_base);
+    a.v_base = static_cast<const __nv_bfloat16 *>(pool->v_base);
+    a.block_table = pool->block_table;
+    a.mpps = pool->max_pages_per_session;
+    a.stride_page = pool->stride_page;
+    a.stride_head = pool->stride_head;
+    a.log2_page = pool->log2_page;
+    a.Hq = pool->cfg.num_q_heads;
+    a.Hkv = pool->cfg.num_kv_heads;
+    int lg = 0;
+    while ((1 << lg) < pool->G) ++lg;
+    a.log2G = lg;
+    a.scale_log2 = sm_scale * 1.4426950408889634f;
+    return a;
+}
+
+template <int D, int MODE>
+cudaError_t launch_flash(const AttnArgs &a, int items, cudaStream_t stream) {
+    constexpr int BM = MODE == 0 ? 16 : kLegacyTileM;
+    constexpr size_t smem = size_t(kStages) * 2 * kBN * D * 2 + size_t(BM) * D * 2;
+    static_assert(smem >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(flash_mma_kernel<D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    flash_mma_kernel<D, MODE><<<unsigned(items), kThreads, smem, stream>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
+                                const void *q, void *out, float *lse, float sm_scale, float *part_o,
+                                float *part_lse, cudaStream_t stream, int32_t *launches) {
+    if (plan.dec_items == 0) return cudaSuccess;
+    AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
+    cudaError_t e = pool->cfg.head_dim == 128 ? launch_flash<128, 0>(a, plan.dec_items, stream)
+                                              : launch_flash<64, 0>(a, plan.dec_items, stream);
+    if (e != cudaSuccess) return e;
+    ++*launches;
+    dim3 grid(unsigned(plan.n_dec), unsigned(pool->cfg.num_kv_heads));
+    if (pool->cfg.head_dim == 128) merge_splits_kernel<128><<<grid, 128, 0, stream>>>(a);
+    else merge_splits_kernel<64><<<grid, 128, 0, stream>>>(a);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_flash_prefill_legacy(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
+                                        const void *q, void *out, float *lse, float sm_scale, cudaStream_t stream,
+                                        int32_t *launches) {
+    if (plan.pre_items == 0) return cudaSuccess;
+    AttnArgs a = make_args(pool, reqs_dev, plan.n_pre, q, out, lse, sm_scale, nullptr, nullptr);
+    cudaError_t e = pool->cfg.head_dim == 128 ? launch_flash<128, 1>(a, plan.pre_items, stream)
+                                              : launch_flash<64, 1>(a, plan.pre_items, stream);
+    if (e == cudaSuccess) ++*launches;
+    return e;
+}
+
+}  // namespace sa

@@ -1,0 +1,200 @@
+"""Drives a Workload through the C-ABI calls (binding.py): open sessions, fill the retained
+prefixes, then -- one "step" of the hot path -- drop the invalidated tail, and re-prefill the
+transformed segments chunk by chunk (sa_rope_kv_append + sa_mixed_attention) co-batched with the
+decode rows.  Orchestration only: all arithmetic happens inside libsmoothagent.so.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Dict, List, Optional
+
+import numpy as np
+import torch
+
+from . import binding as sa
+from .workloads import Workload, gen_session
+
+
+@dataclass
+class Round:
+    sids: List[int]
+    idx: List[int]            # workload session index of each request
+    starts: List[int]         # offset of the request's rows inside its session's new tokens
+    indptr: np.ndarray        # int32 [n+1]
+    k: torch.Tensor
+    v: torch.Tensor
+    q_raw: torch.Tensor
+    q: torch.Tensor           # rotated in place by the append
+    out: torch.Tensor
+    lse: torch.Tensor
+    workspace: Optional[torch.Tensor] = None
+
+
+def make_pool(w: Workload, device: int = 0, page_order="random", sentinel: Optional[int] = None,
+              max_sessions: Optional[int] = None, num_pages: Optional[int] = None) -> sa.Pool:
+    """page_order: "random" (the workload's seeded permutation), "identity", or an int32 array.
+    sentinel: 16-bit pattern written over the whole storage before the pool is created."""
+    L = w.layer
+    cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, num_pages or w.num_pages,
+                        max_sessions or (len(w.sessions) + 4), max(w.max_session_tokens, L.page_size), L.rope_base, device)
+    nbytes = sa.sa_kv_pool_storage_bytes(cfg)
+    storage = torch.empty(nbytes, dtype=torch.uint8, device="cuda:%d" % device)
+    if sentinel is not None:
+        storage.view(torch.int16)[: nbytes // 2].fill_(np.array(sentinel, dtype=np.uint16).view(np.int16).item())
+    if isinstance(page_order, str):
+        order = w.page_order() if page_order == "random" else None
+        if num_pages and order is not None:
+            order = np.random.default_rng(w.seed + 7919).permutation(num_pages).astype(np.int32)
+    else:
+        order = page_order
+    return sa.sa_kv_pool_create(cfg, storage, order)
+
+
+class Runner:
+    def __init__(self, w: Workload, pool: sa.Pool, data: Optional[Dict[int, tuple]] = None, device: int = 0,
+                 scale: Optional[float] = None, want_lse: bool = True):
+        self.w, self.pool, self.device = w, pool, device
+        self.dev = torch.device("cuda:%d" % device)
+        self.data = data if data is not None else {i: gen_session(w, i, self.dev, scale) for i in range(len(w.sessions))}
+        self.want_lse = want_lse
+        self.sids = [sa.sa_kv_session_open(pool) for _ in w.sessions]
+        self.rounds: List[Round] = []
+        self.launches_per_step = 0
+        self._build_rounds()
+
+    # -- retained prefixes -------------------------------------------------------------------
+    def fill_prefixes(self, max_tokens_per_call: int = 1 << 20) -> int:
+        """Append every session's retained prefix (K/V only).  Returns tokens appended."""
+        total = 0
+        batch_s, batch_k, batch_v, lens = [], [], [], []
+
+        def flush():
+            nonlocal batch_s, batch_k, batch_v, lens
+            if not batch_s:
+                return
+            indptr = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+            k = torch.cat(batch_k) if len(batch_k) > 1 else batch_k[0].contiguous()
+            v = torch.cat(batch_v) if len(batch_v) > 1 else batch_v[0].contiguous()
+            sa.sa_rope_kv_append(self.pool, batch_s, indptr, k, v, None)
+            batch_s, batch_k, batch_v, lens = [], [], [], []
+
+        for i, s in enumerate(self.w.sessions):
+            if s.prefix == 0:
+                continue
+            k, v, _ = self.data[i]
+            if sum(lens) + s.prefix > max_tokens_per_call:
+                flush()
+            batch_s.append(self.sids[i])
+            batch_k.append(k[: s.prefix])
+            batch_v.append(v[: s.prefix])
+            lens.append(s.prefix)
+            total += s.prefix
+        flush()
+        return total
+
+    # -- the step ----------------------------------------------------------------------------
+    def _build_rounds(self):
+        w = self.w
+        L = w.layer
+        n_rounds = max(1, max((s.new + (s.chunk or s.new) - 1) // max(s.chunk or s.new, 1) for s in w.sessions))
+        for c in range(n_rounds):
+            sids, idx, starts, lens, ks, vs, qs = [], [], [], [], [], [], []
+            for i, s in enumerate(w.sessions):
+                ch = s.chunk or s.new
+                a, b = c * ch, min(s.new, (c + 1) * ch)
+                if a >= b:
+                    continue
+                k, v, q = self.data[i]
+                sids.append(self.sids[i])
+                idx.append(i)
+                starts.append(a)
+                lens.append(b - a)
+                ks.append(k[s.prefix + a: s.prefix + b])
+                vs.append(v[s.prefix + a: s.prefix + b])
+                qs.append(q[a:b])
+            if not sids:
+                continue
+            indptr = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+            T = int(indptr[-1])
+            q_raw = torch.cat(qs).contiguous()
+            self.rounds.append(Round(
+                sids, idx, starts, indptr, torch.cat(ks).contiguous(), torch.cat(vs).contiguous(), q_raw,
+                torch.empty_like(q_raw), torch.empty_like(q_raw),
+                torch.empty((T, L.num_q_heads), dtype=torch.float32, device=self.dev)))
+
+    def truncate_to_prefix(self):
+        """The context transformation invalidates everything after the retained prefix (L37)."""
+        for i, s in enumerate(self.w.sessions):
+            sa.sa_kv_session_truncate(self.pool, self.sids[i], s.prefix)
+
+    def step(self, attention: bool = True, append: bool = True):
+        """One pass of the hot path: for every chunk round, RoPE+append then mixed attention."""
+        launches = 0
+        self.truncate_to_prefix()
+        for r in self.rounds:
+            if append:
+                r.q.copy_(r.q_raw)
+                sa.sa_rope_kv_append(self.pool, r.sids, r.indptr, r.k, r.v, r.q)
+                launches += sa.sa_last_launch_count(self.pool) + 1
+            if attention:
+                if r.workspace is None:
+                    nb = sa.sa_mixed_attention_workspace_bytes(self.pool, r.sids, r.indptr)
+                    r.workspace = torch.empty(max(nb, 256), dtype=torch.uint8, device=self.dev)
+                sa.sa_mixed_attention(self.pool, r.sids, r.indptr, r.q, r.out, r.lse if self.want_lse else None,
+                                      0.0, r.workspace)
+                launches += sa.sa_last_launch_count(self.pool)
+        self.launches_per_step = launches
+
+    # -- results -----------------------------------------------------------------------------
+    def outputs(self):
+        """Per workload session: out bf16 [new, Hq, D], lse f32 [new, Hq], q_rot bf16 (device tensors)."""
+        res = {}
+        for i, s in enumerate(self.w.sessions):
+            L = self.w.layer
+            o = torch.empty((s.new, L.num_q_heads, L.head_dim), dtype=torch.bfloat16, device=self.dev)
+            l = torch.empty((s.new, L.num_q_heads), dtype=torch.float32, device=self.dev)
+            qr = torch.empty_like(o)
+            res[i] = (o, l, qr)
+        for r in self.rounds:
+            for j, i in enumerate(r.idx):
+                a, b = int(r.indptr[j]), int(r.indptr[j + 1])
+                st = r.starts[j]
+                res[i][0][st: st + b - a] = r.out[a:b]
+                res[i][1][st: st + b - a] = r.lse[a:b]
+                res[i][2][st: st + b - a] = r.q[a:b]
+        return res
+
+    def gather_kv(self, i: int, upto: Optional[int] = None):
+        """Read session i's K', V back through its block table: bf16 [len, Hkv, D] each."""
+        ln, pages = sa.sa_kv_session_query(self.pool, self.sids[i])
+        if upto is not None:
+            ln = min(ln, upto)
+        return gather_kv(self.pool, pages, ln)
+
+    def close(self):
+        for sid in self.sids:
+            sa.sa_kv_session_close(self.pool, sid)
+        self.sids = []
+
+
+def pool_views(pool: sa.Pool):
+    """K and V page arrays as bf16 views [num_pages, Hkv, B, D] of the pool storage."""
+    cfg = pool.cfg
+    lay = sa.sa_kv_pool_layout(pool)
+    base = pool.storage.data_ptr()
+    n = cfg.num_pages * cfg.num_kv_heads * cfg.page_size * cfg.head_dim
+    flat = pool.storage.view(torch.bfloat16)
+    ko, vo = (lay.k_base - base) // 2, (lay.v_base - base) // 2
+    shape = (cfg.num_pages, cfg.num_kv_heads, cfg.page_size, cfg.head_dim)
+    assert lay.stride_page == cfg.num_kv_heads * cfg.page_size * cfg.head_dim
+    return flat[ko: ko + n].view(shape), flat[vo: vo + n].view(shape)
+
+
+def gather_kv(pool: sa.Pool, pages: List[int], length: int):
+    kp, vp = pool_views(pool)
+    B = pool.cfg.page_size
+    n_pages = (length + B - 1) // B
+    idx = torch.as_tensor(pages[:n_pages], dtype=torch.long, device=kp.device)
+    k = kp[idx].permute(0, 2, 1, 3).reshape(n_pages * B, pool.cfg.num_kv_heads, pool.cfg.head_dim)[:length]
+    v = vp[idx].permute(0, 2, 1, 3).reshape(n_pages * B, pool.cfg.num_kv_heads, pool.cfg.head_dim)[:length]
+    return k.contiguous(), v.contiguous()
