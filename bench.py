@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- re-prefill throughput of the SmoothAgent hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: drop the
+invalidated tail of every session (host), then for each chunk round sa_rope_kv_append (fused
+RoPE + page scatter) and sa_mixed_attention (prefill chunks over the paged retained prefix,
+co-batched with the decode rows).  The workload is BASELINE.json configs[1] (config 2: one
+Llama-3-8B-shaped session, 24,576-token retained prefix, 8,192-token segment in 2,048-token
+chunks) unless --config says otherwise.  Prints ONE JSON line (rank 0).
+
+--impl reference times the fp64 CPU oracle, as it stands, on a bounded sample of the same workload
+(the baseline arm of this tier; a deliberately slow program).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+METRIC = "re-prefill tokens/s (RoPE+KV append + paged causal attention, one layer)"
+UNIT = "tokens/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "source": "measured"}
+    # fallback stated in /opt/skills/guides/B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.samples, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def get_workload(cfg_id: int):
+    from paper_2607_00151_b200 import workloads as wl
+    return wl.CONFIGS[cfg_id]()
+
+
+def dist_setup(n_gpus: int):
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        dist.init_process_group(backend=backend)
+    return world, rank, local
+
+
+def dist_max(x: float, world: int, device) -> float:
+    if world == 1:
+        return x
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def dist_barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+# --------------------------------------------------------------------------------- oracle arm
+def oracle_sample(w, seconds_target: float = 15.0, seed: int = 0):
+    """Time the oracle, as it stands, on a bounded sample of the workload's re-prefill rows.
+    Returns (tokens_per_s, cores, description)."""
+    from oracle import oracle as orc
+    from paper_2607_00151_b200.workloads import gen_session
+    L = w.layer
+    pre = [i for i, s in enumerate(w.sessions) if s.new > 1] or [0]
+    i = pre[0]
+    s = w.sessions[i]
+    k, v, q = gen_session(w, i, "cpu")
+    P = s.prefix
+    k_rot_prefix = orc.rope(k[:P], np.arange(P), L.rope_base)  # the stored prefix: built before, not timed
+    v_prefix = orc.widen(v[:P])
+    ch = s.chunk or s.new
+    rng = np.random.default_rng(seed)
+    # calibrate on a few pairs, then size the sample for ~seconds_target
+    n_cal = 64
+    rows = rng.integers(0, ch, size=n_cal)
+    heads = rng.integers(0, L.num_q_heads, size=n_cal).astype(np.int32)
+    t0 = time.perf_counter()
+    orc.oracle_cached(k_rot_prefix, v_prefix, q[:ch], k[P:P + ch], v[P:P + ch], P, L.rope_base, rows=rows, heads=heads)
+    t_cal = time.perf_counter() - t0
+    n = int(max(256, min(ch * L.num_q_heads, n_cal * seconds_target / max(t_cal, 1e-3))))
+    rows = rng.integers(0, ch, size=n)
+    heads = rng.integers(0, L.num_q_heads, size=n).astype(np.int32)
+    t0 = time.perf_counter()
+    orc.oracle_cached(k_rot_prefix, v_prefix, q[:ch], k[P:P + ch], v[P:P + ch], P, L.rope_base, rows=rows, heads=heads)
+    dt = time.perf_counter() - t0
+    tokens = n / L.num_q_heads  # one token = all Hq heads of a row
+    desc = ("%d random (row, head) pairs (= %.1f token-equivalents) of the first %d-token chunk of session %d "
+            "(prefix %d), incl. RoPE of the chunk; %.1f s" % (n, tokens, ch, i, P, dt))
+    return tokens / dt, orc.num_threads(), desc
+
+
+def run_reference(args, world, rank):
+    if rank != 0:
+        return
+    w = get_workload(args.config)
+    vals, desc, cores = [], "", 1
+    per_step = max(2.0, min(20.0, 120.0 / max(args.steps + args.warmup, 1)))
+    for it in range(args.warmup + args.steps):
+        v, cores, desc = oracle_sample(w, per_step, seed=it)
+        if it >= args.warmup:
+            vals.append(v)
+    val = float(np.mean(vals))
+    tokens_step = sum(s.new for s in w.sessions)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tokens_step / val, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "note": w.note, "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------- our arm
+def run_ours(args, world, rank, local):
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle arm)")
+    import __graft_entry__
+    __graft_entry__.build()
+    from paper_2607_00151_b200 import binding as sa
+    from paper_2607_00151_b200.harness import Runner, make_pool
+
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda:%d" % local)
+    peaks = load_peaks()
+    w = get_workload(args.config)
+    L = w.layer
+    pool = make_pool(w, local, "random")
+    r = Runner(w, pool, None, local, want_lse=True)
+    prefix_tokens = r.fill_prefixes()
+    torch.cuda.synchronize()
+
+    tokens_step = sum(s.new for s in w.sessions)
+    A = w.pair_count()
+    flops_step = 4.0 * L.head_dim * L.num_q_heads * A          # algorithmic: causal pairs only (L313)
+    kappa = 2 * L.num_kv_heads * L.head_dim * 2                # KV bytes per token per layer
+    decode_bytes = kappa * w.decode_kv_tokens()
+    append_bytes = tokens_step * (2 * kappa + 2 * L.num_q_heads * L.head_dim * 2)
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def timed_step(attn_events=None):
+        flush.fill_(1)  # evict L2 between timed iterations (256 MiB > 126 MB L2); outside the event pair
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        r.truncate_to_prefix()
+        launches = 0
+        for rd in r.rounds:
+            rd.q.copy_(rd.q_raw)
+            sa.sa_rope_kv_append(pool, rd.sids, rd.indptr, rd.k, rd.v, rd.q)
+            launches += sa.sa_last_launch_count(pool)
+            if attn_events is not None:
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a0.record(stream)
+            sa.sa_mixed_attention(pool, rd.sids, rd.indptr, rd.q, rd.out, rd.lse, 0.0, rd.workspace)
+            launches += sa.sa_last_launch_count(pool)
+            if attn_events is not None:
+                a1.record(stream)
+                attn_events.append((a0, a1))
+        e1.record(stream)
+        return e0, e1, launches
+
+    r.step()  # allocates workspaces
+    for _ in range(max(args.warmup, 3)):
+        timed_step()
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    torch.cuda.synchronize()
+    ev, attn_ev, launches = [], [], 0
+    with ClockSampler(local) as cs:
+        for _ in range(args.steps):
+            e0, e1, n = timed_step(attn_ev)
+            ev.append((e0, e1))
+            launches += n
+        torch.cuda.synchronize()
+    dist_barrier(world)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = dist_max(float(sum(step_ms)), world, dev)
+    attn_ms = float(sum(a.elapsed_time(b) for a, b in attn_ev))
+    clocks = cs.summary()
+    value = world * tokens_step * args.steps / (total_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (prefill attention; decode if the workload has no prefill)
+    n_attn = len(attn_ev)
+    if flops_step > 0:
+        achieved = flops_step * args.steps / (attn_ms * 1e-3) / 1e12
+        peak = peaks["bf16_tflops"]
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peaks["source"] + " (burst; sustained %.1f)" % peaks["bf16_tflops_sustained"],
+                "kernel": "prefill attention inside sa_mixed_attention (%d calls timed, avg %.3f ms; decode rows of the same "
+                          "call included in the time when the workload has them)" % (n_attn, attn_ms / max(n_attn, 1)),
+                "algorithmic_flops_per_step": flops_step}
+    else:
+        achieved = decode_bytes * args.steps / (attn_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+                "traffic": None, "peak_source": peaks["source"], "kernel": "split-KV decode attention"}
+
+    # ---- e2e: the same step through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    host = []
+    for rd in r.rounds:
+        host.append(tuple(t.cpu().pin_memory() for t in (rd.k, rd.v, rd.q_raw)) + (torch.empty_like(rd.out, device="cpu").pin_memory(),))
+    h2d = sum(sum(t.numel() * t.element_size() for t in h[:3]) for h in host)
+    d2h = sum(h[3].numel() * h[3].element_size() for h in host)
+
+    def e2e_step():
+        r.truncate_to_prefix()
+        for rd, (hk, hv, hq, ho) in zip(r.rounds, host):
+            rd.k.copy_(hk, non_blocking=True)
+            rd.v.copy_(hv, non_blocking=True)
+            rd.q.copy_(hq, non_blocking=True)
+            sa.sa_rope_kv_append(pool, rd.sids, rd.indptr, rd.k, rd.v, rd.q)
+            sa.sa_mixed_attention(pool, rd.sids, rd.indptr, rd.q, rd.out, rd.lse, 0.0, rd.workspace)
+            ho.copy_(rd.out, non_blocking=True)
+
+    for _ in range(2):
+        e2e_step()
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        e2e_step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    e2e_ms = dist_max(float(e0.elapsed_time(e1)), world, dev)
+    e2e_val = world * tokens_step * args.steps / (e2e_ms * 1e-3)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": w.name, "note": w.note, "layer": "Hq=%d Hkv=%d D=%d page=%d" % (L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size),
+                   "tokens_per_step": tokens_step, "prefix_tokens": prefix_tokens, "causal_pairs": A,
+                   "l2": "256 MiB L2 flush between timed steps (outside the event pairs); KV working set %.0f MB" % (kappa * sum(s.total for s in w.sessions) / 1e6),
+                   "multi_gpu": "replicas (sessions are independent; no data-path collective)"},
+        "attention_tflops": flops_step * args.steps / (attn_ms * 1e-3) / 1e12 if flops_step else 0.0,
+        "attention_ms_per_step": attn_ms / args.steps,
+        "append_gbs": append_bytes * args.steps / max((float(sum(step_ms)) - attn_ms) * 1e-3, 1e-9) / 1e9,
+        "decode_bytes_per_step": decode_bytes,
+        "roofline": roof,
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": launches,
+        "clocks": clocks,
+    }
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            v, cores, desc = oracle_sample(w, 15.0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2 = configs[1])")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        world = int(os.environ.get("WORLD_SIZE", "1"))
+        rank = int(os.environ.get("RANK", "0"))
+        run_reference(args, world, rank)
+        return
+    world, rank, local = dist_setup(args.gpus)
+    run_ours(args, world, rank, local)
+
+
+if __name__ == "__main__":
+    main()

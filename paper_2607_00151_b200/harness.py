@@ -135,7 +135,7 @@ class Runner:
             if append:
                 r.q.copy_(r.q_raw)
                 sa.sa_rope_kv_append(self.pool, r.sids, r.indptr, r.k, r.v, r.q)
-                launches += sa.sa_last_launch_count(self.pool) + 1
+                launches += sa.sa_last_launch_count(self.pool)
             if attention:
                 if r.workspace is None:
                     nb = sa.sa_mixed_attention_workspace_bytes(self.pool, r.sids, r.indptr)
