@@ -1,20 +1,435 @@
-// sa_prefill_tc5.cu -- prefill-chunk attention on tcgen05 / TMEM / TMA.
-// Placeholder until the kernel lands: the planner asks tc5_supported() and routes prefill
-// chunks to the mma.sync kernel while this returns false.
+// sa_prefill_tc5.cu -- prefill-chunk attention over paged KV on the 5th-generation tensor cores
+// (chunk j has q_j query tokens over prefix_j cached
+// tokens, "the i-th query token attends to prefix_j + i + 1 tokens"; compute-bound, cost ~ A_j).
+//
+// One CTA = one (request, kv head, 256 packed rows) work item; packed row rho is
+// (token rho / G, q head g*G + rho % G), so the G query heads of a group share every K/V tile.
+// The 256 rows are two 128-row Q tiles that ping-pong: while the softmax warps of one tile work
+// on S, the tensor core runs the other tile's MMAs.  Warp roles (384 threads):
+//   warp 0      TMA producer: Q tiles once, then page-gathered K and V tiles (2-stage rings);
+//               zero-fills V rows past the end of the session in the last tile
+//   warp 1      MMA issuer (one lane): S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM, V MN-major)
+//   warp 2      TMEM allocator
+//   warps 4-7   softmax of Q tile 0 (thread = row): S from TMEM, mask, lazy-rescaled online
+//   warps 8-11  softmax of Q tile 1   softmax, P (bf16) back into the S columns, epilogue
+// TMEM (512 columns): S0/P0 [0,128)  S1/P1 [128,256)  O0 [256,384)  O1 [384,512).
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <math.h>
+
 #include "sa_internal.h"
+#include "sa_tc5_ptx.cuh"
 
 namespace sa {
 
+namespace {
+
+using namespace ptx;
+
+constexpr int D = 128;            // head_dim of this kernel
+constexpr int BM = 128;           // rows per Q tile
+constexpr int BN = 128;           // keys per KV tile
+constexpr int kThreadsTc5 = 384;
+constexpr int TILE_BYTES = BN * D * 2;   // 32 KiB: two 64-wide halves of 128 rows x 128 B
+constexpr int HALF_BYTES = TILE_BYTES / 2;
+constexpr int KV_STAGES = 2;
+constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the row max grows by > 2^8
+
+struct Tc5Args {
+    const ReqMeta *reqs;
+    int32_t n_reqs;
+    const int32_t *block_table;
+    int64_t mpps;
+    __nv_bfloat16 *out;
+    float *lse;
+    int32_t Hq, Hkv, log2G;
+    float scale_log2;
+};
+
+enum Bar {
+    BAR_Q = 0,
+    BAR_K_FULL = 1,   // [2]
+    BAR_K_EMPTY = 3,  // [2]
+    BAR_V_FULL = 5,   // [2]
+    BAR_V_EMPTY = 7,  // [2]
+    BAR_S_FULL = 9,   // [2] per Q tile
+    BAR_P_FULL = 11,  // [2]
+    BAR_O_FULL = 13,  // [2]
+    BAR_V_FIXED = 15,
+    BAR_COUNT = 16
+};
+
+__device__ __forceinline__ int find_req_tc5(const ReqMeta *reqs, int n, int item) {
+    int lo = 0, hi = n - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (reqs[mid].item_begin <= item) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+template <int LOG2B>
+__global__ void __launch_bounds__(kThreadsTc5, 1)
+prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
+                   const __grid_constant__ CUtensorMap tmap_v, const Tc5Args a) {
+    constexpr int B = 1 << LOG2B;
+    constexpr int PAGES_PER_TILE = BN / B;
+    constexpr uint32_t PAGE_HALF_BYTES = B * 128;  // one page, one 64-wide half: B rows x 128 B
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const uint32_t sQ = smem_u32(smem);                 // 2 tiles x 32 KiB
+    const uint32_t sK = sQ + 2 * TILE_BYTES;            // KV_STAGES x 32 KiB
+    const uint32_t sV = sK + KV_STAGES * TILE_BYTES;    // KV_STAGES x 32 KiB
+    __shared__ uint64_t bars[BAR_COUNT];
+    __shared__ uint32_t tmem_base_smem;
+    const uint32_t bar0 = smem_u32(&bars[0]);
+    auto bar = [&](int i) -> uint32_t { return bar0 + 8u * uint32_t(i); };
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    // ---- work item
+    const int item = blockIdx.x;
+    const ReqMeta r = a.reqs[find_req_tc5(a.reqs, a.n_reqs, item)];
+    const int local = item - r.item_begin;
+    const int g = local / r.n_tiles;
+    const int tile = r.n_tiles - 1 - local % r.n_tiles;  // late (heavy) tiles first
+    const int G = 1 << a.log2G;
+    const int n_rows = r.q_len * G;
+    const int rho0 = tile * (2 * BM);
+    const int base_lim = r.kv_len - r.q_len;
+    const int tok_max = min(r.q_len - 1, (rho0 + 2 * BM - 1) >> a.log2G);
+    const int k_end = base_lim + tok_max + 1;                   // keys [0, k_end) are needed
+    const int n_kv = (k_end + BN - 1) / BN;
+    const int pages_needed = (k_end + B - 1) >> LOG2B;
+    // last tile: rows at or past `valid_last` hold no session data (unloaded pages or slots >= kv_len)
+    const int last_pages = min(PAGES_PER_TILE, pages_needed - (n_kv - 1) * PAGES_PER_TILE);
+    const int valid_last = min(r.kv_len - (n_kv - 1) * BN, last_pages * B);
+    const bool need_fix = valid_last < BN;
+
+    if (tid == 0) {
+        mbar_init(bar(BAR_Q), 1);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(bar(BAR_K_FULL + s), 1);
+            mbar_init(bar(BAR_K_EMPTY + s), 1);
+            mbar_init(bar(BAR_V_FULL + s), 1);
+            mbar_init(bar(BAR_V_EMPTY + s), 1);
+            mbar_init(bar(BAR_S_FULL + s), 1);
+            mbar_init(bar(BAR_P_FULL + s), BM);
+            mbar_init(bar(BAR_O_FULL + s), 1);
+        }
+        mbar_init(bar(BAR_V_FIXED), 1);
+        fence_mbar_init();
+    }
+    if (warp == 2) tmem_alloc<512>(smem_u32(&tmem_base_smem));
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base_smem;
+
+    if (warp == 0) {
+        // =========================== TMA producer ===========================
+        if (lane == 0) {
+            prefetch_tmap(&tmap_q);
+            prefetch_tmap(&tmap_k);
+            prefetch_tmap(&tmap_v);
+            mbar_expect_tx(bar(BAR_Q), 2 * TILE_BYTES);
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int tok0 = r.q_start + ((rho0 + t * BM) >> a.log2G);
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    tma_load_3d(sQ + t * TILE_BYTES + h * HALF_BYTES, &tmap_q, bar(BAR_Q), h * 64, g << a.log2G, tok0);
+            }
+            const int32_t *bt = a.block_table + int64_t(r.sid) * a.mpps;
+            for (int j = 0; j < n_kv; ++j) {
+                const int s = j & 1, ph = (j >> 1) & 1;
+                const int p0 = j * PAGES_PER_TILE;
+                const int np = min(PAGES_PER_TILE, pages_needed - p0);
+                int32_t pg[PAGES_PER_TILE];
+#pragma unroll
+                for (int u = 0; u < PAGES_PER_TILE; ++u) pg[u] = u < np ? __ldg(bt + p0 + u) : 0;
+                mbar_wait(bar(BAR_K_EMPTY + s), ph ^ 1);
+                mbar_expect_tx(bar(BAR_K_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
+#pragma unroll
+                for (int u = 0; u < PAGES_PER_TILE; ++u)
+                    if (u < np) {
+                        tma_load_4d(sK + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 0, 0, g, pg[u]);
+                        tma_load_4d(sK + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 64, 0, g, pg[u]);
+                    }
+                mbar_wait(bar(BAR_V_EMPTY + s), ph ^ 1);
+                mbar_expect_tx(bar(BAR_V_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
+#pragma unroll
+                for (int u = 0; u < PAGES_PER_TILE; ++u)
+                    if (u < np) {
+                        tma_load_4d(sV + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 0, 0, g, pg[u]);
+                        tma_load_4d(sV + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 64, 0, g, pg[u]);
+                    }
+            }
+        }
+        __syncwarp();
+        if (need_fix) {
+            // V rows that hold no session data must be exactly zero: P is 0 there, and 0 * NaN = NaN
+            const int j = n_kv - 1, s = j & 1, ph = (j >> 1) & 1;
+            mbar_wait(bar(BAR_V_FULL + s), ph);
+            const int n_zero = BN - valid_last;  // rows [valid_last, 128), 2 halves x 8 chunks of 16 B each
+            for (int e = lane; e < n_zero * 16; e += 32) {
+                const int row = valid_last + (e >> 4), hc = e & 15;
+                const uint32_t addr = sV + s * TILE_BYTES + (hc >> 3) * HALF_BYTES + row * 128 + (hc & 7) * 16;
+                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(addr), "r"(0) : "memory");
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(BAR_V_FIXED));
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer ===========================
+        if (lane == 0) {
+            constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
+            constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
+            auto issue_qk = [&](int t, int s) {
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t off = (ks >> 2) * HALF_BYTES + (ks & 3) * 32;
+                    umma_ss(tmem + t * BN, umma_desc(sQ + t * TILE_BYTES + off, 16, 1024),
+                            umma_desc(sK + s * TILE_BYTES + off, 16, 1024), idesc_qk, ks > 0);
+                }
+            };
+            auto issue_pv = [&](int t, int s, bool acc) {
+#pragma unroll
+                for (int ks = 0; ks < BN / 16; ++ks)
+                    umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8,
+                            umma_desc(sV + s * TILE_BYTES + ks * 2048, HALF_BYTES, 1024), idesc_pv, acc || ks > 0);
+            };
+            mbar_wait(bar(BAR_Q), 0);
+            mbar_wait(bar(BAR_K_FULL + 0), 0);
+            tc_fence_after();
+            issue_qk(0, 0);
+            umma_commit(bar(BAR_S_FULL + 0));
+            issue_qk(1, 0);
+            umma_commit(bar(BAR_S_FULL + 1));
+            umma_commit(bar(BAR_K_EMPTY + 0));
+            for (int j = 0; j < n_kv; ++j) {
+                const int s = j & 1, ph = (j >> 1) & 1;
+                const bool has_next = j + 1 < n_kv;
+                const int sn = (j + 1) & 1, phn = ((j + 1) >> 1) & 1;
+                if (j == n_kv - 1 && need_fix) mbar_wait(bar(BAR_V_FIXED), 0);
+                else mbar_wait(bar(BAR_V_FULL + s), ph);
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    mbar_wait(bar(BAR_P_FULL + t), j & 1);
+                    tc_fence_after();
+                    issue_pv(t, s, j > 0);
+                    if (t == 1) umma_commit(bar(BAR_V_EMPTY + s));
+                    if (has_next) {
+                        if (t == 0) {
+                            mbar_wait(bar(BAR_K_FULL + sn), phn);
+                            tc_fence_after();
+                        }
+                        issue_qk(t, sn);
+                        umma_commit(bar(BAR_S_FULL + t));
+                        if (t == 1) umma_commit(bar(BAR_K_EMPTY + sn));
+                    } else {
+                        umma_commit(bar(BAR_O_FULL + t));
+                    }
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // =========================== softmax + epilogue ===========================
+        const int t = (warp - 4) >> 2;                 // Q tile of this warpgroup
+        const int row = ((warp & 3) << 5) + lane;      // TMEM lane == row of the tile
+        const int rho = rho0 + t * BM + row;
+        const bool valid = rho < n_rows;
+        const int lim = valid ? base_lim + (rho >> a.log2G) : -1;
+        const int lim_min = base_lim + ((rho0 + t * BM) >> a.log2G);  // smallest limit among the tile's rows
+        const uint32_t lane_addr = tmem + (uint32_t((warp & 3) << 5) << 16);
+        const uint32_t tS = lane_addr + t * BN, tO = lane_addr + 2 * BN + t * D;
+        const float sl2 = a.scale_log2;
+        float m_used = -INFINITY, l = 0.f;
+
+        for (int j = 0; j < n_kv; ++j) {
+            mbar_wait(bar(BAR_S_FULL + t), j & 1);
+            tc_fence_after();
+            float sv[BN];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                uint32_t rr[32];
+                tmem_ld32(tS + c * 32, rr);
+                tmem_wait_ld();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) sv[c * 32 + i] = __uint_as_float(rr[i]);
+            }
+            const int kt = j * BN;
+            if (kt + BN - 1 > lim_min) {  // uniform over the warpgroup: diagonal / last tiles only
+#pragma unroll
+                for (int i = 0; i < BN; ++i)
+                    if (kt + i > lim) sv[i] = -INFINITY;
+            }
+            float mx = sv[0];
+#pragma unroll
+            for (int i = 1; i < BN; ++i) mx = fmaxf(mx, sv[i]);
+            const float m_new = fmaxf(m_used, mx);
+            const bool need = (m_new - m_used) * sl2 > kRescaleThreshold;  // true on the first live tile
+            if (__any_sync(0xffffffffu, need)) {
+                const float f = need ? ex2_approx((m_used - m_new) * sl2) : 1.0f;
+                if (need) {
+                    l *= f;
+                    m_used = m_new;
+                }
+                if (j > 0) {  // PV(t, j-1) has completed (it precedes QK(t, j) in the pipe); PV(t, j) waits for P
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        uint32_t rr[32];
+                        tmem_ld32(tO + c * 32, rr);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) rr[i] = __float_as_uint(__uint_as_float(rr[i]) * f);
+                        tmem_st32(tO + c * 32, rr);
+                    }
+                }
+            }
+            const float neg = (m_used == -INFINITY) ? 0.f : -m_used * sl2;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                uint32_t pk[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float p0 = ex2_approx(fmaf(sv[c * 32 + 2 * i], sl2, neg));
+                    const float p1 = ex2_approx(fmaf(sv[c * 32 + 2 * i + 1], sl2, neg));
+                    l += p0 + p1;
+                    __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
+                    pk[i] = *reinterpret_cast<uint32_t *>(&pb);
+                }
+                tmem_st16(tS + c * 16, pk);
+            }
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(bar(BAR_P_FULL + t));
+        }
+        // ---- epilogue: O / l -> bf16 -> out
+        mbar_wait(bar(BAR_O_FULL + t), 0);
+        tc_fence_after();
+        const float inv = l > 0.f ? 1.0f / l : 0.f;
+        const int tok = rho >> a.log2G, hq = (g << a.log2G) + (rho & (G - 1));
+        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            uint32_t rr[32];
+            tmem_ld32(tO + c * 32, rr);
+            tmem_wait_ld();
+            if (valid) {
+                uint4 *dst = reinterpret_cast<uint4 *>(a.out + orow * D + c * 32);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    uint32_t w[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        __nv_bfloat162 pb = __floats2bfloat162_rn(__uint_as_float(rr[i * 8 + 2 * e]) * inv,
+                                                                  __uint_as_float(rr[i * 8 + 2 * e + 1]) * inv);
+                        w[e] = *reinterpret_cast<uint32_t *>(&pb);
+                    }
+                    dst[i] = make_uint4(w[0], w[1], w[2], w[3]);
+                }
+            }
+        }
+        if (valid && a.lse) a.lse[orow] = (m_used * sl2 + log2f(l)) * 0.6931471805599453f;
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc<512>(tmem);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        (void)cudaGetLastError();
+    }
+    return fn;
+}
+
+constexpr size_t kSmemTc5 = size_t(2 + 2 * KV_STAGES) * TILE_BYTES + 1024;
+
+}  // namespace
+
 int32_t tc5_init(sa_kv_pool *pool) {
     pool->tc5_ready = false;
+    if (pool->cfg.head_dim != D) return SA_OK;  // head_dim 64 stays on the mma.sync kernel
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return SA_ERR_CUDA;
+    const sa_kv_pool_config &c = pool->cfg;
+    cuuint64_t dims[4] = {cuuint64_t(D), cuuint64_t(c.page_size), cuuint64_t(c.num_kv_heads), cuuint64_t(c.num_pages)};
+    cuuint64_t strides[3] = {cuuint64_t(D) * 2, cuuint64_t(c.page_size) * D * 2,
+                             cuuint64_t(c.num_kv_heads) * c.page_size * D * 2};
+    cuuint32_t box[4] = {64, cuuint32_t(c.page_size), 1, 1};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    for (int w = 0; w < 2; ++w) {
+        CUresult rc = enc(reinterpret_cast<CUtensorMap *>(w ? pool->tmap_v : pool->tmap_k), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+                          4, w ? pool->v_base : pool->k_base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (rc != CUDA_SUCCESS) return SA_ERR_CUDA;
+    }
+    cudaError_t e = pool->cfg.page_size == 64
+                        ? cudaFuncSetAttribute(prefill_tc5_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemTc5))
+                        : cudaFuncSetAttribute(prefill_tc5_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemTc5));
+    if (e != cudaSuccess) return SA_ERR_CUDA;
+    pool->tc5_ready = true;
     return SA_OK;
 }
 
-bool tc5_supported(const sa_kv_pool *pool) { return pool->tc5_ready; }
+// Host-only pools (no device) report the same routing a device pool of this shape would use, so
+// the planner can be tested without a GPU.
+bool tc5_supported(const sa_kv_pool *pool) { return pool->host_only ? pool->cfg.head_dim == D : pool->tc5_ready; }
 
-cudaError_t launch_prefill_tc5(const sa_kv_pool *, const ReqMeta *, const AttnPlan &, int64_t, const void *, void *,
-                               float *, float, cudaStream_t, int32_t *) {
-    return cudaErrorNotSupported;
+cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan, int64_t total_q,
+                               const void *q, void *out, float *lse, float sm_scale, cudaStream_t stream,
+                               int32_t *launches) {
+    if (plan.pre_items == 0) return cudaSuccess;
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return cudaErrorNotSupported;
+    const sa_kv_pool_config &c = pool->cfg;
+    // Q as [T][Hq][D]; one box = 64 dims x G heads x 128/G tokens = a 128-row packed tile half
+    alignas(64) CUtensorMap tq;
+    cuuint64_t dims[3] = {cuuint64_t(D), cuuint64_t(c.num_q_heads), cuuint64_t(total_q)};
+    cuuint64_t strides[2] = {cuuint64_t(D) * 2, cuuint64_t(c.num_q_heads) * D * 2};
+    cuuint32_t box[3] = {64, cuuint32_t(pool->G), cuuint32_t(BM / pool->G)};
+    cuuint32_t es[3] = {1, 1, 1};
+    if (enc(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(q), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorInvalidValue;
+    Tc5Args a;
+    a.reqs = reqs_dev;
+    a.n_reqs = plan.n_pre;
+    a.block_table = pool->block_table;
+    a.mpps = pool->max_pages_per_session;
+    a.out = static_cast<__nv_bfloat16 *>(out);
+    a.lse = lse;
+    a.Hq = c.num_q_heads;
+    a.Hkv = c.num_kv_heads;
+    int lg = 0;
+    while ((1 << lg) < pool->G) ++lg;
+    a.log2G = lg;
+    a.scale_log2 = sm_scale * 1.4426950408889634f;
+    const CUtensorMap &tk = *reinterpret_cast<const CUtensorMap *>(pool->tmap_k);
+    const CUtensorMap &tv = *reinterpret_cast<const CUtensorMap *>(pool->tmap_v);
+    if (c.page_size == 64)
+        prefill_tc5_kernel<6><<<unsigned(plan.pre_items), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+    else
+        prefill_tc5_kernel<4><<<unsigned(plan.pre_items), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+    ++*launches;
+    return cudaGetLastError();
 }
 
 }  // namespace sa
