@@ -68,6 +68,37 @@ __device__ __forceinline__ int find_req_tc5(const ReqMeta *reqs, int n, int item
     return lo;
 }
 
+// ---- per-chunk pieces of the softmax (a chunk = 32 of the 128 S columns of a row, in registers)
+__device__ __forceinline__ void chunk_mask(uint32_t (&s)[32], int key0, int lim) {
+#pragma unroll
+    for (int i = 0; i < 32; ++i)
+        if (key0 + i > lim) s[i] = 0xff800000u;  // -inf: selected, never added
+}
+__device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
+    float m = __uint_as_float(s[0]);
+#pragma unroll
+    for (int i = 1; i < 31; i += 2) m = fmaxf(fmaxf(m, __uint_as_float(s[i])), __uint_as_float(s[i + 1]));
+    return fmaxf(m, __uint_as_float(s[31]));
+}
+// exp2 of one chunk, row sums, bf16 P into 16 TMEM columns.  Three of four exponentials run on
+// the MUFU, one of four as a cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
+template <bool MASKED>
+__device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], float sl2, float neg, float (&lsum)[4],
+                                                uint32_t taddr) {
+    uint32_t pk[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float x0 = fmaf(__uint_as_float(s[2 * i]), sl2, neg);
+        const float x1 = fmaf(__uint_as_float(s[2 * i + 1]), sl2, neg);
+        const float p0 = ex2_approx(x0);
+        const float p1 = ((i & 1) && !MASKED) ? ex2_poly3(x1) : ex2_approx(x1);
+        lsum[i & 3] += p0 + p1;
+        __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
+        pk[i] = *reinterpret_cast<uint32_t *>(&pb);
+    }
+    tmem_st16(taddr, pk);
+}
+
 template <int LOG2B>
 __global__ void __launch_bounds__(kThreadsTc5, 1)
 prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
@@ -127,8 +158,12 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     tc_fence_after();
     const uint32_t tmem = tmem_base_smem;
 
+    // register budget: the 8 softmax warps hold a 128-column S row per thread; the others need few
+    // (setmaxnreg sits inside each role branch so that no control-flow merge follows it)
+
     if (warp == 0) {
         // =========================== TMA producer ===========================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
         if (lane == 0) {
             prefetch_tmap(&tmap_q);
             prefetch_tmap(&tmap_k);
@@ -184,6 +219,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
         if (lane == 0) {
             constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
             constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
@@ -235,8 +271,11 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 }
             }
         }
-    } else if (warp >= 4) {
+    } else if (warp < 4) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+    } else {
         // =========================== softmax + epilogue ===========================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
         const int t = (warp - 4) >> 2;                 // Q tile of this warpgroup
         const int row = ((warp & 3) << 5) + lane;      // TMEM lane == row of the tile
         const int rho = rho0 + t * BM + row;
@@ -246,35 +285,34 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         const uint32_t lane_addr = tmem + (uint32_t((warp & 3) << 5) << 16);
         const uint32_t tS = lane_addr + t * BN, tO = lane_addr + 2 * BN + t * D;
         const float sl2 = a.scale_log2;
-        float m_used = -INFINITY, l = 0.f;
+        float m_used = -INFINITY;
 
+        float lsum[4] = {0.f, 0.f, 0.f, 0.f};  // independent partial row sums (shorter dependency chains)
         for (int j = 0; j < n_kv; ++j) {
             mbar_wait(bar(BAR_S_FULL + t), j & 1);
             tc_fence_after();
-            float sv[BN];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                uint32_t rr[32];
-                tmem_ld32(tS + c * 32, rr);
-                tmem_wait_ld();
-#pragma unroll
-                for (int i = 0; i < 32; ++i) sv[c * 32 + i] = __uint_as_float(rr[i]);
-            }
+            uint32_t s0[32], s1[32], s2[32], s3[32];
+            tmem_ld32(tS, s0);
+            tmem_ld32(tS + 32, s1);
+            tmem_ld32(tS + 64, s2);
+            tmem_ld32(tS + 96, s3);
+            tmem_wait_ld();
             const int kt = j * BN;
-            if (kt + BN - 1 > lim_min) {  // uniform over the warpgroup: diagonal / last tiles only
-#pragma unroll
-                for (int i = 0; i < BN; ++i)
-                    if (kt + i > lim) sv[i] = -INFINITY;
+            const bool masked = kt + BN - 1 > lim_min;  // uniform over the warpgroup: diagonal / last tiles only
+            if (masked) {
+                chunk_mask(s0, kt, lim);
+                chunk_mask(s1, kt + 32, lim);
+                chunk_mask(s2, kt + 64, lim);
+                chunk_mask(s3, kt + 96, lim);
             }
-            float mx = sv[0];
-#pragma unroll
-            for (int i = 1; i < BN; ++i) mx = fmaxf(mx, sv[i]);
+            const float mx = fmaxf(fmaxf(chunk_max(s0), chunk_max(s1)), fmaxf(chunk_max(s2), chunk_max(s3)));
             const float m_new = fmaxf(m_used, mx);
             const bool need = (m_new - m_used) * sl2 > kRescaleThreshold;  // true on the first live tile
             if (__any_sync(0xffffffffu, need)) {
                 const float f = need ? ex2_approx((m_used - m_new) * sl2) : 1.0f;
                 if (need) {
-                    l *= f;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) lsum[c] *= f;
                     m_used = m_new;
                 }
                 if (j > 0) {  // PV(t, j-1) has completed (it precedes QK(t, j) in the pipe); PV(t, j) waits for P
@@ -290,23 +328,22 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 }
             }
             const float neg = (m_used == -INFINITY) ? 0.f : -m_used * sl2;
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                uint32_t pk[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    const float p0 = ex2_approx(fmaf(sv[c * 32 + 2 * i], sl2, neg));
-                    const float p1 = ex2_approx(fmaf(sv[c * 32 + 2 * i + 1], sl2, neg));
-                    l += p0 + p1;
-                    __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
-                    pk[i] = *reinterpret_cast<uint32_t *>(&pb);
-                }
-                tmem_st16(tS + c * 16, pk);
+            if (masked) {
+                chunk_exp_store<true>(s0, sl2, neg, lsum, tS);
+                chunk_exp_store<true>(s1, sl2, neg, lsum, tS + 16);
+                chunk_exp_store<true>(s2, sl2, neg, lsum, tS + 32);
+                chunk_exp_store<true>(s3, sl2, neg, lsum, tS + 48);
+            } else {
+                chunk_exp_store<false>(s0, sl2, neg, lsum, tS);
+                chunk_exp_store<false>(s1, sl2, neg, lsum, tS + 16);
+                chunk_exp_store<false>(s2, sl2, neg, lsum, tS + 32);
+                chunk_exp_store<false>(s3, sl2, neg, lsum, tS + 48);
             }
             tmem_wait_st();
             tc_fence_before();
             mbar_arrive(bar(BAR_P_FULL + t));
         }
+        const float l = (lsum[0] + lsum[1]) + (lsum[2] + lsum[3]);
         // ---- epilogue: O / l -> bf16 -> out
         mbar_wait(bar(BAR_O_FULL + t), 0);
         tc_fence_after();

@@ -150,5 +150,18 @@ __device__ __forceinline__ float ex2_approx(float x) {
     return y;
 }
 
+// 2^x as a cubic on the FMA pipe (max relative error 7.5e-5, far below bf16's 2^-9): floor(x) via
+// a round-down add of 1.5*2^23, cubic in the fraction, exponent patched in with an integer add.
+__device__ __forceinline__ float ex2_poly3(float x) {
+    x = fmaxf(x, -126.0f);
+    float xf;
+    asm("add.rm.f32 %0, %1, %2;" : "=f"(xf) : "f"(x), "f"(12582912.0f));
+    const float fr = x - (xf - 12582912.0f);
+    float p = fmaf(0.07802419364452362f, fr, 0.22606728971004486f);
+    p = fmaf(p, fr, 0.695833683013916f);
+    p = fmaf(p, fr, 0.9999251961708069f);
+    return __int_as_float(__float_as_int(p) + (__float_as_int(xf) << 23));
+}
+
 }  // namespace ptx
 }  // namespace sa
