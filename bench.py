@@ -184,6 +184,91 @@ def run_reference(args, world, rank):
     print(json.dumps(line))
 
 
+# --------------------------------------------------------------------------------- HBM-bound parts
+def measure_parts(local: int, peaks, iters: int = 10):
+    """Decode attention and RoPE+append are HBM-bound and too small in config 2 to carry a bandwidth
+    claim, so they are timed on config 4's decode set (64 rows on 8K-32K contexts, 5.4 GB of K/V per
+    launch: larger than L2, no flush needed) and on its ragged prefix fill (1.3 M tokens in one call)."""
+    from paper_2607_00151_b200 import binding as sa
+    from paper_2607_00151_b200.harness import Runner, make_pool
+    w = get_workload(4)
+    L = w.layer
+    dev = torch.device("cuda:%d" % local)
+    stream = torch.cuda.current_stream()
+    pool = make_pool(w, local, "random")
+    r = Runner(w, pool, None, local, want_lse=False)
+    kappa = 2 * L.num_kv_heads * L.head_dim * 2
+
+    def timed(fn, n):
+        ts = []
+        for _ in range(n):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts)), float(min(ts))
+
+    # ---- append: the ragged prefix fill (K/V only: read kappa + write kappa per token), inputs concatenated beforehand
+    pre = [i for i, s_ in enumerate(w.sessions) if s_.prefix > 0]
+    fk = torch.cat([r.data[i][0][: w.sessions[i].prefix] for i in pre]).contiguous()
+    fv = torch.cat([r.data[i][1][: w.sessions[i].prefix] for i in pre]).contiguous()
+    f_indptr = np.concatenate([[0], np.cumsum([w.sessions[i].prefix for i in pre])]).astype(np.int32)
+    f_sids = [r.sids[i] for i in pre]
+
+    def fill():
+        for sid in r.sids:
+            sa.sa_kv_session_truncate(pool, sid, 0)
+        sa.sa_rope_kv_append(pool, f_sids, f_indptr, fk, fv, None)
+    fill()
+    torch.cuda.synchronize()
+    tok = sum(s.prefix for s in w.sessions)
+    ms_fill, ms_fill_min = timed(fill, max(3, iters // 2))
+    app_bytes = 2.0 * kappa * tok
+    app = {"bound": "hbm", "achieved": app_bytes / (ms_fill * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+           "frac": app_bytes / (ms_fill * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+           "kernel": "rope_append_kernel on config 4's prefix fill: %d tokens, %d sessions, one sa_rope_kv_append call"
+                     " (page allocation and block-table update included)" % (tok, len(w.sessions)),
+           "bytes_per_launch": app_bytes, "ms": ms_fill, "ms_min": ms_fill_min, "peak_source": peaks["source"]}
+    # ---- decode: the 64 decode rows alone
+    del fk, fv
+    r.step()
+    torch.cuda.synchronize()
+    rd = r.rounds[0]
+    dec = [j for j, i in enumerate(rd.idx) if w.sessions[i].new == 1]
+    sids = [rd.sids[j] for j in dec]
+    q = torch.cat([rd.q[int(rd.indptr[j]): int(rd.indptr[j + 1])] for j in dec]).contiguous()
+    indptr = np.arange(len(dec) + 1, dtype=np.int32)
+    out = torch.empty_like(q)
+    ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(pool, sids, indptr), 256), dtype=torch.uint8, device=dev)
+    run_dec = lambda: sa.sa_mixed_attention(pool, sids, indptr, q, out, None, 0.0, ws)
+    for _ in range(3):
+        run_dec()
+    torch.cuda.synchronize()
+    ms_dec, ms_dec_min = timed(run_dec, iters)
+    kv_tok = w.decode_kv_tokens()
+    dec_bytes = float(kappa) * kv_tok + 2.0 * q.numel() * 2
+    decode = {"bound": "hbm", "achieved": dec_bytes / (ms_dec * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+              "frac": dec_bytes / (ms_dec * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+              "kernel": "flash_mma_kernel<128,0> (split-KV decode) + merge_splits_kernel on config 4's %d decode rows, "
+                        "%d cached tokens" % (len(dec), kv_tok),
+              "bytes_per_launch": dec_bytes, "ms": ms_dec, "ms_min": ms_dec_min, "peak_source": peaks["source"]}
+    # ---- the mixed call (4 chunks x 2048 + 64 decode rows) for context
+    if rd.workspace is None:
+        rd.workspace = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(pool, rd.sids, rd.indptr), 256), dtype=torch.uint8, device=dev)
+    run_mixed = lambda: sa.sa_mixed_attention(pool, rd.sids, rd.indptr, rd.q, rd.out, None, 0.0, rd.workspace)
+    run_mixed()
+    torch.cuda.synchronize()
+    ms_mix, _ = timed(run_mixed, iters)
+    flops = 4.0 * L.head_dim * L.num_q_heads * w.pair_count()
+    mixed = {"ms": ms_mix, "prefill_tflops_if_alone": flops / (ms_mix * 1e-3) / 1e12, "prefill_flops": flops,
+             "decode_bytes": dec_bytes, "note": "config 4 mixed lookahead batch: one sa_mixed_attention call"}
+    r.close()
+    sa.sa_kv_pool_destroy(pool)
+    return decode, app, mixed
+
+
 # --------------------------------------------------------------------------------- our arm
 def run_ours(args, world, rank, local):
     if not torch.cuda.is_available():
@@ -316,6 +401,15 @@ def run_ours(args, world, rank, local):
         "gpu_launches": launches,
         "clocks": clocks,
     }
+    if world == 1 and not args.no_parts:
+        r.close()
+        sa.sa_kv_pool_destroy(pool)
+        del r, pool, flush
+        torch.cuda.empty_cache()
+        dec_roof, app_roof, mixed = measure_parts(local, peaks)
+        line["roofline_decode"] = dec_roof
+        line["roofline_append"] = app_roof
+        line["mixed_config4"] = mixed
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_sample(w, 15.0)
@@ -334,6 +428,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2 = configs[1])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parts", action="store_true", help="skip the decode / append bandwidth measurements on config 4")
     args = ap.parse_args()
     if args.impl == "reference":
         world = int(os.environ.get("WORLD_SIZE", "1"))
