@@ -52,20 +52,42 @@ def make_pool(w: Workload, device: int = 0, page_order="random", sentinel: Optio
 
 class Runner:
     def __init__(self, w: Workload, pool: sa.Pool, data: Optional[Dict[int, tuple]] = None, device: int = 0,
-                 scale: Optional[float] = None, want_lse: bool = True):
+                 scale: Optional[float] = None, want_lse: bool = True, lazy: bool = False):
+        """lazy=True (config 5): raw inputs are generated session by session inside fill_prefixes and only
+        the new tokens' k, v, q are kept, so the 45 GB of raw prefix inputs are never resident at once."""
         self.w, self.pool, self.device = w, pool, device
         self.dev = torch.device("cuda:%d" % device)
-        self.data = data if data is not None else {i: gen_session(w, i, self.dev, scale) for i in range(len(w.sessions))}
+        self.scale, self.lazy = scale, lazy
         self.want_lse = want_lse
         self.sids = [sa.sa_kv_session_open(pool) for _ in w.sessions]
         self.rounds: List[Round] = []
         self.launches_per_step = 0
-        self._build_rounds()
+        self.new: Dict[int, tuple] = {}   # session -> (k_new, v_new, q) of its appended tokens
+        if lazy:
+            self.data = {}
+        else:
+            self.data = data if data is not None else {i: gen_session(w, i, self.dev, scale) for i in range(len(w.sessions))}
+            for i, s in enumerate(w.sessions):
+                k, v, q = self.data[i]
+                self.new[i] = (k[s.prefix:], v[s.prefix:], q)
+            self._build_rounds()
 
     # -- retained prefixes -------------------------------------------------------------------
     def fill_prefixes(self, max_tokens_per_call: int = 1 << 20) -> int:
         """Append every session's retained prefix (K/V only).  Returns tokens appended."""
         total = 0
+        if self.lazy:
+            for i, s in enumerate(self.w.sessions):
+                k, v, q = gen_session(self.w, i, self.dev, self.scale)
+                if s.prefix > 0:
+                    sa.sa_rope_kv_append(self.pool, [self.sids[i]], [0, s.prefix], k[: s.prefix].contiguous(),
+                                         v[: s.prefix].contiguous(), None)
+                    total += s.prefix
+                self.new[i] = (k[s.prefix:].clone(), v[s.prefix:].clone(), q)
+                del k, v
+                torch.cuda.synchronize(self.dev)  # the appended slices are freed right after
+            self._build_rounds()
+            return total
         batch_s, batch_k, batch_v, lens = [], [], [], []
 
         def flush():
@@ -104,13 +126,13 @@ class Runner:
                 a, b = c * ch, min(s.new, (c + 1) * ch)
                 if a >= b:
                     continue
-                k, v, q = self.data[i]
+                k, v, q = self.new[i]
                 sids.append(self.sids[i])
                 idx.append(i)
                 starts.append(a)
                 lens.append(b - a)
-                ks.append(k[s.prefix + a: s.prefix + b])
-                vs.append(v[s.prefix + a: s.prefix + b])
+                ks.append(k[a:b])
+                vs.append(v[a:b])
                 qs.append(q[a:b])
             if not sids:
                 continue

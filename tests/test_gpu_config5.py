@@ -1,0 +1,61 @@
+"""BASELINE.json config 5 at full size (64 q heads, 8 kv heads, contexts up to 128K tokens, ~120 GB of
+pages): the oracle runs on sampled rows (reading R16), every element offset is 64-bit (the pool is
+6e10 elements and pages are handed out in random order over all of it)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_00151_b200 import binding as sa
+from paper_2607_00151_b200 import workloads as wl
+from paper_2607_00151_b200.harness import Runner, make_pool
+from paper_2607_00151_b200.workloads import gen_session
+
+from gpu_util import check_lse, check_out, oracle_session
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.timeout(1500)
+def test_config5_long_horizon_sampled():
+    free, total = torch.cuda.mem_get_info()
+    if total < 170e9:
+        pytest.skip("config 5 needs a 180 GB device")
+    w = wl.config5()
+    assert len(w.sessions) == 136 and w.layer.num_q_heads == 64
+    pool = make_pool(w, 0, "random")
+    assert sa.sa_kv_pool_storage_bytes(pool.cfg) > 115e9
+    r = Runner(w, pool, None, 0, lazy=True)
+    filled = r.fill_prefixes()
+    assert filled == sum(s.prefix for s in w.sessions)
+    r.step()
+    torch.cuda.synchronize()
+    rd = r.rounds[0]
+    assert len(rd.sids) == 136
+    st = sa.sa_mixed_attention_plan(pool, rd.sids, rd.indptr)
+    assert st["prefill_requests"] == 8 and st["decode_requests"] == 128 and st["tcgen05"] == 1
+    assert st["sum_prefill_A"] == w.pair_count() and st["sum_decode_kv"] == w.decode_kv_tokens()
+    # sessions do live in the high pages (element offsets far beyond 2^32)
+    top = max(max(sa.sa_kv_session_query(pool, s)[1]) for s in r.sids[:8])
+    assert top * pool.cfg.num_kv_heads * 64 * 128 > 2 ** 34
+    outs = r.outputs()
+    assert all(torch.isfinite(outs[i][0].float()).all() for i in range(136))
+    rng = np.random.default_rng(55)
+    pre = sorted(range(8), key=lambda i: -w.sessions[i].prefix)
+    dec = sorted(range(8, 136), key=lambda i: -w.sessions[i].prefix)
+    sample = [pre[0], pre[-1], dec[0], dec[len(dec) // 2]]   # longest + shortest prefill, longest + median decode
+    for i in sample:
+        s = w.sessions[i]
+        data = {i: gen_session(w, i, "cuda")}
+        if s.new == 1:
+            rows = np.zeros(64, dtype=np.int64)
+            heads = np.arange(64, dtype=np.int32)
+        else:
+            rows = np.concatenate([[0, s.new - 1], rng.integers(0, s.new, size=30)])
+            heads = rng.integers(0, 64, size=32).astype(np.int32)
+        ref = oracle_session(w, i, data, rows=rows, heads=heads)
+        del data
+        g = outs[i][0][torch.as_tensor(rows), torch.as_tensor(heads.astype(np.int64))]
+        gl = outs[i][1][torch.as_tensor(rows), torch.as_tensor(heads.astype(np.int64))]
+        e = check_out(g, ref["o"], "cfg5 s%d" % i)
+        check_lse(gl, ref["lse"], 1e-3, "cfg5 s%d" % i)
+        print("cfg5 session %d (prefix %d, new %d): max-abs %.2e mean-abs %.2e rel-L2 %.2e" % (i, s.prefix, s.new, *e))
