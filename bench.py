@@ -141,14 +141,17 @@ def oracle_sample(w, seconds_target: float = 15.0, seed: int = 0):
     v_prefix = orc.widen(v[:P])
     ch = s.chunk or s.new
     rng = np.random.default_rng(seed)
-    # calibrate on a few pairs, then size the sample for ~seconds_target
-    n_cal = 64
-    rows = rng.integers(0, ch, size=n_cal)
-    heads = rng.integers(0, L.num_q_heads, size=n_cal).astype(np.int32)
-    t0 = time.perf_counter()
-    orc.oracle_cached(k_rot_prefix, v_prefix, q[:ch], k[P:P + ch], v[P:P + ch], P, L.rope_base, rows=rows, heads=heads)
-    t_cal = time.perf_counter() - t0
-    n = int(max(256, min(ch * L.num_q_heads, n_cal * seconds_target / max(t_cal, 1e-3))))
+    # calibrate t = a + b*n on two small samples (a = RoPE of the chunk), then size the sample for ~seconds_target
+    def timed_sample(n_):
+        rows_ = rng.integers(0, ch, size=n_)
+        heads_ = rng.integers(0, L.num_q_heads, size=n_).astype(np.int32)
+        t0_ = time.perf_counter()
+        orc.oracle_cached(k_rot_prefix, v_prefix, q[:ch], k[P:P + ch], v[P:P + ch], P, L.rope_base, rows=rows_, heads=heads_)
+        return time.perf_counter() - t0_
+    t1, t2 = timed_sample(64), timed_sample(320)
+    b_ = max((t2 - t1) / 256.0, 1e-7)
+    a_ = max(t1 - 64 * b_, 0.0)
+    n = int(max(256, min(ch * L.num_q_heads, (seconds_target - a_) / b_)))
     rows = rng.integers(0, ch, size=n)
     heads = rng.integers(0, L.num_q_heads, size=n).astype(np.int32)
     t0 = time.perf_counter()
