@@ -94,6 +94,12 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def load_traffic():
+    """dram bytes per launch of the three kernels, from the committed ncu --set full summaries (profiles/)."""
+    p = os.path.join(ROOT, "profiles", "r1c_traffic.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
+
+
 def get_workload(cfg_id: int):
     from paper_2607_00151_b200 import workloads as wl
     return wl.CONFIGS[cfg_id]()
@@ -230,7 +236,7 @@ def measure_parts(local: int, peaks, iters: int = 10):
     ms_fill, ms_fill_min = timed(fill, max(3, iters // 2))
     app_bytes = 2.0 * kappa * tok
     app = {"bound": "hbm", "achieved": app_bytes / (ms_fill * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-           "frac": app_bytes / (ms_fill * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+           "frac": app_bytes / (ms_fill * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": load_traffic().get("rope_append_cfg4_fill"),
            "kernel": "rope_append_kernel on config 4's prefix fill: %d tokens, %d sessions, one sa_rope_kv_append call"
                      " (page allocation and block-table update included)" % (tok, len(w.sessions)),
            "bytes_per_launch": app_bytes, "ms": ms_fill, "ms_min": ms_fill_min, "peak_source": peaks["source"]}
@@ -253,7 +259,7 @@ def measure_parts(local: int, peaks, iters: int = 10):
     kv_tok = w.decode_kv_tokens()
     dec_bytes = float(kappa) * kv_tok + 2.0 * q.numel() * 2
     decode = {"bound": "hbm", "achieved": dec_bytes / (ms_dec * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-              "frac": dec_bytes / (ms_dec * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+              "frac": dec_bytes / (ms_dec * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": load_traffic().get("flash_mma_decode_cfg4"),
               "kernel": "flash_mma_kernel<128,0> (split-KV decode) + merge_splits_kernel on config 4's %d decode rows, "
                         "%d cached tokens" % (len(dec), kv_tok),
               "bytes_per_launch": dec_bytes, "ms": ms_dec, "ms_min": ms_dec_min, "peak_source": peaks["source"]}
@@ -348,7 +354,7 @@ def run_ours(args, world, rank, local):
         achieved = flops_step * args.steps / (attn_ms * 1e-3) / 1e12
         peak = peaks["bf16_tflops"]
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peaks["source"] + " (burst; sustained %.1f)" % peaks["bf16_tflops_sustained"],
+                "traffic": load_traffic().get("prefill_tc5_kernel_cfg2_avg_per_launch_est") if args.config == 2 else None, "peak_source": peaks["source"] + " (burst; sustained %.1f)" % peaks["bf16_tflops_sustained"],
                 "kernel": "prefill attention inside sa_mixed_attention (%d calls timed, avg %.3f ms; decode rows of the same "
                           "call included in the time when the workload has them)" % (n_attn, attn_ms / max(n_attn, 1)),
                 "algorithmic_flops_per_step": flops_step}
@@ -432,11 +438,18 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parts", action="store_true", help="skip the decode / append bandwidth measurements on config 4")
+    ap.add_argument("--parts-only", action="store_true", help="only the decode / append measurements (for profiling them)")
     args = ap.parse_args()
     if args.impl == "reference":
         world = int(os.environ.get("WORLD_SIZE", "1"))
         rank = int(os.environ.get("RANK", "0"))
         run_reference(args, world, rank)
+        return
+    if args.parts_only:
+        import __graft_entry__
+        __graft_entry__.build()
+        dec, app, mixed = measure_parts(0, load_peaks(), iters=3)
+        print(json.dumps({"roofline_decode": dec, "roofline_append": app, "mixed_config4": mixed}))
         return
     world, rank, local = dist_setup(args.gpus)
     run_ours(args, world, rank, local)
