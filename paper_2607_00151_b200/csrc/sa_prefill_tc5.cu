@@ -33,6 +33,11 @@ constexpr int kThreadsTc5 = 384;
 constexpr int TILE_BYTES = BN * D * 2;   // 32 KiB: two 64-wide halves of 128 rows x 128 B
 constexpr int HALF_BYTES = TILE_BYTES / 2;
 constexpr int KV_STAGES = 2;
+#ifndef SA_POLY_SHARE
+#define SA_POLY_SHARE 0  // 0: all exp2 on the MUFU; 1: one of four as an FMA-pipe cubic; 2: one of two
+                          // (measured on config 2: 1124 / 1035 / 852 TFLOP/s: the softmax warps are issue-bound,
+                          //  not MUFU-bound, so the cubic's extra instructions cost more than they save)
+#endif
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the row max grows by > 2^8
 
 struct Tc5Args {
@@ -83,16 +88,23 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
 // exp2 of one chunk, row sums, bf16 P into 16 TMEM columns.  Three of four exponentials run on
 // the MUFU, one of four as a cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
 template <bool MASKED>
-__device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], float sl2, float neg, float (&lsum)[4],
+__device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
                                                 uint32_t taddr) {
     uint32_t pk[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-        const float x0 = fmaf(__uint_as_float(s[2 * i]), sl2, neg);
-        const float x1 = fmaf(__uint_as_float(s[2 * i + 1]), sl2, neg);
+        // x = s * scale_log2 - m * scale_log2 for two columns at once (FFMA2)
+        float x0, x1;
+        unpack_f32x2(ffma2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sl2_2, neg_2), x0, x1);
         const float p0 = ex2_approx(x0);
+#if SA_POLY_SHARE == 0
+        const float p1 = ex2_approx(x1);
+#elif SA_POLY_SHARE == 1
         const float p1 = ((i & 1) && !MASKED) ? ex2_poly3(x1) : ex2_approx(x1);
-        lsum[i & 3] += p0 + p1;
+#else
+        const float p1 = (!MASKED) ? ex2_poly3(x1) : ex2_approx(x1);
+#endif
+        lsum[i & 3] = fadd2(lsum[i & 3], pack_f32x2(p0, p1));
         __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
         pk[i] = *reinterpret_cast<uint32_t *>(&pb);
     }
@@ -287,7 +299,8 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         const float sl2 = a.scale_log2;
         float m_used = -INFINITY;
 
-        float lsum[4] = {0.f, 0.f, 0.f, 0.f};  // independent partial row sums (shorter dependency chains)
+        uint64_t lsum[4] = {0ull, 0ull, 0ull, 0ull};  // 4 x f32x2 independent partial row sums
+        const uint64_t sl2_2 = pack_f32x2(sl2, sl2);
         for (int j = 0; j < n_kv; ++j) {
             mbar_wait(bar(BAR_S_FULL + t), j & 1);
             tc_fence_after();
@@ -311,8 +324,9 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             if (__any_sync(0xffffffffu, need)) {
                 const float f = need ? ex2_approx((m_used - m_new) * sl2) : 1.0f;
                 if (need) {
+                    const uint64_t f2 = pack_f32x2(f, f);
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) lsum[c] *= f;
+                    for (int c = 0; c < 4; ++c) lsum[c] = fmul2(lsum[c], f2);
                     m_used = m_new;
                 }
                 if (j > 0) {  // PV(t, j-1) has completed (it precedes QK(t, j) in the pipe); PV(t, j) waits for P
@@ -328,22 +342,28 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 }
             }
             const float neg = (m_used == -INFINITY) ? 0.f : -m_used * sl2;
+            const uint64_t neg_2 = pack_f32x2(neg, neg);
             if (masked) {
-                chunk_exp_store<true>(s0, sl2, neg, lsum, tS);
-                chunk_exp_store<true>(s1, sl2, neg, lsum, tS + 16);
-                chunk_exp_store<true>(s2, sl2, neg, lsum, tS + 32);
-                chunk_exp_store<true>(s3, sl2, neg, lsum, tS + 48);
+                chunk_exp_store<true>(s0, sl2_2, neg_2, lsum, tS);
+                chunk_exp_store<true>(s1, sl2_2, neg_2, lsum, tS + 16);
+                chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
+                chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
             } else {
-                chunk_exp_store<false>(s0, sl2, neg, lsum, tS);
-                chunk_exp_store<false>(s1, sl2, neg, lsum, tS + 16);
-                chunk_exp_store<false>(s2, sl2, neg, lsum, tS + 32);
-                chunk_exp_store<false>(s3, sl2, neg, lsum, tS + 48);
+                chunk_exp_store<false>(s0, sl2_2, neg_2, lsum, tS);
+                chunk_exp_store<false>(s1, sl2_2, neg_2, lsum, tS + 16);
+                chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
+                chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
             }
             tmem_wait_st();
             tc_fence_before();
             mbar_arrive(bar(BAR_P_FULL + t));
         }
-        const float l = (lsum[0] + lsum[1]) + (lsum[2] + lsum[3]);
+        float l;
+        {
+            float a0, a1;
+            unpack_f32x2(fadd2(fadd2(lsum[0], lsum[1]), fadd2(lsum[2], lsum[3])), a0, a1);
+            l = a0 + a1;
+        }
         // ---- epilogue: O / l -> bf16 -> out
         mbar_wait(bar(BAR_O_FULL + t), 0);
         tc_fence_after();
