@@ -34,11 +34,17 @@ constexpr int TILE_BYTES = BN * D * 2;   // 32 KiB: two 64-wide halves of 128 ro
 constexpr int HALF_BYTES = TILE_BYTES / 2;
 constexpr int KV_STAGES = 2;
 #ifndef SA_POLY_SHARE
-#define SA_POLY_SHARE 0  // 0: all exp2 on the MUFU; 1: one of four as an FMA-pipe cubic; 2: one of two
-                          // (measured on config 2: 1124 / 1035 / 852 TFLOP/s: the softmax warps are issue-bound,
-                          //  not MUFU-bound, so the cubic's extra instructions cost more than they save)
+#define SA_POLY_SHARE 0  // n of every 4 column pairs take exp2 as a packed cubic on the FMA pipe, the rest the MUFU
 #endif
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the row max grows by > 2^8
+
+#ifdef SA_TC5_TRACE
+// debug build only (-DSA_TC5_TRACE): per-iteration clock stamps of CTA 0, read back by sa_debug_tc5_trace
+__device__ long long g_tc5_trace[12][256];
+#define TC5_STAMP(slot, j) do { if (blockIdx.x == 0 && (j) < 256) g_tc5_trace[slot][j] = clock64(); } while (0)
+#else
+#define TC5_STAMP(slot, j) do { } while (0)
+#endif
 
 struct Tc5Args {
     const ReqMeta *reqs;
@@ -58,10 +64,11 @@ enum Bar {
     BAR_V_FULL = 5,   // [2]
     BAR_V_EMPTY = 7,  // [2]
     BAR_S_FULL = 9,   // [2] per Q tile
-    BAR_P_FULL = 11,  // [2]
-    BAR_O_FULL = 13,  // [2]
-    BAR_V_FIXED = 15,
-    BAR_COUNT = 16
+    BAR_P_LO = 11,    // [2] P columns of keys 0..63 of the tile are in TMEM
+    BAR_P_HI = 13,    // [2] ... keys 64..127
+    BAR_O_FULL = 15,  // [2]
+    BAR_V_FIXED = 17,
+    BAR_COUNT = 18
 };
 
 __device__ __forceinline__ int find_req_tc5(const ReqMeta *reqs, int n, int item) {
@@ -96,14 +103,14 @@ __device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_
         // x = s * scale_log2 - m * scale_log2 for two columns at once (FFMA2)
         float x0, x1;
         unpack_f32x2(ffma2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sl2_2, neg_2), x0, x1);
-        const float p0 = ex2_approx(x0);
-#if SA_POLY_SHARE == 0
-        const float p1 = ex2_approx(x1);
-#elif SA_POLY_SHARE == 1
-        const float p1 = ((i & 1) && !MASKED) ? ex2_poly3(x1) : ex2_approx(x1);
-#else
-        const float p1 = (!MASKED) ? ex2_poly3(x1) : ex2_approx(x1);
-#endif
+        // SA_POLY_SHARE n: pairs with (i % 4) < n take the packed cubic, the others the MUFU
+        float p0, p1;
+        if (!MASKED && (i & 3) < SA_POLY_SHARE) {
+            ex2_poly3_x2(x0, x1, p0, p1);
+        } else {
+            p0 = ex2_approx(x0);
+            p1 = ex2_approx(x1);
+        }
         lsum[i & 3] = fadd2(lsum[i & 3], pack_f32x2(p0, p1));
         __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
         pk[i] = *reinterpret_cast<uint32_t *>(&pb);
@@ -158,7 +165,8 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             mbar_init(bar(BAR_V_FULL + s), 1);
             mbar_init(bar(BAR_V_EMPTY + s), 1);
             mbar_init(bar(BAR_S_FULL + s), 1);
-            mbar_init(bar(BAR_P_FULL + s), BM);
+            mbar_init(bar(BAR_P_LO + s), BM);
+            mbar_init(bar(BAR_P_HI + s), BM);
             mbar_init(bar(BAR_O_FULL + s), 1);
         }
         mbar_init(bar(BAR_V_FIXED), 1);
@@ -243,11 +251,11 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                             umma_desc(sK + s * TILE_BYTES + off, 16, 1024), idesc_qk, ks > 0);
                 }
             };
-            auto issue_pv = [&](int t, int s, bool acc) {
+            auto issue_pv = [&](int t, int s, int ks0, bool acc) {  // 4 k-steps = 64 keys
 #pragma unroll
-                for (int ks = 0; ks < BN / 16; ++ks)
+                for (int ks = ks0; ks < ks0 + 4; ++ks)
                     umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8,
-                            umma_desc(sV + s * TILE_BYTES + ks * 2048, HALF_BYTES, 1024), idesc_pv, acc || ks > 0);
+                            umma_desc(sV + s * TILE_BYTES + ks * 2048, HALF_BYTES, 1024), idesc_pv, acc || ks > ks0);
             };
             mbar_wait(bar(BAR_Q), 0);
             mbar_wait(bar(BAR_K_FULL + 0), 0);
@@ -265,9 +273,14 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 else mbar_wait(bar(BAR_V_FULL + s), ph);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
-                    mbar_wait(bar(BAR_P_FULL + t), j & 1);
+                    // P arrives in two halves so that the first 64 keys' PV runs under the last exponentials
+                    mbar_wait(bar(BAR_P_LO + t), j & 1);
                     tc_fence_after();
-                    issue_pv(t, s, j > 0);
+                    TC5_STAMP(4 + t, j);  // MMA thread: first half of P_t(j) seen
+                    issue_pv(t, s, 0, j > 0);
+                    mbar_wait(bar(BAR_P_HI + t), j & 1);
+                    tc_fence_after();
+                    issue_pv(t, s, 4, true);
                     if (t == 1) umma_commit(bar(BAR_V_EMPTY + s));
                     if (has_next) {
                         if (t == 0) {
@@ -304,12 +317,14 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         for (int j = 0; j < n_kv; ++j) {
             mbar_wait(bar(BAR_S_FULL + t), j & 1);
             tc_fence_after();
+            if (row == 0) TC5_STAMP(t * 2, j);  // S_t(j) seen
             uint32_t s0[32], s1[32], s2[32], s3[32];
             tmem_ld32(tS, s0);
             tmem_ld32(tS + 32, s1);
             tmem_ld32(tS + 64, s2);
             tmem_ld32(tS + 96, s3);
             tmem_wait_ld();
+            if (row == 0 && t == 0) TC5_STAMP(6, j);  // S row in registers
             const int kt = j * BN;
             const bool masked = kt + BN - 1 > lim_min;  // uniform over the warpgroup: diagonal / last tiles only
             if (masked) {
@@ -320,6 +335,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             }
             const float mx = fmaxf(fmaxf(chunk_max(s0), chunk_max(s1)), fmaxf(chunk_max(s2), chunk_max(s3)));
             const float m_new = fmaxf(m_used, mx);
+            if (row == 0 && t == 0) TC5_STAMP(7, j);  // row max known
             const bool need = (m_new - m_used) * sl2 > kRescaleThreshold;  // true on the first live tile
             if (__any_sync(0xffffffffu, need)) {
                 const float f = need ? ex2_approx((m_used - m_new) * sl2) : 1.0f;
@@ -347,16 +363,21 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 chunk_exp_store<true>(s0, sl2_2, neg_2, lsum, tS);
                 chunk_exp_store<true>(s1, sl2_2, neg_2, lsum, tS + 16);
                 chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
-                chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
             } else {
                 chunk_exp_store<false>(s0, sl2_2, neg_2, lsum, tS);
                 chunk_exp_store<false>(s1, sl2_2, neg_2, lsum, tS + 16);
                 chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
-                chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
             }
+            tmem_wait_st();  // chunks 0..2 are in TMEM (the wait costs nothing: chunk 2's math ran meanwhile)
+            tc_fence_before();
+            mbar_arrive(bar(BAR_P_LO + t));
+            if (masked) chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
+            else chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
+            if (row == 0 && t == 0) TC5_STAMP(8, j);  // exp + P stores issued
             tmem_wait_st();
             tc_fence_before();
-            mbar_arrive(bar(BAR_P_FULL + t));
+            mbar_arrive(bar(BAR_P_HI + t));
+            if (row == 0) TC5_STAMP(t * 2 + 1, j);  // P_t(j) published
         }
         float l;
         {
@@ -419,6 +440,12 @@ EncodeTiledFn get_encode() {
 constexpr size_t kSmemTc5 = size_t(2 + 2 * KV_STAGES) * TILE_BYTES + 1024;
 
 }  // namespace
+
+#ifdef SA_TC5_TRACE
+extern "C" __attribute__((visibility("default"))) int32_t sa_debug_tc5_trace(long long *out) {
+    return cudaMemcpyFromSymbol(out, g_tc5_trace, sizeof(long long) * 12 * 256) == cudaSuccess ? 0 : -4;
+}
+#endif
 
 int32_t tc5_init(sa_kv_pool *pool) {
     pool->tc5_ready = false;

@@ -188,5 +188,24 @@ __device__ __forceinline__ float ex2_poly3(float x) {
     return __int_as_float(__float_as_int(p) + (__float_as_int(xf) << 23));
 }
 
+// the same cubic on two values at once (FADD2.RM / FFMA2): (x0, x1) -> (2^x0, 2^x1)
+__device__ __forceinline__ void ex2_poly3_x2(float x0, float x1, float &p0, float &p1) {
+    const uint64_t x2 = pack_f32x2(fmaxf(x0, -126.0f), fmaxf(x1, -126.0f));
+    const uint64_t magic = pack_f32x2(12582912.0f, 12582912.0f);
+    uint64_t xf2;
+    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(xf2) : "l"(x2), "l"(magic));
+    const uint64_t xi2 = fadd2(xf2, pack_f32x2(-12582912.0f, -12582912.0f));
+    const uint64_t fr2 = ffma2(xi2, pack_f32x2(-1.0f, -1.0f), x2);
+    uint64_t q2 = ffma2(pack_f32x2(0.07802419364452362f, 0.07802419364452362f), fr2,
+                        pack_f32x2(0.22606728971004486f, 0.22606728971004486f));
+    q2 = ffma2(q2, fr2, pack_f32x2(0.695833683013916f, 0.695833683013916f));
+    q2 = ffma2(q2, fr2, pack_f32x2(0.9999251961708069f, 0.9999251961708069f));
+    float q0, q1, f0, f1;
+    unpack_f32x2(q2, q0, q1);
+    unpack_f32x2(xf2, f0, f1);
+    p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(f0) << 23));
+    p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(f1) << 23));
+}
+
 }  // namespace ptx
 }  // namespace sa
