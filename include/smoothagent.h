@@ -133,9 +133,11 @@ SA_API int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t 
  * tokens, WHICH ALREADY CONTAINS its own q_r tokens (append first, then attend; L305 "its full
  * KV cache").  Row i of request r attends keys 0 .. kv_r - q_r + i (L311-313), softmax in fp32
  * with scale sm_scale, GQA head mapping h -> h / G.  q_r == 1 is a decode row, q_r > 1 a
- * prefill chunk, q_r == 0 a no-op; they may be mixed freely in one call.  The bits of a row's
- * output depend only on that request (co-batching changes nothing) and not on which physical
- * pages hold its cache.  Contents of page slots >= kv_r never influence a result, NaN included.
+ * prefill chunk, q_r == 0 a no-op; they may be mixed freely in one call.  The bits of a decode
+ * row's output depend only on that request; the bits of a prefill row depend on the set of
+ * prefill requests of the call (their work is balanced over the SMs by cutting items along KV,
+ * see sa_mixed_attention_schedule) and not on the decode rows co-batched with them; neither depends
+ * on which physical pages hold the cache.  Contents of page slots >= kv_r never influence a result, NaN included.
  *   q    : device bf16 [T, Hq, D], already rotated (sa_rope_kv_append's q_inout)
  *   out  : device bf16 [T, Hq, D]
  *   lse  : device f32 [T, Hq], nullable; natural-log sum-exp of the scaled scores of the row
@@ -150,11 +152,26 @@ SA_API int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t
 
 /* Host-side planner statistics of the batch sa_mixed_attention would run (no device work; works
  * on host-only pools).  out_stats (host int64[8]) = { decode-like requests, prefill requests,
- * decode CTAs, prefill CTAs, split partial rows, sum_j L_j over decode-like requests,
+ * decode CTAs, prefill work items (parts of the schedule on the tcgen05 path), split partial rows, sum_j L_j over decode-like requests,
  * sum_j A_j over prefill requests (A_j = q_j*prefix_j + q_j(q_j+1)/2, L313), 1 if prefill chunks
  * run on the tcgen05 kernel else 0 }. */
 SA_API int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                 const int32_t *qo_indptr, int64_t *out_stats);
+
+/* The static schedule the tcgen05 prefill kernel would run for this batch (host only; works on
+ * host-only pools; SA_ERR_UNSUPPORTED when prefill chunks do not take the tcgen05 path).  An item is
+ * (request, kv head, tile of 256 packed rows: row rho = token*G + head-in-group); its cost is n_kv =
+ * the number of 128-key tiles it attends to (the causal work A_j of L313 in tiles).  Items are
+ * assigned to one persistent CTA per SM; an item that does not fit under the balanced makespan is
+ * cut along KV into parts [u0, u1) whose partial results are merged in KV order.
+ *   out_parts (host int32 [cap][8], nullable): per part {cta, request index in the caller's list,
+ *       kv head, tile, u0, u1, n_kv, partial slot or -1 for a whole item}, grouped by CTA in
+ *       execution order; at most cap rows are written
+ *   out_summary (host int64 [6]): {CTAs, parts, split items, partial slots, sum of n_kv over
+ *       items, largest CTA load in tiles incl. the fixed cost per part} */
+SA_API int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                    const int32_t *qo_indptr, int32_t *out_parts, int32_t cap,
+                                    int64_t *out_summary);
 
 /* Number of kernel launches the last successful sa_mixed_attention / sa_rope_kv_append on this
  * pool enqueued (for launch accounting in benchmarks). */

@@ -75,6 +75,7 @@ PROTOTYPES = {
     "sa_mixed_attention_workspace_bytes": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_mixed_attention": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _vp, _vp, _vp, ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
     "sa_mixed_attention_plan": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _i64p]),
+    "sa_mixed_attention_schedule": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _i32p, ctypes.c_int32, _i64p]),
     "sa_last_launch_count": (ctypes.c_int32, [_vp, _i32p]),
     "sa_latency_table": (ctypes.c_int32, [_vp, _i32p, ctypes.c_int32, _i32p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
                                           ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32, ctypes.c_int32, _f32p, _i64p, _vp]),
@@ -278,6 +279,21 @@ def sa_mixed_attention_plan(pool: Pool, sids, qo_indptr) -> dict:
     keys = ["decode_requests", "prefill_requests", "decode_ctas", "prefill_ctas", "partial_rows", "sum_decode_kv",
             "sum_prefill_A", "tcgen05"]
     return dict(zip(keys, (int(x) for x in st)))
+
+
+def sa_mixed_attention_schedule(pool: Pool, sids, qo_indptr):
+    """-> (parts int32 [n_parts, 8] = (cta, request, kv head, tile, u0, u1, n_kv, slot), summary dict)"""
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    lib = load_library()
+    sm = np.zeros(6, dtype=np.int64)
+    _check(lib.sa_mixed_attention_schedule(pool.handle, s_keep.shape[0], s_ptr, i_ptr, None, 0, sm.ctypes.data_as(_i64p)),
+           "sa_mixed_attention_schedule")
+    parts = np.zeros((int(sm[1]), 8), dtype=np.int32)
+    _check(lib.sa_mixed_attention_schedule(pool.handle, s_keep.shape[0], s_ptr, i_ptr, parts.ctypes.data_as(_i32p),
+                                           parts.shape[0], sm.ctypes.data_as(_i64p)), "sa_mixed_attention_schedule")
+    keys = ["ctas", "parts", "split_items", "slots", "total_units", "makespan"]
+    return parts, dict(zip(keys, (int(x) for x in sm)))
 
 
 def sa_last_launch_count(pool: Pool) -> int:

@@ -3,6 +3,7 @@
 // lookahead (BE) prefill chunks are co-batched with LC decode rows; L311-313
 // and L305 define what each row attends to.
 #include <math.h>
+#include <string.h>
 
 #include <algorithm>
 #include <vector>
@@ -22,6 +23,8 @@ struct HostPlan {
     int64_t sum_decode_kv = 0;   // sum_j L_j over decode-like requests   (Eq. 1, alpha_d term)
     int64_t sum_prefill_A = 0;   // sum_j A_j over prefill requests       (Eq. 1, alpha_p term)
     bool use_tc5 = false;
+    Tc5Schedule sched;            // tcgen05 path: parts per persistent CTA, merges of split items
+    std::vector<int32_t> pre_orig;  // prefill request -> index in the caller's request list
 };
 
 // The split of a request depends only on that request (never on its batch), so co-batching
@@ -34,6 +37,7 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
     const int G = pool->G, Hq = pool->cfg.num_q_heads, Hkv = pool->cfg.num_kv_heads;
     hp->use_tc5 = tc5_supported(pool);
     const int tile_m = hp->use_tc5 ? kTc5TileM : kLegacyTileM;
+    std::vector<std::pair<ReqMeta, int32_t>> pre;
     for (int r = 0; r < n_req; ++r) {
         const int32_t sid = sids[r];
         if (sid < 0 || size_t(sid) >= pool->sessions.size() || !pool->sessions[size_t(sid)].open) return SA_ERR_INVALID_ARG;
@@ -52,14 +56,19 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
             hp->sum_decode_kv += kv * n;
         } else {
             m.n_tiles = int32_t((n * G + tile_m - 1) / tile_m);
-            hp->pre.push_back(m);
+            pre.push_back(std::make_pair(m, int32_t(r)));
             hp->sum_prefill_A += n * (kv - n) + n * (n + 1) / 2;
         }
     }
     hp->total_q = qo_indptr[n_req];
     // prefill: longest context first (its tiles carry the most work)
-    std::stable_sort(hp->pre.begin(), hp->pre.end(),
-                     [](const ReqMeta &a, const ReqMeta &b) { return a.kv_len > b.kv_len; });
+    std::stable_sort(pre.begin(), pre.end(), [](const std::pair<ReqMeta, int32_t> &a, const std::pair<ReqMeta, int32_t> &b) {
+        return a.first.kv_len > b.first.kv_len;
+    });
+    for (const auto &pr : pre) {
+        hp->pre.push_back(pr.first);
+        hp->pre_orig.push_back(pr.second);
+    }
     int64_t items = 0, parts = 0, rows = 0;
     for (ReqMeta &m : hp->dec) {
         m.item_begin = int32_t(items);
@@ -81,12 +90,35 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
     if (items > INT32_MAX) return SA_ERR_UNSUPPORTED;
     hp->plan.n_pre = int32_t(hp->pre.size());
     hp->plan.pre_items = int32_t(items);
+    if (hp->use_tc5 && !hp->pre.empty()) {
+        tc5_schedule(hp->pre, G, Hkv, pool->num_sms, &hp->sched);
+        hp->plan.pre_items = int32_t(hp->sched.parts.size());
+    }
     return SA_OK;
 }
 
-size_t workspace_need(const sa_kv_pool *pool, const HostPlan &hp) {
+// workspace: [decode partial O f32][decode partial lse f32][tcgen05 partial slots][tcgen05 schedule payload]
+struct WsLayout {
+    size_t off_part_lse, off_slots, off_sched, total;
+};
+WsLayout workspace_layout(const sa_kv_pool *pool, const HostPlan &hp) {
     const size_t D = size_t(pool->cfg.head_dim);
-    return align_up(size_t(hp.plan.part_rows) * D * 4, 256) + align_up(size_t(hp.plan.part_rows) * 4, 256) + 256;
+    WsLayout w;
+    w.off_part_lse = align_up(size_t(hp.plan.part_rows) * D * 4, 256);
+    w.off_slots = w.off_part_lse + align_up(size_t(hp.plan.part_rows) * 4, 256);
+    w.off_sched = w.off_slots + align_up(size_t(hp.sched.n_slots) * kTc5SlotBytes, 256);
+    w.total = w.off_sched + align_up(hp.sched.parts.empty() ? 0 : hp.sched.payload_bytes(), 256) + 256;
+    return w;
+}
+size_t workspace_need(const sa_kv_pool *pool, const HostPlan &hp) { return workspace_layout(pool, hp).total; }
+
+void write_sched_payload(const Tc5Schedule &sc, char *dst) {
+    const size_t off_parts = (sc.cta_begin.size() * 4 + 31) / 32 * 32;
+    memset(dst, 0, off_parts);
+    memcpy(dst, sc.cta_begin.data(), sc.cta_begin.size() * 4);
+    if (!sc.parts.empty()) memcpy(dst + off_parts, sc.parts.data(), sc.parts.size() * sizeof(Tc5Part));
+    if (!sc.merges.empty())
+        memcpy(dst + off_parts + sc.parts.size() * sizeof(Tc5Part), sc.merges.data(), sc.merges.size() * sizeof(Tc5Merge));
 }
 
 }  // namespace
@@ -119,6 +151,39 @@ extern "C" int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req
     return SA_OK;
 }
 
+extern "C" int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                               const int32_t *qo_indptr, int32_t *out_parts, int32_t cap,
+                                               int64_t *out_summary) {
+    if (!out_summary || cap < 0) return SA_ERR_INVALID_ARG;
+    sa::HostPlan hp;
+    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hp);
+    if (st != SA_OK) return st;
+    if (!sa::tc5_supported(pool)) return SA_ERR_UNSUPPORTED;
+    const sa::Tc5Schedule &sc = hp.sched;
+    out_summary[0] = pool->num_sms;
+    out_summary[1] = int64_t(sc.parts.size());
+    out_summary[2] = int64_t(sc.merges.size());
+    out_summary[3] = sc.n_slots;
+    out_summary[4] = sc.total_units;
+    out_summary[5] = sc.makespan;
+    if (out_parts) {
+        const size_t n = std::min(size_t(cap), sc.parts.size());
+        for (size_t i = 0; i < n; ++i) {
+            const sa::Tc5Part &p = sc.parts[i];
+            int32_t *o = out_parts + 8 * i;
+            o[0] = p.cta;
+            o[1] = hp.pre_orig[size_t(p.req)];
+            o[2] = p.g;
+            o[3] = p.tile;
+            o[4] = p.u0;
+            o[5] = p.u1;
+            o[6] = p.n_kv;
+            o[7] = p.slot;
+        }
+    }
+    return SA_OK;
+}
+
 extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
                                       const void *q, void *out, float *lse, float sm_scale, void *workspace,
                                       size_t workspace_bytes, void *stream_) {
@@ -130,30 +195,53 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     pool->last_launches = 0;
     if (hp.plan.n_dec + hp.plan.n_pre == 0) return SA_OK;
     if (!q || !out) return SA_ERR_INVALID_ARG;
-    const size_t need = workspace_need(pool, hp);
-    if (hp.plan.part_rows > 0 && (!workspace || workspace_bytes < need)) return SA_ERR_WORKSPACE_TOO_SMALL;
+    const WsLayout wl = workspace_layout(pool, hp);
+    const bool needs_ws = hp.plan.part_rows > 0 || !hp.sched.parts.empty();
+    if (needs_ws && (!workspace || workspace_bytes < wl.total)) return SA_ERR_WORKSPACE_TOO_SMALL;
     if (!(sm_scale > 0.f)) sm_scale = 1.0f / sqrtf(float(pool->cfg.head_dim));
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    uintptr_t w = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255);
 
+    // per-call metadata: [decode ReqMeta][prefill ReqMeta][tcgen05 schedule] through the pinned slab ring; a
+    // schedule too long for the slab goes through the pool's growable pinned buffer into the workspace
     char *mh = nullptr, *md = nullptr;
     st = acquire_meta(pool, &mh, &md);
     if (st != SA_OK) return st;
     const size_t dec_bytes = sizeof(ReqMeta) * hp.dec.size(), pre_bytes = sizeof(ReqMeta) * hp.pre.size();
+    const size_t sched_bytes = hp.sched.parts.empty() ? 0 : hp.sched.payload_bytes();
+    const size_t off_sched = align_up(dec_bytes + pre_bytes, 32);
     if (dec_bytes) memcpy(mh, hp.dec.data(), dec_bytes);
     if (pre_bytes) memcpy(mh + dec_bytes, hp.pre.data(), pre_bytes);
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    if (commit_meta(pool, dec_bytes + pre_bytes, stream) != SA_OK) return SA_ERR_CUDA;
+    const char *sched_dev = nullptr;
+    size_t slab_used = dec_bytes + pre_bytes;
+    if (sched_bytes > 0) {
+        if (off_sched + sched_bytes <= pool->meta_slab_bytes) {
+            write_sched_payload(hp.sched, mh + off_sched);
+            sched_dev = md + off_sched;
+            slab_used = off_sched + sched_bytes;
+        } else {
+            char *big = nullptr;
+            st = acquire_big_meta(pool, sched_bytes, &big);
+            if (st != SA_OK) return st;
+            write_sched_payload(hp.sched, big);
+            char *dst = reinterpret_cast<char *>(w + wl.off_sched);
+            if (commit_big_meta(pool, dst, sched_bytes, stream) != SA_OK) return SA_ERR_CUDA;
+            sched_dev = dst;
+        }
+    }
+    if (commit_meta(pool, slab_used, stream) != SA_OK) return SA_ERR_CUDA;
     const ReqMeta *dec_dev = reinterpret_cast<const ReqMeta *>(md);
     const ReqMeta *pre_dev = reinterpret_cast<const ReqMeta *>(md + dec_bytes);
 
-    // workspace carve-up: [partial O f32][partial lse f32]
-    uintptr_t w = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255);
     float *part_o = reinterpret_cast<float *>(w);
-    float *part_lse = reinterpret_cast<float *>(w + align_up(size_t(hp.plan.part_rows) * size_t(pool->cfg.head_dim) * 4, 256));
+    float *part_lse = reinterpret_cast<float *>(w + wl.off_part_lse);
+    char *tc5_partials = reinterpret_cast<char *>(w + wl.off_slots);
 
     // prefill first: it is the long pole; the decode kernel fills in behind it on the same stream
     cudaError_t e;
     if (hp.use_tc5)
-        e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.total_q, q, out, lse, sm_scale, stream, &pool->last_launches);
+        e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.sched, sched_dev, tc5_partials, hp.total_q, q, out, lse, sm_scale,
+                               stream, &pool->last_launches);
     else
         e = launch_flash_prefill_legacy(pool, pre_dev, hp.plan, q, out, lse, sm_scale, stream, &pool->last_launches);
     if (e != cudaSuccess) return SA_ERR_CUDA;

@@ -16,6 +16,11 @@ constexpr int kDecodeSplitKeys = 1024;  // split-KV granularity of decode-like r
 constexpr int kLegacyTileM = 64;        // packed rows per CTA of the mma.sync prefill kernel
 constexpr int kTc5TileM = 256;          // packed rows per CTA of the tcgen05 prefill kernel
 constexpr int kMaxChunkLatency = 2048;  // sa_latency_table prefill chunk size
+constexpr int kTc5KeysPerUnit = 128;    // one schedule unit of the tcgen05 kernel = one 128-key KV tile of an item
+constexpr int kTc5FixedCost = 3;        // per-part overhead (Q load, first QK, epilogue) in schedule units
+constexpr int kTc5MinPart = 4;          // never cut a part shorter than this many units
+// one partial result of a split item: unnormalised O f32 [256][128], then (m * scale_log2, l) f32 [256][2]
+constexpr size_t kTc5SlotBytes = size_t(kTc5TileM) * 128 * 4 + size_t(kTc5TileM) * 2 * 4;
 
 // One request of a hot call as the kernels see it (device copy lives in the metadata ring).
 struct ReqMeta {
@@ -28,6 +33,36 @@ struct ReqMeta {
     int32_t part_begin;  // decode-like class: first partial row ([split][token][head])
     int32_t n_tiles;     // prefill class: packed-row tiles per kv head
 };
+
+// tcgen05 prefill kernel: one persistent CTA per SM walks a list of parts.  An item is (request, kv
+// head, 256 packed rows); a part is the KV-tile range [u0, u1) of an item.  slot < 0: the part is the
+// whole item and writes the output directly; otherwise it writes partial slot `slot` and the merge
+// kernel combines the item's parts (consecutive slots, KV order).
+struct Tc5Part {
+    int32_t req;    // index into the prefill ReqMeta array of the call
+    int32_t g;      // kv head
+    int32_t tile;   // 256-row tile of the request's packed rows
+    int32_t u0, u1; // KV tiles [u0, u1) of the item's n_kv
+    int32_t slot;   // partial slot, or -1
+    int32_t n_kv;   // KV tiles of the whole item
+    int32_t cta;    // CTA that runs it (host-side bookkeeping)
+};
+struct Tc5Merge {
+    int32_t req, g, tile, slot0, n_parts, pad0, pad1, pad2;
+};
+struct Tc5Schedule {
+    std::vector<int32_t> cta_begin;  // [n_cta + 1] into parts
+    std::vector<Tc5Part> parts;      // grouped by CTA, execution order
+    std::vector<Tc5Merge> merges;
+    int32_t n_slots = 0;
+    int64_t total_units = 0;         // sum of n_kv over items
+    int64_t makespan = 0;            // largest CTA load in units (incl. fixed costs)
+    size_t payload_bytes() const {
+        return (cta_begin.size() * 4 + 31) / 32 * 32 + parts.size() * sizeof(Tc5Part) + merges.size() * sizeof(Tc5Merge);
+    }
+};
+// Static schedule of the prefill items of a call over n_cta persistent CTAs (sa_tc5_schedule.cu).
+void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc5Schedule *out);
 
 struct Session {
     bool open = false;
@@ -60,6 +95,10 @@ struct sa_kv_pool {
     cudaEvent_t meta_event[sa::kMetaRing] = {};
     bool meta_event_used[sa::kMetaRing] = {};
     int meta_next = 0;
+    char *big_host = nullptr;   // pinned, grown on demand: metadata too long for a slab (long tcgen05 schedules)
+    size_t big_cap = 0;
+    cudaEvent_t big_event = nullptr;
+    bool big_event_used = false;
     std::vector<int32_t> free_pages;  // stack: back() is handed out next
     std::vector<sa::Session> sessions;
     int32_t last_launches = 0;
@@ -77,6 +116,10 @@ namespace sa {
 // copy if it is still in flight.  commit_meta enqueues the H2D copy of `bytes` bytes.
 int32_t acquire_meta(sa_kv_pool *pool, char **host, char **dev);
 int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream);
+// Metadata that does not fit a slab: one growable pinned buffer (waits for its previous copy),
+// copied to a device address of the caller's workspace.
+int32_t acquire_big_meta(sa_kv_pool *pool, size_t bytes, char **host);
+int32_t commit_big_meta(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream);
 
 // --- kernel launchers (each returns a cudaError_t from the launch) ---
 cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
@@ -100,7 +143,9 @@ cudaError_t launch_flash_prefill_legacy(const sa_kv_pool *pool, const ReqMeta *r
 // tcgen05 path (sa_prefill_tc5.cu)
 int32_t tc5_init(sa_kv_pool *pool);  // builds the TMA descriptors; SA_OK or SA_ERR_CUDA
 bool tc5_supported(const sa_kv_pool *pool);
+// sched_dev: the schedule payload on the device ([cta_begin][parts][merges]); partials: n_slots slots
 cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
+                               const Tc5Schedule &sched, const char *sched_dev, char *partials,
                                int64_t total_q, const void *q, void *out, float *lse, float sm_scale,
                                cudaStream_t stream, int32_t *launches);
 

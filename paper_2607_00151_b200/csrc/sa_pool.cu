@@ -38,7 +38,8 @@ Carve carve(const sa_kv_pool_config *c) {
     Carve r;
     r.mpps = (c->max_session_tokens + c->page_size - 1) / c->page_size;
     r.kv_bytes = size_t(c->num_pages) * c->num_kv_heads * c->page_size * c->head_dim * 2;
-    r.slab = align_up(2 * sizeof(sa::ReqMeta) * (size_t(c->max_sessions) + 8) + 4 * size_t(c->num_pages) + 64, 256);
+    // room for the requests of a call, the new page ids of an append, and a tcgen05 schedule of ~2000 parts
+    r.slab = align_up(2 * sizeof(sa::ReqMeta) * (size_t(c->max_sessions) + 8) + 4 * size_t(c->num_pages) + 64 + (64 << 10), 256);
     size_t off = 0;
     r.k_off = off;
     off = align_up(off + r.kv_bytes, 1024);
@@ -121,6 +122,7 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
         ok = ok && cudaMallocHost(reinterpret_cast<void **>(&pool->meta_host), cv.slab * sa::kMetaRing) == cudaSuccess;
         for (int i = 0; ok && i < sa::kMetaRing; ++i)
             ok = cudaEventCreateWithFlags(&pool->meta_event[i], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&pool->big_event, cudaEventDisableTiming) == cudaSuccess;
         int sms = 0;
         ok = ok && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cfg->device) == cudaSuccess;
         if (ok) {
@@ -158,6 +160,11 @@ extern "C" int32_t sa_kv_pool_destroy(sa_kv_pool *pool) {
             }
         }
         if (pool->meta_host) cudaFreeHost(pool->meta_host);
+        if (pool->big_event) {
+            if (pool->big_event_used) cudaEventSynchronize(pool->big_event);
+            cudaEventDestroy(pool->big_event);
+        }
+        if (pool->big_host) cudaFreeHost(pool->big_host);
     }
     delete pool;
     return SA_OK;
@@ -260,6 +267,33 @@ int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream) {
     if (cudaEventRecord(pool->meta_event[i], stream) != cudaSuccess) return SA_ERR_CUDA;
     pool->meta_event_used[i] = true;
     pool->meta_next = (i + 1) % kMetaRing;
+    return SA_OK;
+}
+
+int32_t acquire_big_meta(sa_kv_pool *pool, size_t bytes, char **host) {
+    if (pool->big_event_used) {
+        if (cudaEventSynchronize(pool->big_event) != cudaSuccess) return SA_ERR_CUDA;
+        pool->big_event_used = false;
+    }
+    if (bytes > pool->big_cap) {
+        if (pool->big_host) cudaFreeHost(pool->big_host);
+        pool->big_host = nullptr;
+        pool->big_cap = 0;
+        const size_t cap = std::max(bytes * 2, size_t(1) << 20);
+        if (cudaMallocHost(reinterpret_cast<void **>(&pool->big_host), cap) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return SA_ERR_CUDA;
+        }
+        pool->big_cap = cap;
+    }
+    *host = pool->big_host;
+    return SA_OK;
+}
+
+int32_t commit_big_meta(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream) {
+    if (cudaMemcpyAsync(dev_dst, pool->big_host, bytes, cudaMemcpyHostToDevice, stream) != cudaSuccess) return SA_ERR_CUDA;
+    if (cudaEventRecord(pool->big_event, stream) != cudaSuccess) return SA_ERR_CUDA;
+    pool->big_event_used = true;
     return SA_OK;
 }
 

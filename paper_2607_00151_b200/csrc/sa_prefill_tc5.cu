@@ -2,13 +2,17 @@
 // (chunk j has q_j query tokens over prefix_j cached
 // tokens, "the i-th query token attends to prefix_j + i + 1 tokens"; compute-bound, cost ~ A_j).
 //
-// One CTA = one (request, kv head, 256 packed rows) work item; packed row rho is
-// (token rho / G, q head g*G + rho % G), so the G query heads of a group share every K/V tile.
+// An item = one (request, kv head, 256 packed rows); packed row rho is (token rho / G, q head
+// g*G + rho % G), so the G query heads of a group share every K/V tile.  The kernel is persistent:
+// one CTA per SM walks the list of parts (KV-tile ranges of items) that the host schedule
+// (sa_tc5_schedule.cu) gave it; a part that is a whole item writes the output, a part of a split
+// item writes an fp32 partial and tc5_merge_kernel combines the item's parts in KV order.
 // The 256 rows are two 128-row Q tiles that ping-pong: while the softmax warps of one tile work
 // on S, the tensor core runs the other tile's MMAs.  Warp roles (384 threads):
-//   warp 0      TMA producer: Q tiles once, then page-gathered K and V tiles (2-stage rings);
-//               zero-fills V rows past the end of the session in the last tile
-//   warp 1      MMA issuer (one lane): S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM, V MN-major)
+//   warp 0      TMA producer (one lane): Q tiles of the part, then page-gathered K and V tiles
+//               (2-stage rings); runs ahead across part boundaries
+//   warp 1      MMA issuer: S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM, V MN-major); zeroes
+//               the V rows past the end of the session in an item's last tile
 //   warp 2      TMEM allocator
 //   warps 4-7   softmax of Q tile 0 (thread = row): S from TMEM, mask, lazy-rescaled online
 //   warps 8-11  softmax of Q tile 1   softmax, P (bf16) back into the S columns, epilogue
@@ -38,17 +42,22 @@ constexpr int KV_STAGES = 2;
 #endif
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the row max grows by > 2^8
 
-#ifdef SA_TC5_TRACE
-// debug build only (-DSA_TC5_TRACE): per-iteration clock stamps of CTA 0, read back by sa_debug_tc5_trace
-__device__ long long g_tc5_trace[12][256];
-#define TC5_STAMP(slot, j) do { if (blockIdx.x == 0 && (j) < 256) g_tc5_trace[slot][j] = clock64(); } while (0)
-#else
-#define TC5_STAMP(slot, j) do { } while (0)
+#ifdef SA_TC5_PROBE
+// debug build only (-DSA_TC5_PROBE): per-CTA (clock64, globaltimer) at start and end, read back by sa_debug_tc5_probe
+__device__ unsigned long long g_tc5_probe[256][4];
+__device__ __forceinline__ unsigned long long gtimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
 #endif
 
 struct Tc5Args {
     const ReqMeta *reqs;
-    int32_t n_reqs;
+    const int32_t *cta_begin;  // [gridDim.x + 1] into parts
+    const Tc5Part *parts;
+    const Tc5Merge *merges;
+    char *partials;            // [n_slots] x kTc5SlotBytes
     const int32_t *block_table;
     int64_t mpps;
     __nv_bfloat16 *out;
@@ -58,26 +67,49 @@ struct Tc5Args {
 };
 
 enum Bar {
-    BAR_Q = 0,
-    BAR_K_FULL = 1,   // [2]
-    BAR_K_EMPTY = 3,  // [2]
-    BAR_V_FULL = 5,   // [2]
-    BAR_V_EMPTY = 7,  // [2]
-    BAR_S_FULL = 9,   // [2] per Q tile
-    BAR_P_LO = 11,    // [2] P columns of keys 0..63 of the tile are in TMEM
-    BAR_P_HI = 13,    // [2] ... keys 64..127
-    BAR_O_FULL = 15,  // [2]
-    BAR_V_FIXED = 17,
-    BAR_COUNT = 18
+    BAR_Q_FULL = 0,
+    BAR_Q_EMPTY = 1,
+    BAR_K_FULL = 2,   // [2]
+    BAR_K_EMPTY = 4,  // [2]
+    BAR_V_FULL = 6,   // [2]
+    BAR_V_EMPTY = 8,  // [2]
+    BAR_S_FULL = 10,  // [2] per Q tile
+    BAR_P_LO = 12,    // [2] P columns of keys 0..63 of the tile are in TMEM
+    BAR_P_HI = 14,    // [2] ... keys 64..127
+    BAR_O_FULL = 16,  // [2] all PV products of the part have landed in O_t
+    BAR_O_EMPTY = 18, // [2] the epilogue has read O_t out of TMEM
+    BAR_COUNT = 20
 };
 
-__device__ __forceinline__ int find_req_tc5(const ReqMeta *reqs, int n, int item) {
-    int lo = 0, hi = n - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (reqs[mid].item_begin <= item) lo = mid; else hi = mid - 1;
-    }
-    return lo;
+// Everything a role needs to know about one part; every role derives the same values.
+struct PartGeom {
+    ReqMeta r;
+    int g, rho0, base_lim, u0, u1, slot, pages_needed, valid_last;
+    bool fix_last;  // the part ends on the item's last KV tile and that tile has rows past the session end
+};
+
+template <int LOG2B>
+__device__ __forceinline__ PartGeom load_part(const Tc5Args &a, int p) {
+    constexpr int B = 1 << LOG2B;
+    constexpr int PAGES_PER_TILE = BN / B;
+    const Tc5Part pt = a.parts[p];
+    PartGeom gm;
+    gm.r = a.reqs[pt.req];
+    gm.g = pt.g;
+    gm.u0 = pt.u0;
+    gm.u1 = pt.u1;
+    gm.slot = pt.slot;
+    gm.rho0 = pt.tile * (2 * BM);
+    gm.base_lim = gm.r.kv_len - gm.r.q_len;
+    const int tok_max = min(gm.r.q_len - 1, (gm.rho0 + 2 * BM - 1) >> a.log2G);
+    const int k_end = gm.base_lim + tok_max + 1;                   // keys [0, k_end) are needed
+    const int n_kv = (k_end + BN - 1) / BN;
+    gm.pages_needed = (k_end + B - 1) >> LOG2B;
+    // last tile: rows at or past `valid_last` hold no session data (unloaded pages or slots >= kv_len)
+    const int last_pages = min(PAGES_PER_TILE, gm.pages_needed - (n_kv - 1) * PAGES_PER_TILE);
+    gm.valid_last = min(gm.r.kv_len - (n_kv - 1) * BN, last_pages * B);
+    gm.fix_last = pt.u1 == n_kv && gm.valid_last < BN;
+    return gm;
 }
 
 // ---- per-chunk pieces of the softmax (a chunk = 32 of the 128 S columns of a row, in registers)
@@ -92,8 +124,8 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
     for (int i = 1; i < 31; i += 2) m = fmaxf(fmaxf(m, __uint_as_float(s[i])), __uint_as_float(s[i + 1]));
     return fmaxf(m, __uint_as_float(s[31]));
 }
-// exp2 of one chunk, row sums, bf16 P into 16 TMEM columns.  Three of four exponentials run on
-// the MUFU, one of four as a cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
+// exp2 of one chunk, row sums, bf16 P into 16 TMEM columns.  SA_POLY_SHARE of every four column
+// pairs take the packed cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
 template <bool MASKED>
 __device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
                                                 uint32_t taddr) {
@@ -103,7 +135,6 @@ __device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_
         // x = s * scale_log2 - m * scale_log2 for two columns at once (FFMA2)
         float x0, x1;
         unpack_f32x2(ffma2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sl2_2, neg_2), x0, x1);
-        // SA_POLY_SHARE n: pairs with (i % 4) < n take the packed cubic, the others the MUFU
         float p0, p1;
         if (!MASKED && (i & 3) < SA_POLY_SHARE) {
             ex2_poly3_x2(x0, x1, p0, p1);
@@ -126,6 +157,16 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     constexpr int PAGES_PER_TILE = BN / B;
     constexpr uint32_t PAGE_HALF_BYTES = B * 128;  // one page, one 64-wide half: B rows x 128 B
 
+    // ---- the parts of this persistent CTA (uniform over the CTA: an idle CTA leaves at once)
+    const int pb = a.cta_begin[blockIdx.x], pe = a.cta_begin[blockIdx.x + 1];
+    if (pb == pe) return;
+#ifdef SA_TC5_PROBE
+    if (threadIdx.x == 0) {
+        g_tc5_probe[blockIdx.x][0] = clock64();
+        g_tc5_probe[blockIdx.x][1] = gtimer();
+    }
+#endif
+
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t sQ = smem_u32(smem);                 // 2 tiles x 32 KiB
@@ -138,27 +179,9 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
-    // ---- work item
-    const int item = blockIdx.x;
-    const ReqMeta r = a.reqs[find_req_tc5(a.reqs, a.n_reqs, item)];
-    const int local = item - r.item_begin;
-    const int g = local / r.n_tiles;
-    const int tile = r.n_tiles - 1 - local % r.n_tiles;  // late (heavy) tiles first
-    const int G = 1 << a.log2G;
-    const int n_rows = r.q_len * G;
-    const int rho0 = tile * (2 * BM);
-    const int base_lim = r.kv_len - r.q_len;
-    const int tok_max = min(r.q_len - 1, (rho0 + 2 * BM - 1) >> a.log2G);
-    const int k_end = base_lim + tok_max + 1;                   // keys [0, k_end) are needed
-    const int n_kv = (k_end + BN - 1) / BN;
-    const int pages_needed = (k_end + B - 1) >> LOG2B;
-    // last tile: rows at or past `valid_last` hold no session data (unloaded pages or slots >= kv_len)
-    const int last_pages = min(PAGES_PER_TILE, pages_needed - (n_kv - 1) * PAGES_PER_TILE);
-    const int valid_last = min(r.kv_len - (n_kv - 1) * BN, last_pages * B);
-    const bool need_fix = valid_last < BN;
-
     if (tid == 0) {
-        mbar_init(bar(BAR_Q), 1);
+        mbar_init(bar(BAR_Q_FULL), 1);
+        mbar_init(bar(BAR_Q_EMPTY), 1);
         for (int s = 0; s < 2; ++s) {
             mbar_init(bar(BAR_K_FULL + s), 1);
             mbar_init(bar(BAR_K_EMPTY + s), 1);
@@ -168,8 +191,8 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             mbar_init(bar(BAR_P_LO + s), BM);
             mbar_init(bar(BAR_P_HI + s), BM);
             mbar_init(bar(BAR_O_FULL + s), 1);
+            mbar_init(bar(BAR_O_EMPTY + s), BM);
         }
-        mbar_init(bar(BAR_V_FIXED), 1);
         fence_mbar_init();
     }
     if (warp == 2) tmem_alloc<512>(smem_u32(&tmem_base_smem));
@@ -178,7 +201,9 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     tc_fence_after();
     const uint32_t tmem = tmem_base_smem;
 
-    // register budget: the 8 softmax warps hold a 128-column S row per thread; the others need few
+    // Phase bookkeeping shared by all roles: kc counts the KV tiles this CTA has gone through (K/V
+    // ring stage kc & 1, ring phase (kc >> 1) & 1; S/P barriers complete once per tile: phase
+    // kc & 1), pc = p - pb counts its parts (Q, O barriers: phase pc & 1).
     // (setmaxnreg sits inside each role branch so that no control-flow merge follows it)
 
     if (warp == 0) {
@@ -188,113 +213,140 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             prefetch_tmap(&tmap_q);
             prefetch_tmap(&tmap_k);
             prefetch_tmap(&tmap_v);
-            mbar_expect_tx(bar(BAR_Q), 2 * TILE_BYTES);
+            int kc = 0;
+            for (int p = pb; p < pe; ++p) {
+                const PartGeom gm = load_part<LOG2B>(a, p);
+                // Q of this part may land once every QK product of the previous part has read its Q
+                if (p > pb) mbar_wait(bar(BAR_Q_EMPTY), (p - pb - 1) & 1);
+                mbar_expect_tx(bar(BAR_Q_FULL), 2 * TILE_BYTES);
 #pragma unroll
-            for (int t = 0; t < 2; ++t) {
-                const int tok0 = r.q_start + ((rho0 + t * BM) >> a.log2G);
+                for (int t = 0; t < 2; ++t) {
+                    const int tok0 = gm.r.q_start + ((gm.rho0 + t * BM) >> a.log2G);
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
-                    tma_load_3d(sQ + t * TILE_BYTES + h * HALF_BYTES, &tmap_q, bar(BAR_Q), h * 64, g << a.log2G, tok0);
+                    for (int h = 0; h < 2; ++h)
+                        tma_load_3d(sQ + t * TILE_BYTES + h * HALF_BYTES, &tmap_q, bar(BAR_Q_FULL), h * 64, gm.g << a.log2G, tok0);
+                }
+                const int32_t *bt = a.block_table + int64_t(gm.r.sid) * a.mpps;
+                for (int j = gm.u0; j < gm.u1; ++j, ++kc) {
+                    const int s = kc & 1, ph = (kc >> 1) & 1;
+                    const int p0 = j * PAGES_PER_TILE;
+                    const int np = min(PAGES_PER_TILE, gm.pages_needed - p0);
+                    int32_t pg[PAGES_PER_TILE];
+#pragma unroll
+                    for (int u = 0; u < PAGES_PER_TILE; ++u) pg[u] = u < np ? __ldg(bt + p0 + u) : 0;
+                    mbar_wait(bar(BAR_K_EMPTY + s), ph ^ 1);
+                    mbar_expect_tx(bar(BAR_K_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
+#pragma unroll
+                    for (int u = 0; u < PAGES_PER_TILE; ++u)
+                        if (u < np) {
+                            tma_load_4d(sK + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 0, 0, gm.g, pg[u]);
+                            tma_load_4d(sK + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 64, 0, gm.g, pg[u]);
+                        }
+                    mbar_wait(bar(BAR_V_EMPTY + s), ph ^ 1);
+                    mbar_expect_tx(bar(BAR_V_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
+#pragma unroll
+                    for (int u = 0; u < PAGES_PER_TILE; ++u)
+                        if (u < np) {
+                            tma_load_4d(sV + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 0, 0, gm.g, pg[u]);
+                            tma_load_4d(sV + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 64, 0, gm.g, pg[u]);
+                        }
+                }
             }
-            const int32_t *bt = a.block_table + int64_t(r.sid) * a.mpps;
-            for (int j = 0; j < n_kv; ++j) {
-                const int s = j & 1, ph = (j >> 1) & 1;
-                const int p0 = j * PAGES_PER_TILE;
-                const int np = min(PAGES_PER_TILE, pages_needed - p0);
-                int32_t pg[PAGES_PER_TILE];
-#pragma unroll
-                for (int u = 0; u < PAGES_PER_TILE; ++u) pg[u] = u < np ? __ldg(bt + p0 + u) : 0;
-                mbar_wait(bar(BAR_K_EMPTY + s), ph ^ 1);
-                mbar_expect_tx(bar(BAR_K_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
-#pragma unroll
-                for (int u = 0; u < PAGES_PER_TILE; ++u)
-                    if (u < np) {
-                        tma_load_4d(sK + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 0, 0, g, pg[u]);
-                        tma_load_4d(sK + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 64, 0, g, pg[u]);
-                    }
-                mbar_wait(bar(BAR_V_EMPTY + s), ph ^ 1);
-                mbar_expect_tx(bar(BAR_V_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
-#pragma unroll
-                for (int u = 0; u < PAGES_PER_TILE; ++u)
-                    if (u < np) {
-                        tma_load_4d(sV + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 0, 0, g, pg[u]);
-                        tma_load_4d(sV + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 64, 0, g, pg[u]);
-                    }
-            }
-        }
-        __syncwarp();
-        if (need_fix) {
-            // V rows that hold no session data must be exactly zero: P is 0 there, and 0 * NaN = NaN
-            const int j = n_kv - 1, s = j & 1, ph = (j >> 1) & 1;
-            mbar_wait(bar(BAR_V_FULL + s), ph);
-            const int n_zero = BN - valid_last;  // rows [valid_last, 128), 2 halves x 8 chunks of 16 B each
-            for (int e = lane; e < n_zero * 16; e += 32) {
-                const int row = valid_last + (e >> 4), hc = e & 15;
-                const uint32_t addr = sV + s * TILE_BYTES + (hc >> 3) * HALF_BYTES + row * 128 + (hc & 7) * 16;
-                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(addr), "r"(0) : "memory");
-            }
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(BAR_V_FIXED));
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
+        // The whole warp walks the loop and waits on the barriers; lane 0 issues.  (All lanes are
+        // needed once per item: V rows past the session end must be zeroed, see fix_last.)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
-        if (lane == 0) {
-            constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
-            constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
-            auto issue_qk = [&](int t, int s) {
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
+        auto issue_qk = [&](int t, int s) {
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t off = (ks >> 2) * HALF_BYTES + (ks & 3) * 32;
-                    umma_ss(tmem + t * BN, umma_desc(sQ + t * TILE_BYTES + off, 16, 1024),
-                            umma_desc(sK + s * TILE_BYTES + off, 16, 1024), idesc_qk, ks > 0);
+            for (int ks = 0; ks < D / 16; ++ks) {
+                const uint32_t off = (ks >> 2) * HALF_BYTES + (ks & 3) * 32;
+                umma_ss(tmem + t * BN, umma_desc(sQ + t * TILE_BYTES + off, 16, 1024),
+                        umma_desc(sK + s * TILE_BYTES + off, 16, 1024), idesc_qk, ks > 0);
+            }
+        };
+        auto issue_pv = [&](int t, int s, int ks0, bool acc) {  // 4 k-steps = 64 keys
+#pragma unroll
+            for (int ks = ks0; ks < ks0 + 4; ++ks)
+                umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8,
+                        umma_desc(sV + s * TILE_BYTES + ks * 2048, HALF_BYTES, 1024), idesc_pv, acc || ks > ks0);
+        };
+        // S_t of the first KV tile of a part; `single`: that tile is also the part's last, so its
+        // second QK product is the last reader of the part's Q
+        auto issue_first_qk = [&](int t, int s, bool single) {
+            if (lane == 0) {
+                issue_qk(t, s);
+                umma_commit(bar(BAR_S_FULL + t));
+                if (t == 1) {
+                    umma_commit(bar(BAR_K_EMPTY + s));
+                    if (single) umma_commit(bar(BAR_Q_EMPTY));
                 }
-            };
-            auto issue_pv = [&](int t, int s, int ks0, bool acc) {  // 4 k-steps = 64 keys
-#pragma unroll
-                for (int ks = ks0; ks < ks0 + 4; ++ks)
-                    umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8,
-                            umma_desc(sV + s * TILE_BYTES + ks * 2048, HALF_BYTES, 1024), idesc_pv, acc || ks > ks0);
-            };
-            mbar_wait(bar(BAR_Q), 0);
-            mbar_wait(bar(BAR_K_FULL + 0), 0);
-            tc_fence_after();
-            issue_qk(0, 0);
-            umma_commit(bar(BAR_S_FULL + 0));
-            issue_qk(1, 0);
-            umma_commit(bar(BAR_S_FULL + 1));
-            umma_commit(bar(BAR_K_EMPTY + 0));
-            for (int j = 0; j < n_kv; ++j) {
-                const int s = j & 1, ph = (j >> 1) & 1;
-                const bool has_next = j + 1 < n_kv;
-                const int sn = (j + 1) & 1, phn = ((j + 1) >> 1) & 1;
-                if (j == n_kv - 1 && need_fix) mbar_wait(bar(BAR_V_FIXED), 0);
-                else mbar_wait(bar(BAR_V_FULL + s), ph);
+            }
+        };
+        int kc = 0;
+        PartGeom gm = load_part<LOG2B>(a, pb);
+        mbar_wait(bar(BAR_Q_FULL), 0);
+        mbar_wait(bar(BAR_K_FULL + 0), 0);
+        tc_fence_after();
+        issue_first_qk(0, 0, gm.u1 - gm.u0 == 1);
+        issue_first_qk(1, 0, gm.u1 - gm.u0 == 1);
+        for (int p = pb; p < pe; ++p) {
+            const bool has_next_part = p + 1 < pe;
+            PartGeom gn = gm;
+            if (has_next_part) gn = load_part<LOG2B>(a, p + 1);
+            for (int j = gm.u0; j < gm.u1; ++j, ++kc) {
+                const int s = kc & 1, ph = (kc >> 1) & 1;
+                const int sn = s ^ 1, phn = ((kc + 1) >> 1) & 1;
+                const bool last = j == gm.u1 - 1;
+                mbar_wait(bar(BAR_V_FULL + s), ph);
+                if (last && gm.fix_last) {
+                    // V rows that hold no session data must be exactly zero: P is 0 there, and 0 * NaN = NaN
+                    const int n_zero = BN - gm.valid_last;  // rows [valid_last, 128), 2 halves x 8 chunks of 16 B each
+                    for (int e = lane; e < n_zero * 16; e += 32) {
+                        const int row = gm.valid_last + (e >> 4), hc = e & 15;
+                        const uint32_t addr = sV + s * TILE_BYTES + (hc >> 3) * HALF_BYTES + row * 128 + (hc & 7) * 16;
+                        asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(addr), "r"(0) : "memory");
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                }
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
+                    // the first PV product of a part overwrites O_t: the previous part's epilogue must have read it
+                    if (j == gm.u0 && p > pb) mbar_wait(bar(BAR_O_EMPTY + t), (p - pb - 1) & 1);
                     // P arrives in two halves so that the first 64 keys' PV runs under the last exponentials
-                    mbar_wait(bar(BAR_P_LO + t), j & 1);
+                    mbar_wait(bar(BAR_P_LO + t), kc & 1);
                     tc_fence_after();
-                    TC5_STAMP(4 + t, j);  // MMA thread: first half of P_t(j) seen
-                    issue_pv(t, s, 0, j > 0);
-                    mbar_wait(bar(BAR_P_HI + t), j & 1);
+                    if (lane == 0) issue_pv(t, s, 0, j > gm.u0);
+                    mbar_wait(bar(BAR_P_HI + t), kc & 1);
                     tc_fence_after();
-                    issue_pv(t, s, 4, true);
-                    if (t == 1) umma_commit(bar(BAR_V_EMPTY + s));
-                    if (has_next) {
+                    if (lane == 0) {
+                        issue_pv(t, s, 4, true);
+                        if (t == 1) umma_commit(bar(BAR_V_EMPTY + s));
+                    }
+                    if (!last) {
                         if (t == 0) {
                             mbar_wait(bar(BAR_K_FULL + sn), phn);
                             tc_fence_after();
                         }
-                        issue_qk(t, sn);
-                        umma_commit(bar(BAR_S_FULL + t));
-                        if (t == 1) umma_commit(bar(BAR_K_EMPTY + sn));
+                        issue_first_qk(t, sn, j + 1 == gm.u1 - 1);
                     } else {
-                        umma_commit(bar(BAR_O_FULL + t));
+                        if (lane == 0) umma_commit(bar(BAR_O_FULL + t));
+                        if (has_next_part) {  // keep the tensor pipe fed across the part boundary
+                            if (t == 0) {
+                                mbar_wait(bar(BAR_Q_FULL), (p + 1 - pb) & 1);
+                                mbar_wait(bar(BAR_K_FULL + sn), phn);
+                                tc_fence_after();
+                            }
+                            issue_first_qk(t, sn, gn.u1 - gn.u0 == 1);
+                        }
                     }
                 }
             }
+            gm = gn;
         }
     } else if (warp < 4) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
@@ -303,119 +355,197 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
         const int t = (warp - 4) >> 2;                 // Q tile of this warpgroup
         const int row = ((warp & 3) << 5) + lane;      // TMEM lane == row of the tile
-        const int rho = rho0 + t * BM + row;
-        const bool valid = rho < n_rows;
-        const int lim = valid ? base_lim + (rho >> a.log2G) : -1;
-        const int lim_min = base_lim + ((rho0 + t * BM) >> a.log2G);  // smallest limit among the tile's rows
         const uint32_t lane_addr = tmem + (uint32_t((warp & 3) << 5) << 16);
         const uint32_t tS = lane_addr + t * BN, tO = lane_addr + 2 * BN + t * D;
         const float sl2 = a.scale_log2;
-        float m_used = -INFINITY;
-
-        uint64_t lsum[4] = {0ull, 0ull, 0ull, 0ull};  // 4 x f32x2 independent partial row sums
         const uint64_t sl2_2 = pack_f32x2(sl2, sl2);
-        for (int j = 0; j < n_kv; ++j) {
-            mbar_wait(bar(BAR_S_FULL + t), j & 1);
+        const int G = 1 << a.log2G;
+        int kc = 0;
+        for (int p = pb; p < pe; ++p) {
+            const PartGeom gm = load_part<LOG2B>(a, p);
+            const int n_rows = gm.r.q_len * G;
+            const int rho = gm.rho0 + t * BM + row;
+            const bool valid = rho < n_rows;
+            const int lim = valid ? gm.base_lim + (rho >> a.log2G) : -1;
+            const int lim_min = gm.base_lim + ((gm.rho0 + t * BM) >> a.log2G);  // smallest limit among the tile's rows
+            float m_used = -INFINITY;
+            uint64_t lsum[4] = {0ull, 0ull, 0ull, 0ull};  // 4 x f32x2 independent partial row sums
+            for (int j = gm.u0; j < gm.u1; ++j, ++kc) {
+                mbar_wait(bar(BAR_S_FULL + t), kc & 1);
+                tc_fence_after();
+                uint32_t s0[32], s1[32], s2[32], s3[32];
+                tmem_ld32(tS, s0);
+                tmem_ld32(tS + 32, s1);
+                tmem_ld32(tS + 64, s2);
+                tmem_ld32(tS + 96, s3);
+                tmem_wait_ld();
+                const int kt = j * BN;
+                const bool masked = kt + BN - 1 > lim_min;  // uniform over the warpgroup: diagonal / last tiles only
+                if (masked) {
+                    chunk_mask(s0, kt, lim);
+                    chunk_mask(s1, kt + 32, lim);
+                    chunk_mask(s2, kt + 64, lim);
+                    chunk_mask(s3, kt + 96, lim);
+                }
+                const float mx = fmaxf(fmaxf(chunk_max(s0), chunk_max(s1)), fmaxf(chunk_max(s2), chunk_max(s3)));
+                const float m_new = fmaxf(m_used, mx);
+                const bool need = (m_new - m_used) * sl2 > kRescaleThreshold;  // true on the first live tile
+                if (__any_sync(0xffffffffu, need)) {
+                    const float f = need ? ex2_approx((m_used - m_new) * sl2) : 1.0f;
+                    if (need) {
+                        const uint64_t f2 = pack_f32x2(f, f);
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) lsum[c] = fmul2(lsum[c], f2);
+                        m_used = m_new;
+                    }
+                    if (j > gm.u0) {  // PV(t, j-1) has completed (it precedes QK(t, j) in the pipe); PV(t, j) waits for P
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t rr[32];
+                            tmem_ld32(tO + c * 32, rr);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) rr[i] = __float_as_uint(__uint_as_float(rr[i]) * f);
+                            tmem_st32(tO + c * 32, rr);
+                        }
+                    }
+                }
+                const float neg = (m_used == -INFINITY) ? 0.f : -m_used * sl2;
+                const uint64_t neg_2 = pack_f32x2(neg, neg);
+                if (masked) {
+                    chunk_exp_store<true>(s0, sl2_2, neg_2, lsum, tS);
+                    chunk_exp_store<true>(s1, sl2_2, neg_2, lsum, tS + 16);
+                    chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
+                } else {
+                    chunk_exp_store<false>(s0, sl2_2, neg_2, lsum, tS);
+                    chunk_exp_store<false>(s1, sl2_2, neg_2, lsum, tS + 16);
+                    chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
+                }
+                tmem_wait_st();  // chunks 0..2 are in TMEM (the wait costs nothing: chunk 2's math ran meanwhile)
+                tc_fence_before();
+                mbar_arrive(bar(BAR_P_LO + t));
+                if (masked) chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
+                else chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(bar(BAR_P_HI + t));
+            }
+            float l;
+            {
+                float a0, a1;
+                unpack_f32x2(fadd2(fadd2(lsum[0], lsum[1]), fadd2(lsum[2], lsum[3])), a0, a1);
+                l = a0 + a1;
+            }
+            // ---- epilogue of the part
+            mbar_wait(bar(BAR_O_FULL + t), (p - pb) & 1);
             tc_fence_after();
-            if (row == 0) TC5_STAMP(t * 2, j);  // S_t(j) seen
-            uint32_t s0[32], s1[32], s2[32], s3[32];
-            tmem_ld32(tS, s0);
-            tmem_ld32(tS + 32, s1);
-            tmem_ld32(tS + 64, s2);
-            tmem_ld32(tS + 96, s3);
-            tmem_wait_ld();
-            if (row == 0 && t == 0) TC5_STAMP(6, j);  // S row in registers
-            const int kt = j * BN;
-            const bool masked = kt + BN - 1 > lim_min;  // uniform over the warpgroup: diagonal / last tiles only
-            if (masked) {
-                chunk_mask(s0, kt, lim);
-                chunk_mask(s1, kt + 32, lim);
-                chunk_mask(s2, kt + 64, lim);
-                chunk_mask(s3, kt + 96, lim);
-            }
-            const float mx = fmaxf(fmaxf(chunk_max(s0), chunk_max(s1)), fmaxf(chunk_max(s2), chunk_max(s3)));
-            const float m_new = fmaxf(m_used, mx);
-            if (row == 0 && t == 0) TC5_STAMP(7, j);  // row max known
-            const bool need = (m_new - m_used) * sl2 > kRescaleThreshold;  // true on the first live tile
-            if (__any_sync(0xffffffffu, need)) {
-                const float f = need ? ex2_approx((m_used - m_new) * sl2) : 1.0f;
-                if (need) {
-                    const uint64_t f2 = pack_f32x2(f, f);
+            if (gm.slot < 0) {
+                // whole item: O / l -> bf16 -> out
+                const float inv = l > 0.f ? 1.0f / l : 0.f;
+                const int tok = rho >> a.log2G, hq = (gm.g << a.log2G) + (rho & (G - 1));
+                const int64_t orow = int64_t(gm.r.q_start + tok) * a.Hq + hq;
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) lsum[c] = fmul2(lsum[c], f2);
-                    m_used = m_new;
-                }
-                if (j > 0) {  // PV(t, j-1) has completed (it precedes QK(t, j) in the pipe); PV(t, j) waits for P
+                for (int c = 0; c < 4; ++c) {
+                    uint32_t rr[32];
+                    tmem_ld32(tO + c * 32, rr);
+                    tmem_wait_ld();
+                    if (c == 3) {  // O_t is in registers: the next part's PV products may overwrite it
+                        tc_fence_before();
+                        mbar_arrive(bar(BAR_O_EMPTY + t));
+                    }
+                    if (valid) {
+                        uint4 *dst = reinterpret_cast<uint4 *>(a.out + orow * D + c * 32);
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        uint32_t rr[32];
-                        tmem_ld32(tO + c * 32, rr);
-                        tmem_wait_ld();
+                        for (int i = 0; i < 4; ++i) {
+                            uint32_t w[4];
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) rr[i] = __float_as_uint(__uint_as_float(rr[i]) * f);
-                        tmem_st32(tO + c * 32, rr);
+                            for (int e = 0; e < 4; ++e) {
+                                __nv_bfloat162 pb2 = __floats2bfloat162_rn(__uint_as_float(rr[i * 8 + 2 * e]) * inv,
+                                                                           __uint_as_float(rr[i * 8 + 2 * e + 1]) * inv);
+                                w[e] = *reinterpret_cast<uint32_t *>(&pb2);
+                            }
+                            dst[i] = make_uint4(w[0], w[1], w[2], w[3]);
+                        }
                     }
                 }
-            }
-            const float neg = (m_used == -INFINITY) ? 0.f : -m_used * sl2;
-            const uint64_t neg_2 = pack_f32x2(neg, neg);
-            if (masked) {
-                chunk_exp_store<true>(s0, sl2_2, neg_2, lsum, tS);
-                chunk_exp_store<true>(s1, sl2_2, neg_2, lsum, tS + 16);
-                chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
+                if (valid && a.lse) a.lse[orow] = (m_used * sl2 + log2f(l)) * 0.6931471805599453f;
             } else {
-                chunk_exp_store<false>(s0, sl2_2, neg_2, lsum, tS);
-                chunk_exp_store<false>(s1, sl2_2, neg_2, lsum, tS + 16);
-                chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
-            }
-            tmem_wait_st();  // chunks 0..2 are in TMEM (the wait costs nothing: chunk 2's math ran meanwhile)
-            tc_fence_before();
-            mbar_arrive(bar(BAR_P_LO + t));
-            if (masked) chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
-            else chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
-            if (row == 0 && t == 0) TC5_STAMP(8, j);  // exp + P stores issued
-            tmem_wait_st();
-            tc_fence_before();
-            mbar_arrive(bar(BAR_P_HI + t));
-            if (row == 0) TC5_STAMP(t * 2 + 1, j);  // P_t(j) published
-        }
-        float l;
-        {
-            float a0, a1;
-            unpack_f32x2(fadd2(fadd2(lsum[0], lsum[1]), fadd2(lsum[2], lsum[3])), a0, a1);
-            l = a0 + a1;
-        }
-        // ---- epilogue: O / l -> bf16 -> out
-        mbar_wait(bar(BAR_O_FULL + t), 0);
-        tc_fence_after();
-        const float inv = l > 0.f ? 1.0f / l : 0.f;
-        const int tok = rho >> a.log2G, hq = (g << a.log2G) + (rho & (G - 1));
-        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+                // part of a split item: unnormalised O, running max (log2 domain) and row sum to the partial slot
+                char *slot = a.partials + size_t(gm.slot) * kTc5SlotBytes;
+                float *po = reinterpret_cast<float *>(slot) + size_t(t * BM + row) * D;
+                float2 *pml = reinterpret_cast<float2 *>(slot + size_t(2 * BM) * D * 4) + (t * BM + row);
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            uint32_t rr[32];
-            tmem_ld32(tO + c * 32, rr);
-            tmem_wait_ld();
-            if (valid) {
-                uint4 *dst = reinterpret_cast<uint4 *>(a.out + orow * D + c * 32);
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    uint32_t w[4];
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        __nv_bfloat162 pb = __floats2bfloat162_rn(__uint_as_float(rr[i * 8 + 2 * e]) * inv,
-                                                                  __uint_as_float(rr[i * 8 + 2 * e + 1]) * inv);
-                        w[e] = *reinterpret_cast<uint32_t *>(&pb);
+                for (int c = 0; c < 4; ++c) {
+                    uint32_t rr[32];
+                    tmem_ld32(tO + c * 32, rr);
+                    tmem_wait_ld();
+                    if (c == 3) {
+                        tc_fence_before();
+                        mbar_arrive(bar(BAR_O_EMPTY + t));
                     }
-                    dst[i] = make_uint4(w[0], w[1], w[2], w[3]);
+                    if (valid) {
+                        uint4 *dst = reinterpret_cast<uint4 *>(po + c * 32);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) dst[i] = make_uint4(rr[4 * i], rr[4 * i + 1], rr[4 * i + 2], rr[4 * i + 3]);
+                    }
                 }
+                if (valid) *pml = make_float2(m_used * sl2, l);
             }
         }
-        if (valid && a.lse) a.lse[orow] = (m_used * sl2 + log2f(l)) * 0.6931471805599453f;
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 2) tmem_dealloc<512>(tmem);
+#ifdef SA_TC5_PROBE
+    if (threadIdx.x == 0) {
+        g_tc5_probe[blockIdx.x][2] = clock64();
+        g_tc5_probe[blockIdx.x][3] = gtimer();
+    }
+#endif
+}
+
+// Merge of the parts of split items, in KV order (fixed, so bit-reproducible).  grid = (split
+// items, 8): each CTA takes 32 of the item's 256 rows, each warp 4 rows, lanes cover D with float4.
+__global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
+    const Tc5Merge mg = a.merges[blockIdx.x];
+    const ReqMeta r = a.reqs[mg.req];
+    const int G = 1 << a.log2G;
+    const int n_rows = r.q_len * G;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const char *slot0 = a.partials + size_t(mg.slot0) * kTc5SlotBytes;
+#pragma unroll 1
+    for (int i = 0; i < 4; ++i) {
+        const int lrow = blockIdx.y * 32 + warp * 4 + i;
+        const int rho = mg.tile * (2 * BM) + lrow;
+        if (rho >= n_rows) continue;
+        float M = -INFINITY;
+        for (int s = 0; s < mg.n_parts; ++s)
+            M = fmaxf(M, reinterpret_cast<const float2 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(2 * BM) * D * 4)[lrow].x);
+        const float Mb = (M == -INFINITY) ? 0.f : M;
+        float L = 0.f;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int s = 0; s < mg.n_parts; ++s) {
+            const char *sl = slot0 + size_t(s) * kTc5SlotBytes;
+            const float2 ml = reinterpret_cast<const float2 *>(sl + size_t(2 * BM) * D * 4)[lrow];
+            if (ml.x == -INFINITY) continue;  // the part saw no live key of this row (uniform over the warp)
+            const float w = exp2f(ml.x - Mb);
+            L += ml.y * w;
+            const float4 ov = reinterpret_cast<const float4 *>(sl + size_t(lrow) * D * 4)[lane];
+            acc.x += ov.x * w;
+            acc.y += ov.y * w;
+            acc.z += ov.z * w;
+            acc.w += ov.w * w;
+        }
+        const float inv = L > 0.f ? 1.f / L : 0.f;
+        const int tok = rho >> a.log2G, hq = (mg.g << a.log2G) + (rho & (G - 1));
+        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+        __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv), hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
+        uint2 pk;
+        pk.x = *reinterpret_cast<uint32_t *>(&lo);
+        pk.y = *reinterpret_cast<uint32_t *>(&hi);
+        *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
+        if (a.lse && lane == 0) a.lse[orow] = (M + log2f(L)) * 0.6931471805599453f;
+    }
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -441,9 +571,9 @@ constexpr size_t kSmemTc5 = size_t(2 + 2 * KV_STAGES) * TILE_BYTES + 1024;
 
 }  // namespace
 
-#ifdef SA_TC5_TRACE
-extern "C" __attribute__((visibility("default"))) int32_t sa_debug_tc5_trace(long long *out) {
-    return cudaMemcpyFromSymbol(out, g_tc5_trace, sizeof(long long) * 12 * 256) == cudaSuccess ? 0 : -4;
+#ifdef SA_TC5_PROBE
+extern "C" __attribute__((visibility("default"))) int32_t sa_debug_tc5_probe(unsigned long long *out) {
+    return cudaMemcpyFromSymbol(out, g_tc5_probe, sizeof(unsigned long long) * 256 * 4) == cudaSuccess ? 0 : -4;
 }
 #endif
 
@@ -476,10 +606,11 @@ int32_t tc5_init(sa_kv_pool *pool) {
 // the planner can be tested without a GPU.
 bool tc5_supported(const sa_kv_pool *pool) { return pool->host_only ? pool->cfg.head_dim == D : pool->tc5_ready; }
 
-cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan, int64_t total_q,
-                               const void *q, void *out, float *lse, float sm_scale, cudaStream_t stream,
-                               int32_t *launches) {
-    if (plan.pre_items == 0) return cudaSuccess;
+cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
+                               const Tc5Schedule &sched, const char *sched_dev, char *partials,
+                               int64_t total_q, const void *q, void *out, float *lse, float sm_scale,
+                               cudaStream_t stream, int32_t *launches) {
+    if (plan.n_pre == 0 || sched.parts.empty()) return cudaSuccess;
     EncodeTiledFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;
     const sa_kv_pool_config &c = pool->cfg;
@@ -493,9 +624,14 @@ cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorInvalidValue;
+    const int n_cta = int(sched.cta_begin.size()) - 1;
     Tc5Args a;
     a.reqs = reqs_dev;
-    a.n_reqs = plan.n_pre;
+    a.cta_begin = reinterpret_cast<const int32_t *>(sched_dev);
+    const size_t off_parts = (sched.cta_begin.size() * 4 + 31) / 32 * 32;
+    a.parts = reinterpret_cast<const Tc5Part *>(sched_dev + off_parts);
+    a.merges = reinterpret_cast<const Tc5Merge *>(sched_dev + off_parts + sched.parts.size() * sizeof(Tc5Part));
+    a.partials = partials;
     a.block_table = pool->block_table;
     a.mpps = pool->max_pages_per_session;
     a.out = static_cast<__nv_bfloat16 *>(out);
@@ -509,11 +645,18 @@ cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
     const CUtensorMap &tk = *reinterpret_cast<const CUtensorMap *>(pool->tmap_k);
     const CUtensorMap &tv = *reinterpret_cast<const CUtensorMap *>(pool->tmap_v);
     if (c.page_size == 64)
-        prefill_tc5_kernel<6><<<unsigned(plan.pre_items), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        prefill_tc5_kernel<6><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
     else
-        prefill_tc5_kernel<4><<<unsigned(plan.pre_items), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        prefill_tc5_kernel<4><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
     ++*launches;
-    return cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (!sched.merges.empty()) {
+        tc5_merge_kernel<<<dim3(unsigned(sched.merges.size()), 8), 256, 0, stream>>>(a);
+        ++*launches;
+        e = cudaGetLastError();
+    }
+    return e;
 }
 
 }  // namespace sa

@@ -100,9 +100,76 @@ def test_planner_classes_and_sums():
     assert st["partial_rows"] == 20 * 1 * 32 + 3 * 3 * 32    # [split][token][head]
     assert st["sum_decode_kv"] == 20480 * 1 + 3000 * 3
     assert st["sum_prefill_A"] == 2048 * 8192 + 2048 * 2049 // 2
-    tile = 256 if st["tcgen05"] else 64
-    assert st["prefill_ctas"] == 8 * (2048 * 4 // tile)
+    if st["tcgen05"]:
+        parts, sm = sa.sa_mixed_attention_schedule(p, sids, [0, 1, 4, 4 + 2048, 4 + 2048])
+        assert st["prefill_ctas"] == sm["parts"] == len(parts) >= 8 * (2048 * 4 // 256)
+    else:
+        assert st["prefill_ctas"] == 8 * (2048 * 4 // 64)
     # a request cannot have more query rows than cached tokens (append first, then attend)
     with pytest.raises(sa.SAError):
         sa.sa_mixed_attention_plan(p, [sids[3]], [0, 6])
     assert sa.sa_mixed_attention_workspace_bytes(p, sids, [0, 1, 4, 4 + 2048, 4 + 2048]) >= st["partial_rows"] * (128 + 1) * 4
+
+
+def _check_schedule(p, sids, lens_prefix, lens_new, G=4, Hkv=8):
+    """Every item (request, kv head, 256-row tile) is covered exactly once, in KV order, by its parts."""
+    indptr = np.concatenate([[0], np.cumsum(lens_new)]).astype(np.int32)
+    parts, sm = sa.sa_mixed_attention_schedule(p, sids, indptr)
+    assert sm["parts"] == len(parts) and sm["ctas"] >= 1
+    # parts are grouped by CTA in execution order
+    assert (np.diff(parts[:, 0]) >= 0).all()
+    items = {}
+    for cta, r, g, tile, u0, u1, n_kv, slot in parts.tolist():
+        assert 0 <= u0 < u1 <= n_kv
+        items.setdefault((r, g, tile), []).append((u0, u1, n_kv, slot, cta))
+    n_items, total, n_split, slots = 0, 0, 0, []
+    for r, (P, n) in enumerate(zip(lens_prefix, lens_new)):
+        if n * G <= 16:
+            continue
+        for g in range(Hkv):
+            for tile in range((n * G + 255) // 256):
+                tok_max = min(n - 1, (tile * 256 + 255) // G)
+                n_kv = (P + tok_max + 1 + 127) // 128           # keys 0 .. prefix + tok_max (PAPER.md L311)
+                ps = sorted(items.pop((r, g, tile)))
+                assert ps[0][0] == 0 and ps[-1][1] == n_kv and all(a[1] == b[0] for a, b in zip(ps, ps[1:]))
+                assert all(x[2] == n_kv for x in ps)
+                if len(ps) == 1:
+                    assert ps[0][3] == -1
+                else:
+                    assert [x[3] for x in ps] == list(range(ps[0][3], ps[0][3] + len(ps)))   # consecutive slots, KV order
+                    assert len(set(x[4] for x in ps)) == len(ps)                          # on different CTAs
+                    n_split += 1
+                    slots += [x[3] for x in ps]
+                n_items += 1
+                total += n_kv
+    assert not items, "schedule has parts of items that do not exist"
+    assert sorted(slots) == list(range(sm["slots"])) and n_split == sm["split_items"] and total == sm["total_units"]
+    load = np.zeros(sm["ctas"], dtype=np.int64)
+    for cta, r, g, tile, u0, u1, n_kv, slot in parts.tolist():
+        load[cta] += u1 - u0 + 3
+    assert load.max() == sm["makespan"]
+    return parts, sm, n_items, load
+
+
+def test_tc5_schedule_covers_items_and_balances():
+    p = _pool(num_pages=20000, page_size=64, max_sessions=24, max_tokens=65536, Hq=32, Hkv=8, D=128)
+    cases = [
+        ([24576], [2048]),                       # config 2's chunk: 256 equal items on 148 CTAs
+        ([20480], [512]),                        # a small lookahead chunk: 64 items, fewer than the SMs
+        ([0], [100]),                            # one short request without a prefix
+        ([8192, 16384, 24576, 32768, 20000, 77], [2048, 2048, 2048, 2048, 1, 3]),   # config 4 shaped, with decode rows
+        (list(range(1000, 17000, 1000)), [512 + 211 * i for i in range(16)]),       # ragged like config 3
+        ([5, 130, 0, 17], [7, 40, 300, 5]),      # tiny ragged requests
+    ]
+    for prefix, new in cases:
+        sids = [sa.sa_kv_session_open(p) for _ in prefix]
+        sa.sa_rope_kv_append(p, sids, np.concatenate([[0], np.cumsum([a + b for a, b in zip(prefix, new)])]), None, None)
+        parts, sm, n_items, load = _check_schedule(p, sids, prefix, new)
+        ideal = (sm["total_units"] + 3 * n_items) / sm["ctas"]
+        # balanced: the makespan is within a few tiles (fixed costs of the extra parts, minimum part) of the ideal
+        assert sm["makespan"] <= ideal + 3 * 2 + 4 + 1, (prefix, new, sm, ideal)
+        if n_items >= 64 and sm["total_units"] >= 16 * sm["ctas"]:
+            assert (load > 0).sum() == sm["ctas"], "a balanced schedule of a large batch uses every CTA"
+            assert sm["slots"] <= 2 * sm["ctas"] + n_items // 4
+        for sid in sids:
+            sa.sa_kv_session_close(p, sid)
