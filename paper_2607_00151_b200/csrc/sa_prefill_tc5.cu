@@ -505,7 +505,8 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
 }
 
 // Merge of the parts of split items, in KV order (fixed, so bit-reproducible).  grid = (split
-// items, 8): each CTA takes 32 of the item's 256 rows, each warp 4 rows, lanes cover D with float4.
+// items, 32): each CTA takes 8 of the item's 256 rows, one row per warp, lanes cover D with float4;
+// the loads of up to four parts are issued together (the kernel is latency-bound otherwise).
 __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
     const Tc5Merge mg = a.merges[blockIdx.x];
     const ReqMeta r = a.reqs[mg.req];
@@ -513,39 +514,45 @@ __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
     const int n_rows = r.q_len * G;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const char *slot0 = a.partials + size_t(mg.slot0) * kTc5SlotBytes;
-#pragma unroll 1
-    for (int i = 0; i < 4; ++i) {
-        const int lrow = blockIdx.y * 32 + warp * 4 + i;
-        const int rho = mg.tile * (2 * BM) + lrow;
-        if (rho >= n_rows) continue;
-        float M = -INFINITY;
-        for (int s = 0; s < mg.n_parts; ++s)
-            M = fmaxf(M, reinterpret_cast<const float2 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(2 * BM) * D * 4)[lrow].x);
-        const float Mb = (M == -INFINITY) ? 0.f : M;
-        float L = 0.f;
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int s = 0; s < mg.n_parts; ++s) {
-            const char *sl = slot0 + size_t(s) * kTc5SlotBytes;
-            const float2 ml = reinterpret_cast<const float2 *>(sl + size_t(2 * BM) * D * 4)[lrow];
-            if (ml.x == -INFINITY) continue;  // the part saw no live key of this row (uniform over the warp)
-            const float w = exp2f(ml.x - Mb);
-            L += ml.y * w;
-            const float4 ov = reinterpret_cast<const float4 *>(sl + size_t(lrow) * D * 4)[lane];
-            acc.x += ov.x * w;
-            acc.y += ov.y * w;
-            acc.z += ov.z * w;
-            acc.w += ov.w * w;
-        }
-        const float inv = L > 0.f ? 1.f / L : 0.f;
-        const int tok = rho >> a.log2G, hq = (mg.g << a.log2G) + (rho & (G - 1));
-        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
-        __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv), hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
-        uint2 pk;
-        pk.x = *reinterpret_cast<uint32_t *>(&lo);
-        pk.y = *reinterpret_cast<uint32_t *>(&hi);
-        *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
-        if (a.lse && lane == 0) a.lse[orow] = (M + log2f(L)) * 0.6931471805599453f;
+    const int lrow = blockIdx.y * 8 + warp;
+    const int rho = mg.tile * (2 * BM) + lrow;
+    if (rho >= n_rows) return;
+    auto ml_of = [&](int s) { return reinterpret_cast<const float2 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(2 * BM) * D * 4)[lrow]; };
+    auto o_of = [&](int s) { return reinterpret_cast<const float4 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(lrow) * D * 4)[lane]; };
+    float M = -INFINITY;
+    for (int s = 0; s < mg.n_parts; ++s) M = fmaxf(M, ml_of(s).x);
+    const float Mb = (M == -INFINITY) ? 0.f : M;
+    float L = 0.f;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s0 = 0; s0 < mg.n_parts; s0 += 4) {
+        float2 ml[4];
+        float4 ov[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (s0 + u < mg.n_parts) {
+                ml[u] = ml_of(s0 + u);
+                ov[u] = o_of(s0 + u);
+            }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)  // KV order
+            if (s0 + u < mg.n_parts && ml[u].x != -INFINITY) {  // -inf: the part saw no live key of this row
+                const float w = exp2f(ml[u].x - Mb);
+                L += ml[u].y * w;
+                acc.x += ov[u].x * w;
+                acc.y += ov[u].y * w;
+                acc.z += ov[u].z * w;
+                acc.w += ov[u].w * w;
+            }
     }
+    const float inv = L > 0.f ? 1.f / L : 0.f;
+    const int tok = rho >> a.log2G, hq = (mg.g << a.log2G) + (rho & (G - 1));
+    const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+    __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv), hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
+    uint2 pk;
+    pk.x = *reinterpret_cast<uint32_t *>(&lo);
+    pk.y = *reinterpret_cast<uint32_t *>(&hi);
+    *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
+    if (a.lse && lane == 0) a.lse[orow] = (M + log2f(L)) * 0.6931471805599453f;
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -652,7 +659,7 @@ cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (!sched.merges.empty()) {
-        tc5_merge_kernel<<<dim3(unsigned(sched.merges.size()), 8), 256, 0, stream>>>(a);
+        tc5_merge_kernel<<<dim3(unsigned(sched.merges.size()), 32), 256, 0, stream>>>(a);
         ++*launches;
         e = cudaGetLastError();
     }
