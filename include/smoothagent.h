@@ -113,6 +113,25 @@ SA_API int32_t sa_kv_session_truncate(sa_kv_pool *pool, int32_t sid, int64_t new
 SA_API int32_t sa_kv_session_query(const sa_kv_pool *pool, int32_t sid, int64_t *len, int32_t *pages,
                             int32_t *n_pages);
 
+/* ---- session operations of the commit splice ------------------------------
+ * A lookahead request rebuilds the transformed context's KV ahead of time in a session of its own
+ * and, at the commit point, "directly replaces the prefix in the working context" (L47, L170,
+ * L186-187); sub-agent contexts are built chunk by chunk while the main agent decodes (L265-281).
+ *
+ * sa_kv_session_fork: open a new session whose first prefix_len tokens are those of src_sid (the
+ * retained prefix).  Whole pages of the prefix are SHARED (reference-counted, never written
+ * again); if the prefix ends inside a page, that page is copied into a fresh page now (enqueued
+ * on `stream`), so the two sessions append independently.  Needs at most one free page.
+ * sa_rope_kv_append also copies on write: appending into a partly filled last page that another
+ * session still holds first moves the appender to a private copy of that page.
+ * sa_kv_session_commit: main_sid takes over the lookahead session's pages and length (its device
+ * block-table row is rewritten on `stream`), the pages it held before lose a holder, and
+ * lookahead_sid is closed.  A page returns to the free list when its last holder lets go. */
+SA_API int32_t sa_kv_session_fork(sa_kv_pool *pool, int32_t src_sid, int64_t prefix_len, int32_t *out_sid,
+                           void *stream);
+SA_API int32_t sa_kv_session_commit(sa_kv_pool *pool, int32_t main_sid, int32_t lookahead_sid, void *stream);
+SA_API int32_t sa_kv_page_refcount(const sa_kv_pool *pool, int32_t page, int32_t *out_refs);
+
 /* ---- sa_rope_kv_append: fused RoPE + scatter of new K/V into pages (step a2) -------------
  * Request r appends q_r = qo_indptr[r+1]-qo_indptr[r] tokens to session sids[r]; token i of
  * request r sits at absolute position session_len(r) + i IN THE TRANSFORMED CONTEXT (the

@@ -71,6 +71,9 @@ PROTOTYPES = {
     "sa_kv_session_close": (ctypes.c_int32, [_vp, ctypes.c_int32]),
     "sa_kv_session_truncate": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64]),
     "sa_kv_session_query": (ctypes.c_int32, [_vp, ctypes.c_int32, _i64p, _i32p, _i32p]),
+    "sa_kv_session_fork": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, _i32p, _vp]),
+    "sa_kv_session_commit": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int32, _vp]),
+    "sa_kv_page_refcount": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p]),
     "sa_rope_kv_append": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _vp, _vp, _vp, _vp]),
     "sa_mixed_attention_workspace_bytes": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_mixed_attention": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _vp, _vp, _vp, ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
@@ -228,6 +231,24 @@ def sa_kv_session_close(pool: Pool, sid: int) -> None:
 
 def sa_kv_session_truncate(pool: Pool, sid: int, new_len: int) -> None:
     _check(load_library().sa_kv_session_truncate(pool.handle, sid, new_len), "sa_kv_session_truncate")
+
+
+def sa_kv_session_fork(pool: Pool, src_sid: int, prefix_len: int, stream=None) -> int:
+    out = ctypes.c_int32(-1)
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_kv_session_fork(pool.handle, src_sid, prefix_len, ctypes.byref(out), sp), "sa_kv_session_fork")
+    return int(out.value)
+
+
+def sa_kv_session_commit(pool: Pool, main_sid: int, lookahead_sid: int, stream=None) -> None:
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_kv_session_commit(pool.handle, main_sid, lookahead_sid, sp), "sa_kv_session_commit")
+
+
+def sa_kv_page_refcount(pool: Pool, page: int) -> int:
+    out = ctypes.c_int32(0)
+    _check(load_library().sa_kv_page_refcount(pool.handle, page, ctypes.byref(out)), "sa_kv_page_refcount")
+    return int(out.value)
 
 
 def sa_kv_session_query(pool: Pool, sid: int):

@@ -4,6 +4,7 @@
 #include <cuda_bf16.h>
 
 #include <algorithm>
+#include <utility>
 #include <vector>
 
 #include "sa_internal.h"
@@ -197,6 +198,8 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
         const Session &s = pool->sessions[size_t(sid)];
         if (s.len + n > pool->cfg.max_session_tokens) return SA_ERR_INVALID_ARG;
         need_pages += (s.len + n + B - 1) / B - int64_t(s.pages.size());
+        // copy-on-write: appending into a partly filled last page that another session also holds
+        if (n > 0 && s.len % B != 0 && pool->page_ref[size_t(s.pages.back())] > 1) ++need_pages;
     }
     const int64_t total = qo_indptr[n_req];
     if (need_pages > int64_t(pool->free_pages.size())) return SA_ERR_OUT_OF_PAGES;
@@ -222,6 +225,7 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
     }
     // ---- allocate pages (cannot fail any more) and build the metadata
     int32_t n_list = 0, n_gain = 0;
+    std::vector<std::pair<int32_t, int32_t>> cow;  // (private copy, shared page) of this call
     std::vector<ReqMeta> gain;  // requests that gained pages, for the block-table update
     for (int r = 0; r < n_req; ++r) {
         Session &s = pool->sessions[size_t(sids[r])];
@@ -234,9 +238,18 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
         m.kv_len = int32_t(s.len);  // position of the request's first new token
         m.item_begin = n_list;
         m.part_begin = int32_t(s.pages.size());
+        if (n > 0 && s.len % B != 0 && pool->page_ref[size_t(s.pages.back())] > 1) {
+            // the shared page keeps its bits for its other holders; this session continues in a private copy
+            const int32_t shared = s.pages.back();
+            const int32_t p = take_page(pool);
+            if (!pool->host_only) cow.push_back(std::make_pair(p, shared));
+            release_page(pool, shared);
+            s.pages.back() = p;
+            m.part_begin = int32_t(s.pages.size()) - 1;  // the block-table update rewrites this entry too
+            page_list[n_list++] = p;
+        }
         while (int64_t(s.pages.size()) < want) {
-            const int32_t p = pool->free_pages.back();
-            pool->free_pages.pop_back();
+            const int32_t p = take_page(pool);
             s.pages.push_back(p);
             page_list[n_list++] = p;
         }
@@ -252,6 +265,8 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
     if (pool->host_only) return SA_OK;
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    for (const auto &c : cow)
+        if (copy_page_async(pool, c.first, c.second, stream) != cudaSuccess) return SA_ERR_CUDA;
     // slab layout: [ReqMeta x n_req][new page ids x n_list][ReqMeta x n_gain]
     size_t off_gain = sizeof(ReqMeta) * size_t(n_req) + sizeof(int32_t) * size_t(n_list);
     off_gain = (off_gain + 15) / 16 * 16;

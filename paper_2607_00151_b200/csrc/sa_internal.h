@@ -100,6 +100,7 @@ struct sa_kv_pool {
     cudaEvent_t big_event = nullptr;
     bool big_event_used = false;
     std::vector<int32_t> free_pages;  // stack: back() is handed out next
+    std::vector<int32_t> page_ref;    // sessions holding each page (forked sessions share the retained prefix's pages)
     std::vector<sa::Session> sessions;
     int32_t last_launches = 0;
     int32_t num_sms = 148;
@@ -116,6 +117,13 @@ namespace sa {
 // copy if it is still in flight.  commit_meta enqueues the H2D copy of `bytes` bytes.
 int32_t acquire_meta(sa_kv_pool *pool, char **host, char **dev);
 int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream);
+// Same slab, but the bytes go to `dev_dst` (a block-table row) instead of the slab's device twin.
+int32_t commit_meta_to(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream);
+// Page bookkeeping: a page returns to the free list when its last holder lets go of it.
+int32_t take_page(sa_kv_pool *pool);
+void release_page(sa_kv_pool *pool, int32_t page);
+// Device copy of one whole page (K and V, all heads) on `stream`: copy-on-write of a shared partial page.
+cudaError_t copy_page_async(const sa_kv_pool *pool, int32_t dst_page, int32_t src_page, cudaStream_t stream);
 // Metadata that does not fit a slab: one growable pinned buffer (waits for its previous copy),
 // copied to a device address of the caller's workspace.
 int32_t acquire_big_meta(sa_kv_pool *pool, size_t bytes, char **host);

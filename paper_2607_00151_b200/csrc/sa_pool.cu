@@ -106,6 +106,7 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
     pool->meta_slab_bytes = cv.slab;
     pool->sessions.resize(size_t(cfg->max_sessions));
     pool->free_pages.resize(size_t(cfg->num_pages));
+    pool->page_ref.assign(size_t(cfg->num_pages), 0);
     for (int64_t i = 0; i < cfg->num_pages; ++i)  // stack: first of the order is popped first
         pool->free_pages[size_t(cfg->num_pages - 1 - i)] = free_page_order ? free_page_order[i] : int32_t(i);
     pool->host_only = (dev_storage == nullptr);
@@ -210,10 +211,79 @@ extern "C" int32_t sa_kv_session_truncate(sa_kv_pool *pool, int32_t sid, int64_t
     if (!s || new_len < 0 || new_len > s->len) return SA_ERR_INVALID_ARG;
     size_t keep = size_t((new_len + pool->cfg.page_size - 1) / pool->cfg.page_size);
     while (s->pages.size() > keep) {
-        pool->free_pages.push_back(s->pages.back());
+        sa::release_page(pool, s->pages.back());
         s->pages.pop_back();
     }
     s->len = new_len;
+    return SA_OK;
+}
+
+// ---- session operations of the commit splice ----
+// Upload the session's page list into its row of the device block table.
+static int32_t upload_row(sa_kv_pool *pool, int32_t sid, cudaStream_t stream) {
+    const sa::Session &s = pool->sessions[size_t(sid)];
+    if (pool->host_only || s.pages.empty()) return SA_OK;
+    char *mh = nullptr, *md = nullptr;
+    int32_t st = sa::acquire_meta(pool, &mh, &md);
+    if (st != SA_OK) return st;
+    const size_t bytes = s.pages.size() * sizeof(int32_t);
+    memcpy(mh, s.pages.data(), bytes);  // the slab holds 4 bytes per pool page: always fits
+    return sa::commit_meta_to(pool, pool->block_table + int64_t(sid) * pool->max_pages_per_session, bytes, stream);
+}
+
+extern "C" int32_t sa_kv_session_fork(sa_kv_pool *pool, int32_t src_sid, int64_t prefix_len, int32_t *out_sid, void *stream_) {
+    sa::Session *src = get_session(pool, src_sid);
+    if (!src || !out_sid || prefix_len < 0 || prefix_len > src->len) return SA_ERR_INVALID_ARG;
+    const int B = pool->cfg.page_size;
+    const size_t full = size_t(prefix_len / B);
+    const bool partial = prefix_len % B != 0;
+    if (partial && pool->free_pages.empty()) return SA_ERR_OUT_OF_PAGES;
+    int32_t sid = -1;
+    int32_t st = sa_kv_session_open(pool, &sid);
+    if (st != SA_OK) return st;
+    src = get_session(pool, src_sid);
+    sa::Session &dst = pool->sessions[size_t(sid)];
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    for (size_t i = 0; i < full; ++i) {  // whole pages of the retained prefix are shared, never written again
+        dst.pages.push_back(src->pages[i]);
+        ++pool->page_ref[size_t(src->pages[i])];
+    }
+    if (partial) {  // the page the prefix ends in will be appended to by the fork: it gets its own copy now
+        const int32_t p = sa::take_page(pool);
+        dst.pages.push_back(p);
+        if (!pool->host_only && sa::copy_page_async(pool, p, src->pages[full], stream) != cudaSuccess) {
+            sa_kv_session_close(pool, sid);
+            return SA_ERR_CUDA;
+        }
+    }
+    dst.len = prefix_len;
+    st = upload_row(pool, sid, stream);
+    if (st != SA_OK) {
+        sa_kv_session_close(pool, sid);
+        return st;
+    }
+    *out_sid = sid;
+    return SA_OK;
+}
+
+extern "C" int32_t sa_kv_session_commit(sa_kv_pool *pool, int32_t main_sid, int32_t lookahead_sid, void *stream_) {
+    sa::Session *m = get_session(pool, main_sid);
+    sa::Session *la = get_session(pool, lookahead_sid);
+    if (!m || !la || main_sid == lookahead_sid) return SA_ERR_INVALID_ARG;
+    // the main session takes over the lookahead's block table; the superseded pages lose a holder
+    std::vector<int32_t> old;
+    old.swap(m->pages);
+    m->pages.swap(la->pages);
+    m->len = la->len;
+    la->len = 0;
+    la->open = false;
+    for (int32_t p : old) sa::release_page(pool, p);
+    return upload_row(pool, main_sid, static_cast<cudaStream_t>(stream_));
+}
+
+extern "C" int32_t sa_kv_page_refcount(const sa_kv_pool *pool, int32_t page, int32_t *out_refs) {
+    if (!pool || !out_refs || page < 0 || page >= pool->cfg.num_pages) return SA_ERR_INVALID_ARG;
+    *out_refs = pool->page_ref[size_t(page)];
     return SA_OK;
 }
 
@@ -259,10 +329,36 @@ int32_t acquire_meta(sa_kv_pool *pool, char **host, char **dev) {
     return SA_OK;
 }
 
+int32_t take_page(sa_kv_pool *pool) {
+    const int32_t p = pool->free_pages.back();
+    pool->free_pages.pop_back();
+    pool->page_ref[size_t(p)] = 1;
+    return p;
+}
+
+void release_page(sa_kv_pool *pool, int32_t page) {
+    if (--pool->page_ref[size_t(page)] == 0) pool->free_pages.push_back(page);
+}
+
+cudaError_t copy_page_async(const sa_kv_pool *pool, int32_t dst_page, int32_t src_page, cudaStream_t stream) {
+    const size_t bytes = size_t(pool->stride_page) * 2;
+    const char *kb = static_cast<const char *>(pool->k_base), *vb = static_cast<const char *>(pool->v_base);
+    cudaError_t e = cudaMemcpyAsync(const_cast<char *>(kb) + size_t(dst_page) * bytes, kb + size_t(src_page) * bytes, bytes,
+                                    cudaMemcpyDeviceToDevice, stream);
+    if (e != cudaSuccess) return e;
+    return cudaMemcpyAsync(const_cast<char *>(vb) + size_t(dst_page) * bytes, vb + size_t(src_page) * bytes, bytes,
+                           cudaMemcpyDeviceToDevice, stream);
+}
+
 int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream) {
     int i = pool->meta_next;
-    char *host = pool->meta_host + size_t(i) * pool->meta_slab_bytes;
     char *dev = pool->meta_dev + size_t(i) * pool->meta_slab_bytes;
+    return commit_meta_to(pool, dev, bytes, stream);
+}
+
+int32_t commit_meta_to(sa_kv_pool *pool, void *dev, size_t bytes, cudaStream_t stream) {
+    int i = pool->meta_next;
+    char *host = pool->meta_host + size_t(i) * pool->meta_slab_bytes;
     if (cudaMemcpyAsync(dev, host, bytes, cudaMemcpyHostToDevice, stream) != cudaSuccess) return SA_ERR_CUDA;
     if (cudaEventRecord(pool->meta_event[i], stream) != cudaSuccess) return SA_ERR_CUDA;
     pool->meta_event_used[i] = true;

@@ -173,3 +173,89 @@ def test_tc5_schedule_covers_items_and_balances():
             assert sm["slots"] <= 2 * sm["ctas"] + n_items // 4
         for sid in sids:
             sa.sa_kv_session_close(p, sid)
+
+
+# ---- session operations of the commit splice -------------
+def test_fork_shares_whole_pages_and_copies_the_partial_one():
+    p = _pool(num_pages=32, page_size=16, max_sessions=4)
+    src = sa.sa_kv_session_open(p)
+    sa.sa_rope_kv_append(p, [src], [0, 100], None, None)          # 7 pages: 6 full + 4 tokens
+    _, pg = sa.sa_kv_session_query(p, src)
+    # fork at a page boundary: shares pages, takes none
+    f0 = sa.sa_kv_session_fork(p, src, 64)
+    assert sa.sa_kv_session_query(p, f0) == (64, pg[:4]) and sa.sa_kv_pool_free_pages(p) == 25
+    assert [sa.sa_kv_page_refcount(p, x) for x in pg] == [2, 2, 2, 2, 1, 1, 1]
+    # fork inside a page: shares the whole pages below, owns a copy of the page the prefix ends in
+    f1 = sa.sa_kv_session_fork(p, src, 70)
+    l1, pg1 = sa.sa_kv_session_query(p, f1)
+    assert l1 == 70 and pg1[:4] == pg[:4] and pg1[4] not in pg and len(pg1) == 5
+    assert sa.sa_kv_pool_free_pages(p) == 24
+    assert [sa.sa_kv_page_refcount(p, x) for x in pg[:5]] == [3, 3, 3, 3, 1] and sa.sa_kv_page_refcount(p, pg1[4]) == 1
+    # the fork appends on its own pages; the source is untouched
+    sa.sa_rope_kv_append(p, [f1], [0, 30], None, None)
+    assert sa.sa_kv_session_query(p, src) == (100, pg)
+    l1, pg1b = sa.sa_kv_session_query(p, f1)
+    assert l1 == 100 and pg1b[:5] == pg1 and not set(pg1b[4:]) & set(pg)
+    # closing a holder only frees pages nobody else holds
+    sa.sa_kv_session_close(p, src)
+    assert [sa.sa_kv_page_refcount(p, x) for x in pg] == [2, 2, 2, 2, 0, 0, 0]
+    sa.sa_kv_session_close(p, f0)
+    sa.sa_kv_session_close(p, f1)
+    assert sa.sa_kv_pool_free_pages(p) == 32 and all(sa.sa_kv_page_refcount(p, x) == 0 for x in range(32))
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_fork(p, src, 0)                            # closed source
+
+
+def test_append_copies_a_shared_partial_page_on_write():
+    p = _pool(num_pages=16, page_size=16, max_sessions=4)
+    src = sa.sa_kv_session_open(p)
+    sa.sa_rope_kv_append(p, [src], [0, 64], None, None)           # 4 full pages
+    f = sa.sa_kv_session_fork(p, src, 64)
+    _, pg = sa.sa_kv_session_query(p, src)
+    # truncating the source into a shared page and appending again must not write that page
+    sa.sa_kv_session_truncate(p, src, 40)                          # keeps pages 0..2, page 2 is now partly valid
+    assert [sa.sa_kv_page_refcount(p, x) for x in pg] == [2, 2, 2, 1]
+    free0 = sa.sa_kv_pool_free_pages(p)
+    sa.sa_rope_kv_append(p, [src], [0, 4], None, None)
+    l, pg2 = sa.sa_kv_session_query(p, src)
+    assert l == 44 and pg2[:2] == pg[:2] and pg2[2] != pg[2] and len(pg2) == 3
+    assert sa.sa_kv_page_refcount(p, pg[2]) == 1 and sa.sa_kv_page_refcount(p, pg2[2]) == 1
+    assert sa.sa_kv_pool_free_pages(p) == free0 - 1
+    assert sa.sa_kv_session_query(p, f) == (64, pg)               # the fork still sees the old pages
+    # a second append into the now private page takes nothing
+    sa.sa_rope_kv_append(p, [src], [0, 2], None, None)
+    assert sa.sa_kv_session_query(p, src)[1] == pg2 and sa.sa_kv_pool_free_pages(p) == free0 - 1
+    # out of pages: a copy-on-write needs a page like any other growth, and a failed call changes nothing
+    q = _pool(num_pages=4, page_size=16, max_sessions=4)
+    a = sa.sa_kv_session_open(q)
+    sa.sa_rope_kv_append(q, [a], [0, 64], None, None)
+    b = sa.sa_kv_session_fork(q, a, 64)
+    sa.sa_kv_session_truncate(q, a, 50)
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_rope_kv_append(q, [a], [0, 1], None, None)
+    assert e.value.status == sa.SA_ERR_OUT_OF_PAGES and sa.sa_kv_session_query(q, a)[0] == 50
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_kv_session_fork(q, a, 50)                            # would need a page for the partial copy
+    assert e.value.status == sa.SA_ERR_OUT_OF_PAGES
+
+
+def test_commit_swaps_block_tables_and_releases_superseded_pages():
+    p = _pool(num_pages=32, page_size=16, max_sessions=4)
+    main = sa.sa_kv_session_open(p)
+    sa.sa_rope_kv_append(p, [main], [0, 200], None, None)         # 13 pages
+    _, pg_main = sa.sa_kv_session_query(p, main)
+    # lookahead: keep 3 pages' worth of prefix, rebuild a shorter (transformed) context behind it
+    la = sa.sa_kv_session_fork(p, main, 48)
+    sa.sa_rope_kv_append(p, [la], [0, 40], None, None)
+    l_la, pg_la = sa.sa_kv_session_query(p, la)
+    assert l_la == 88 and pg_la[:3] == pg_main[:3]
+    sa.sa_kv_session_commit(p, main, la)
+    assert sa.sa_kv_session_query(p, main) == (88, pg_la)
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_query(p, la)                              # the lookahead session is gone
+    # the 10 superseded pages are free again, the shared prefix pages have one holder
+    assert sa.sa_kv_pool_free_pages(p) == 32 - len(pg_la)
+    assert [sa.sa_kv_page_refcount(p, x) for x in pg_la] == [1] * len(pg_la)
+    assert all(sa.sa_kv_page_refcount(p, x) == 0 for x in pg_main[3:])
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_commit(p, main, main)
