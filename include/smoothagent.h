@@ -214,6 +214,79 @@ SA_API int32_t sa_latency_table(sa_kv_pool *pool, const int32_t *prefill_tokens,
                          int32_t warmup, int32_t iters, float *out_ms, int64_t *out_sum_kv,
                          void *stream);
 
+/* ---- lookahead-aware scheduler core (section 4) --------------
+ * Host-only calls (no device work, no pool): the consumer of sa_latency_table.
+ *
+ * Latency model (Eq. 1):
+ *     EstBatchLatency(B) = c0 + T_GEMM(M) + alpha_d * sum_{j in decode} L_j + alpha_p * sum_{j in prefill} A_j
+ * M = |B_decode| + sum_j q_j (L301); L_j = cache length of decode request j (L305); A_j = q_j*prefix_j +
+ * q_j(q_j+1)/2 (L313).  c0 is a fixed cost per call that the paper's equation does not have (0
+ * reproduces it).  T_GEMM(M): the offline-profiled lookup table with interpolation of L299-303,
+ * piecewise linear through (gemm_m[i], gemm_ms[i]), constant below the first point, the last
+ * segment's slope beyond the last; n_gemm = 0 gives T_GEMM = 0 (this path has no GEMMs).  An empty
+ * batch costs 0.  Estimates are computed in double, the three integer sums exactly. */
+#define SA_GEMM_TABLE_MAX 64
+typedef struct {
+    double c0_ms;
+    double alpha_d_ms;                  /* ms per cached token read by decode rows */
+    double alpha_p_ms;                  /* ms per causal (query, key) pair of prefill chunks */
+    int32_t n_gemm;
+    int32_t reserved;
+    double gemm_m[SA_GEMM_TABLE_MAX];   /* strictly increasing */
+    double gemm_ms[SA_GEMM_TABLE_MAX];
+} sa_latency_model;
+
+typedef struct {
+    int64_t q;      /* query tokens of the chunk (q_j) */
+    int64_t prefix; /* cached tokens before them (prefix_j) */
+} sa_chunk;
+
+typedef struct {
+    double t_arrival_ms;
+    double slo_ttft_ms;
+    int64_t q;      /* prefill tokens the request still needs */
+    int64_t prefix; /* tokens of it already cached */
+} sa_lc_request;
+
+/* Least-squares fit of ms[i] ~ c0 + alpha_d*sum_kv[i][0] + alpha_p*sum_kv[i][1] over n profiled batches:
+ * exactly the out_ms / out_sum_kv arrays of sa_latency_table ("profiled coefficient", L309, L319).
+ * with_intercept == 0 fits Eq. 1 literally (c0 = 0).  A column that is zero in every batch keeps a zero
+ * coefficient.  out_max_rel_err (nullable): max_i |fit_i - ms_i| / ms_i.  out->n_gemm is set to 0. */
+SA_API int32_t sa_latency_fit(const float *ms, const int64_t *sum_kv, int32_t n, int32_t with_intercept,
+                       sa_latency_model *out, double *out_max_rel_err);
+
+SA_API int32_t sa_est_batch_latency(const sa_latency_model *model, const int64_t *decode_L, int32_t n_dec,
+                             const sa_chunk *chunks, int32_t n_pre, double *out_ms);
+
+/* Algorithm 2 (PD co-located, L363-388): admit decode requests, then LC prefill chunks, then BE
+ * (lookahead) chunks, each queue in order, each candidate only while EstBatchLatency(B + {c}) <=
+ * delta_ms; the first candidate of a queue that does not fit ends that queue.
+ * out_admitted (host int32[3]) = admitted {decode, LC chunks, BE chunks}: always a prefix of each queue.
+ * out_est_ms (nullable): the estimate of the admitted batch. */
+SA_API int32_t sa_schedule_hybrid(const sa_latency_model *model, const int64_t *decode_L, int32_t n_dec,
+                           const sa_chunk *lc, int32_t n_lc, const sa_chunk *be, int32_t n_be,
+                           double delta_ms, int32_t *out_admitted, double *out_est_ms);
+
+/* Algorithm 1 (PD disaggregated, L321-347): lc_queue is the LC queue in the order of the LC policy;
+ * p accumulates EstPrefillLatency(r) (= Eq. 1 of r's remaining prefill alone), the slack of request j is
+ * (t_arrival + SLO_TTFT) - t_now - p, t_budget = max(0, min_j slack) (+inf with an empty queue).
+ * lc_chunks = NextChunks(Q_LC) is always in the batch; BE chunks are admitted in order while
+ * EstBatchLatency(B_LC + B_BE + {c}) <= t_budget, and the first one that does not fit ends the scan
+ * (the listing's lines 15-17 are garbled in PAPER.md; this is Algorithm 2's rule and keeps the
+ * lookahead queue in order, L168). */
+SA_API int32_t sa_schedule_prefill_slack(const sa_latency_model *model, const sa_lc_request *lc_queue, int32_t n_queue,
+                                  double t_now_ms, const sa_chunk *lc_chunks, int32_t n_lc_chunks,
+                                  const sa_chunk *be, int32_t n_be, int32_t *out_be_admitted,
+                                  double *out_budget_ms, double *out_est_ms);
+
+/* Dynamic chunking (L59, L359, L396): the largest next chunk of a lookahead prefill with `remaining`
+ * tokens over `prefix` cached ones that keeps the batch (decode_L, chunks) within budget_ms:
+ * min(remaining, max_chunk) if it fits, else the largest multiple of `granularity` below it that
+ * fits, else 0. */
+SA_API int32_t sa_dynamic_chunk(const sa_latency_model *model, const int64_t *decode_L, int32_t n_dec,
+                         const sa_chunk *chunks, int32_t n_pre, int64_t prefix, int64_t remaining,
+                         int64_t max_chunk, int64_t granularity, double budget_ms, int64_t *out_q);
+
 #ifdef __cplusplus
 }
 #endif

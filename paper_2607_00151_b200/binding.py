@@ -54,10 +54,37 @@ class sa_kv_layout(ctypes.Structure):
     ]
 
 
+SA_GEMM_TABLE_MAX = 64
+
+
+class sa_latency_model(ctypes.Structure):
+    _fields_ = [
+        ("c0_ms", ctypes.c_double),
+        ("alpha_d_ms", ctypes.c_double),
+        ("alpha_p_ms", ctypes.c_double),
+        ("n_gemm", ctypes.c_int32),
+        ("reserved", ctypes.c_int32),
+        ("gemm_m", ctypes.c_double * SA_GEMM_TABLE_MAX),
+        ("gemm_ms", ctypes.c_double * SA_GEMM_TABLE_MAX),
+    ]
+
+
+class sa_chunk(ctypes.Structure):
+    _fields_ = [("q", ctypes.c_int64), ("prefix", ctypes.c_int64)]
+
+
+class sa_lc_request(ctypes.Structure):
+    _fields_ = [("t_arrival_ms", ctypes.c_double), ("slo_ttft_ms", ctypes.c_double), ("q", ctypes.c_int64),
+                ("prefix", ctypes.c_int64)]
+
+
 _i32p = ctypes.POINTER(ctypes.c_int32)
 _i64p = ctypes.POINTER(ctypes.c_int64)
 _f32p = ctypes.POINTER(ctypes.c_float)
+_f64p = ctypes.POINTER(ctypes.c_double)
 _vp = ctypes.c_void_p
+_modelp = ctypes.POINTER(sa_latency_model)
+_chunkp = ctypes.POINTER(sa_chunk)
 
 # name -> (restype, argtypes); also the list the symbol test checks against the header
 PROTOTYPES = {
@@ -82,6 +109,14 @@ PROTOTYPES = {
     "sa_last_launch_count": (ctypes.c_int32, [_vp, _i32p]),
     "sa_latency_table": (ctypes.c_int32, [_vp, _i32p, ctypes.c_int32, _i32p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
                                           ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32, ctypes.c_int32, _f32p, _i64p, _vp]),
+    "sa_latency_fit": (ctypes.c_int32, [_f32p, _i64p, ctypes.c_int32, ctypes.c_int32, _modelp, _f64p]),
+    "sa_est_batch_latency": (ctypes.c_int32, [_modelp, _i64p, ctypes.c_int32, _chunkp, ctypes.c_int32, _f64p]),
+    "sa_schedule_hybrid": (ctypes.c_int32, [_modelp, _i64p, ctypes.c_int32, _chunkp, ctypes.c_int32, _chunkp, ctypes.c_int32,
+                                            ctypes.c_double, _i32p, _f64p]),
+    "sa_schedule_prefill_slack": (ctypes.c_int32, [_modelp, ctypes.POINTER(sa_lc_request), ctypes.c_int32, ctypes.c_double,
+                                                   _chunkp, ctypes.c_int32, _chunkp, ctypes.c_int32, _i32p, _f64p, _f64p]),
+    "sa_dynamic_chunk": (ctypes.c_int32, [_modelp, _i64p, ctypes.c_int32, _chunkp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
+                                          ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.POINTER(ctypes.c_int64)]),
 }
 
 _lib = None
@@ -334,3 +369,91 @@ def sa_latency_table(pool: Pool, prefill_tokens, decode_batch, prefill_prefix_le
                                            decode_ctx_lo, decode_ctx_hi, seed, warmup, iters, ms.ctypes.data_as(_f32p),
                                            sums.ctypes.data_as(_i64p), _stream_ptr(stream)), "sa_latency_table")
     return ms, sums
+
+
+# ---------------------------------------------------------------- scheduler core (host only)
+@dataclass
+class LatencyModel:
+    """Eq. 1 of PAPER.md (L349-353): c0 + T_GEMM(M) + alpha_d * sum L_j + alpha_p * sum A_j, in ms."""
+    c0_ms: float = 0.0
+    alpha_d_ms: float = 0.0
+    alpha_p_ms: float = 0.0
+    gemm: Sequence = ()      # [(M, ms), ...] strictly increasing in M; empty: T_GEMM = 0
+
+    def to_c(self) -> sa_latency_model:
+        m = sa_latency_model()
+        m.c0_ms, m.alpha_d_ms, m.alpha_p_ms = self.c0_ms, self.alpha_d_ms, self.alpha_p_ms
+        assert len(self.gemm) <= SA_GEMM_TABLE_MAX
+        m.n_gemm = len(self.gemm)
+        for i, (x, y) in enumerate(self.gemm):
+            m.gemm_m[i], m.gemm_ms[i] = float(x), float(y)
+        return m
+
+
+def _i64(a):
+    arr = np.ascontiguousarray(np.asarray(a, dtype=np.int64).reshape(-1))
+    return arr, arr.ctypes.data_as(_i64p)
+
+
+def _chunks(cs):
+    arr = (sa_chunk * max(len(cs), 1))()
+    for i, (q, p) in enumerate(cs):
+        arr[i].q, arr[i].prefix = int(q), int(p)
+    return arr
+
+
+def sa_latency_fit(ms, sum_kv, with_intercept: bool = True):
+    """-> (LatencyModel, max relative error of the fit); ms and sum_kv as returned by sa_latency_table."""
+    y = np.ascontiguousarray(np.asarray(ms, dtype=np.float32).reshape(-1))
+    s_keep, s_ptr = _i64(sum_kv)
+    assert s_keep.shape[0] == 2 * y.shape[0]
+    m = sa_latency_model()
+    err = ctypes.c_double(0.0)
+    _check(load_library().sa_latency_fit(y.ctypes.data_as(_f32p), s_ptr, y.shape[0], int(with_intercept), ctypes.byref(m),
+                                         ctypes.byref(err)), "sa_latency_fit")
+    return LatencyModel(m.c0_ms, m.alpha_d_ms, m.alpha_p_ms, ()), float(err.value)
+
+
+def sa_est_batch_latency(model: LatencyModel, decode_L, chunks) -> float:
+    d_keep, d_ptr = _i64(decode_L)
+    out = ctypes.c_double(0.0)
+    cm = model.to_c()
+    _check(load_library().sa_est_batch_latency(ctypes.byref(cm), d_ptr, d_keep.shape[0], _chunks(chunks), len(chunks),
+                                               ctypes.byref(out)), "sa_est_batch_latency")
+    return float(out.value)
+
+
+def sa_schedule_hybrid(model: LatencyModel, decode_L, lc, be, delta_ms: float):
+    """Algorithm 2 -> (admitted decode, LC chunks, BE chunks, estimate of the admitted batch in ms)"""
+    d_keep, d_ptr = _i64(decode_L)
+    adm = (ctypes.c_int32 * 3)()
+    est = ctypes.c_double(0.0)
+    cm = model.to_c()
+    _check(load_library().sa_schedule_hybrid(ctypes.byref(cm), d_ptr, d_keep.shape[0], _chunks(lc), len(lc), _chunks(be), len(be),
+                                             float(delta_ms), adm, ctypes.byref(est)), "sa_schedule_hybrid")
+    return int(adm[0]), int(adm[1]), int(adm[2]), float(est.value)
+
+
+def sa_schedule_prefill_slack(model: LatencyModel, lc_queue, t_now_ms: float, lc_chunks, be):
+    """Algorithm 1; lc_queue: [(t_arrival_ms, slo_ttft_ms, q, prefix), ...] -> (admitted BE chunks, t_budget, estimate)"""
+    qarr = (sa_lc_request * max(len(lc_queue), 1))()
+    for i, (ta, slo, q, p) in enumerate(lc_queue):
+        qarr[i].t_arrival_ms, qarr[i].slo_ttft_ms, qarr[i].q, qarr[i].prefix = float(ta), float(slo), int(q), int(p)
+    n = ctypes.c_int32(0)
+    budget, est = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    cm = model.to_c()
+    _check(load_library().sa_schedule_prefill_slack(ctypes.byref(cm), qarr, len(lc_queue), float(t_now_ms), _chunks(lc_chunks),
+                                                    len(lc_chunks), _chunks(be), len(be), ctypes.byref(n), ctypes.byref(budget),
+                                                    ctypes.byref(est)), "sa_schedule_prefill_slack")
+    return int(n.value), float(budget.value), float(est.value)
+
+
+def sa_dynamic_chunk(model: LatencyModel, decode_L, chunks, prefix: int, remaining: int, max_chunk: int, granularity: int,
+                     budget_ms: float) -> int:
+    d_keep, d_ptr = _i64(decode_L)
+    out = ctypes.c_int64(0)
+    cm = model.to_c()
+    _check(load_library().sa_dynamic_chunk(ctypes.byref(cm), d_ptr, d_keep.shape[0], _chunks(chunks), len(chunks), int(prefix),
+                                           int(remaining), int(max_chunk), int(granularity), float(budget_ms), ctypes.byref(out)),
+           "sa_dynamic_chunk")
+    return int(out.value)
