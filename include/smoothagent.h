@@ -287,6 +287,85 @@ SA_API int32_t sa_dynamic_chunk(const sa_latency_model *model, const int64_t *de
                          const sa_chunk *chunks, int32_t n_pre, int64_t prefix, int64_t remaining,
                          int64_t max_chunk, int64_t granularity, double budget_ms, int64_t *out_q);
 
+/* ---- dense operators of the layer (section 4 "GEMM", L299-303) ----------
+ * "All tokens in the batch, including decode tokens and prefill chunk tokens, are processed by the
+ * same dense operators in each transformer layer, including the projection matrices in attention
+ * (QKV and output projections) and the FFN layers" (L299); their cost T_GEMM(M) depends on the total
+ * number of forward tokens M only (L301-303).  The layer is BASELINE.json's "Llama-3-8B-shaped"
+ * pre-norm decoder layer without biases (readings R21-R24 in DESIGN.md):
+ *     h  = RMSNorm(x; norm1)            q|k|v = h W_qkv^T  (rows of W_qkv: Hq Q heads, Hkv K heads, Hkv V heads)
+ *     a  = attention(RoPE(q), RoPE(k), v)                   (sa_mixed_attention over the paged cache)
+ *     x1 = x + a W_o^T
+ *     h2 = RMSNorm(x1; norm2)
+ *     y  = x1 + (SiLU(h2 W_gate^T) * (h2 W_up^T)) W_down^T
+ * All tensors are device bf16, row-major, weights stored [out_features, in_features] (y = x W^T);
+ * accumulation is fp32 on the tensor cores (tcgen05, TMEM accumulators), every stored tensor is
+ * rounded once to bf16 (round to nearest even).  All calls enqueue on `stream`, never allocate and
+ * never synchronise (sa_gemm_table excepted).  Shape limits of the tcgen05 GEMM: in_features a
+ * multiple of 64, out_features a multiple of 8, every pointer 16-byte aligned, M >= 0 arbitrary. */
+
+/* y[M, N] = x[M, K] W[N, K]^T (+ residual[M, N] if non-null; y may alias residual). */
+SA_API int32_t sa_linear(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N,
+                  int32_t K, void *stream);
+
+/* act[M, F] = SiLU(x W_gate^T) * (x W_up^T): one GEMM over both weight matrices with the activation fused
+ * into its epilogue (the two products of an FFN unit are accumulated side by side in TMEM). */
+SA_API int32_t sa_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F,
+                  int32_t K, void *stream);
+
+/* y[M, H] = x / sqrt(mean_j x_j^2 + eps) * w  (fp32 arithmetic, one rounding). */
+SA_API int32_t sa_rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, void *stream);
+
+/* Fused QKV projection + RoPE + KV append: the same effect as projecting h with W_qkv and handing the
+ * result to sa_rope_kv_append, but K', V go from the fp32 accumulators straight into the pool pages
+ * and Q' into q_out, each rounded once (the unfused route rounds q, k twice).  Requests, positions,
+ * page allocation, copy-on-write and failure behaviour are exactly sa_rope_kv_append's.
+ *   h      : device bf16 [T, hidden]  (the normalised hidden states of the batch's new tokens)
+ *   w_qkv  : device bf16 [(Hq + 2 Hkv) * D, hidden]
+ *   q_out  : device bf16 [T, Hq, D], rotated queries for sa_mixed_attention
+ *   workspace : device, >= sa_qkv_rope_append_workspace_bytes(T) (per-token cos/sin and slot table)
+ * Only head_dim 128 (SA_ERR_UNSUPPORTED otherwise). */
+SA_API int32_t sa_qkv_rope_append_workspace_bytes(const sa_kv_pool *pool, int64_t total_tokens, size_t *out_bytes);
+SA_API int32_t sa_qkv_rope_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
+                           const void *h, const void *w_qkv, int32_t hidden, void *q_out, void *workspace,
+                           size_t workspace_bytes, void *stream);
+
+typedef struct {
+    int32_t hidden;      /* H */
+    int32_t ffn;         /* F */
+    float rms_eps;
+    int32_t reserved;
+    const void *norm1;   /* device bf16 [H] */
+    const void *w_qkv;   /* device bf16 [(Hq + 2 Hkv) * D, H] */
+    const void *w_o;     /* device bf16 [H, Hq * D] */
+    const void *norm2;   /* device bf16 [H] */
+    const void *w_gate;  /* device bf16 [F, H] */
+    const void *w_up;    /* device bf16 [F, H] */
+    const void *w_down;  /* device bf16 [H, F] */
+} sa_layer_weights;
+
+/* One decoder layer over a mixed batch (the formulas above): RMSNorm, fused QKV + RoPE + append,
+ * sa_mixed_attention, output projection + residual, RMSNorm, SwiGLU GEMM, down projection + residual.
+ * The batch is described as for sa_rope_kv_append (request r appends and queries q_r new tokens:
+ * a prefill chunk if q_r > 1, a decode row if q_r == 1).
+ *   x : device bf16 [T, H] in;  y : device bf16 [T, H] out (may alias x)
+ *   workspace : device, >= sa_layer_workspace_bytes(...) for the same batch */
+SA_API int32_t sa_layer_workspace_bytes(const sa_kv_pool *pool, const sa_layer_weights *layer, int32_t n_req,
+                                 const int32_t *sids, const int32_t *qo_indptr, size_t *out_bytes);
+SA_API int32_t sa_layer_forward(sa_kv_pool *pool, const sa_layer_weights *layer, int32_t n_req, const int32_t *sids,
+                         const int32_t *qo_indptr, const void *x, void *y, float sm_scale, void *workspace,
+                         size_t workspace_bytes, void *stream);
+
+/* T_GEMM(M), the "offline-profiled lookup table" of L303: for every M in m_list the time of the layer's
+ * dense operators on M tokens (QKV projection, output projection + residual, SwiGLU GEMM, down
+ * projection + residual, the two RMSNorms), median over iters of CUDA-event times on `stream`, L2
+ * evicted between iterations.  NOT a hot call: allocates its own activations and weights of the given
+ * shape (cudaMalloc, values irrelevant to the timing), synchronises, frees.  The result goes into
+ * sa_latency_model.gemm_m / gemm_ms. */
+SA_API int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
+                      const int32_t *m_list, int32_t n_m, int32_t warmup, int32_t iters, float *out_ms,
+                      void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -78,6 +78,12 @@ class sa_lc_request(ctypes.Structure):
                 ("prefix", ctypes.c_int64)]
 
 
+class sa_layer_weights(ctypes.Structure):
+    _fields_ = [("hidden", ctypes.c_int32), ("ffn", ctypes.c_int32), ("rms_eps", ctypes.c_float), ("reserved", ctypes.c_int32),
+                ("norm1", ctypes.c_void_p), ("w_qkv", ctypes.c_void_p), ("w_o", ctypes.c_void_p), ("norm2", ctypes.c_void_p),
+                ("w_gate", ctypes.c_void_p), ("w_up", ctypes.c_void_p), ("w_down", ctypes.c_void_p)]
+
+
 _i32p = ctypes.POINTER(ctypes.c_int32)
 _i64p = ctypes.POINTER(ctypes.c_int64)
 _f32p = ctypes.POINTER(ctypes.c_float)
@@ -117,6 +123,18 @@ PROTOTYPES = {
                                                    _chunkp, ctypes.c_int32, _chunkp, ctypes.c_int32, _i32p, _f64p, _f64p]),
     "sa_dynamic_chunk": (ctypes.c_int32, [_modelp, _i64p, ctypes.c_int32, _chunkp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
                                           ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.POINTER(ctypes.c_int64)]),
+    "sa_linear": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp]),
+    "sa_swiglu": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp]),
+    "sa_rmsnorm": (ctypes.c_int32, [_vp, _vp, ctypes.c_float, _vp, ctypes.c_int64, ctypes.c_int32, _vp]),
+    "sa_qkv_rope_append_workspace_bytes": (ctypes.c_int32, [_vp, ctypes.c_int64, ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_qkv_rope_append": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _vp, _vp, ctypes.c_int32, _vp, _vp,
+                                            ctypes.c_size_t, _vp]),
+    "sa_layer_workspace_bytes": (ctypes.c_int32, [_vp, ctypes.POINTER(sa_layer_weights), ctypes.c_int32, _i32p, _i32p,
+                                                  ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_layer_forward": (ctypes.c_int32, [_vp, ctypes.POINTER(sa_layer_weights), ctypes.c_int32, _i32p, _i32p, _vp, _vp,
+                                          ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
+    "sa_gemm_table": (ctypes.c_int32, [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p,
+                                       ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _f32p, _vp]),
 }
 
 _lib = None
@@ -457,3 +475,93 @@ def sa_dynamic_chunk(model: LatencyModel, decode_L, chunks, prefix: int, remaini
                                            int(remaining), int(max_chunk), int(granularity), float(budget_ms), ctypes.byref(out)),
            "sa_dynamic_chunk")
     return int(out.value)
+
+
+# ---------------------------------------------------------------- dense operators of the layer (N3)
+def _nbytes(t) -> int:
+    return 0 if t is None else t.numel() * t.element_size()
+
+
+def sa_linear(x, w, y, residual=None, stream=None) -> None:
+    """y[M, N] = x[M, K] w[N, K]^T (+ residual)."""
+    M, K = x.shape
+    N = w.shape[0]
+    assert w.shape[1] == K and tuple(y.shape) == (M, N)
+    _check(load_library().sa_linear(_ptr(x), _ptr(w), _ptr(residual), _ptr(y), M, N, K, _stream_ptr(stream)), "sa_linear")
+
+
+def sa_swiglu(x, w_gate, w_up, act, stream=None) -> None:
+    M, K = x.shape
+    F = w_gate.shape[0]
+    assert w_gate.shape == w_up.shape and w_gate.shape[1] == K and tuple(act.shape) == (M, F)
+    _check(load_library().sa_swiglu(_ptr(x), _ptr(w_gate), _ptr(w_up), _ptr(act), M, F, K, _stream_ptr(stream)), "sa_swiglu")
+
+
+def sa_rmsnorm(x, w, eps: float, y, stream=None) -> None:
+    M, H = x.shape
+    assert w.shape[0] == H and y.shape == x.shape
+    _check(load_library().sa_rmsnorm(_ptr(x), _ptr(w), float(eps), _ptr(y), M, H, _stream_ptr(stream)), "sa_rmsnorm")
+
+
+def sa_qkv_rope_append_workspace_bytes(pool: Pool, total_tokens: int) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_qkv_rope_append_workspace_bytes(pool.handle, total_tokens, ctypes.byref(out)),
+           "sa_qkv_rope_append_workspace_bytes")
+    return int(out.value)
+
+
+def sa_qkv_rope_append(pool: Pool, sids, qo_indptr, h, w_qkv, q_out, workspace, stream=None) -> None:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    assert i_keep.shape[0] == s_keep.shape[0] + 1
+    hidden = w_qkv.shape[1]
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_qkv_rope_append(pool.handle, s_keep.shape[0], s_ptr, i_ptr, _ptr(h), _ptr(w_qkv), hidden,
+                                             _ptr(q_out), _ptr(workspace), _nbytes(workspace), sp), "sa_qkv_rope_append")
+
+
+@dataclass
+class LayerWeights:
+    """Device bf16 tensors of one decoder layer, weights [out_features, in_features]."""
+    norm1: object
+    w_qkv: object
+    w_o: object
+    norm2: object
+    w_gate: object
+    w_up: object
+    w_down: object
+    rms_eps: float = 1e-5
+
+    def to_c(self) -> sa_layer_weights:
+        return sa_layer_weights(self.w_qkv.shape[1], self.w_gate.shape[0], self.rms_eps, 0, _ptr(self.norm1), _ptr(self.w_qkv),
+                                _ptr(self.w_o), _ptr(self.norm2), _ptr(self.w_gate), _ptr(self.w_up), _ptr(self.w_down))
+
+
+def sa_layer_workspace_bytes(pool: Pool, layer: LayerWeights, sids, qo_indptr) -> int:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    c = layer.to_c()
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_layer_workspace_bytes(pool.handle, ctypes.byref(c), s_keep.shape[0], s_ptr, i_ptr, ctypes.byref(out)),
+           "sa_layer_workspace_bytes")
+    return int(out.value)
+
+
+def sa_layer_forward(pool: Pool, layer: LayerWeights, sids, qo_indptr, x, y, workspace, sm_scale: float = 0.0, stream=None) -> None:
+    s_keep, s_ptr = _i32(sids)
+    i_keep, i_ptr = _i32(qo_indptr)
+    assert i_keep.shape[0] == s_keep.shape[0] + 1
+    c = layer.to_c()
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_layer_forward(pool.handle, ctypes.byref(c), s_keep.shape[0], s_ptr, i_ptr, _ptr(x), _ptr(y),
+                                           float(sm_scale), _ptr(workspace), _nbytes(workspace), sp), "sa_layer_forward")
+
+
+def sa_gemm_table(hidden: int, ffn: int, num_q_heads: int, num_kv_heads: int, head_dim: int, m_list, warmup: int = 3,
+                  iters: int = 10, stream=None):
+    """-> ms float32 [len(m_list)]: T_GEMM(M) of PAPER.md L299-303 measured on this library's kernels."""
+    m_keep, m_ptr = _i32(m_list)
+    ms = np.zeros(m_keep.shape[0], dtype=np.float32)
+    _check(load_library().sa_gemm_table(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_ptr, m_keep.shape[0], warmup, iters,
+                                        ms.ctypes.data_as(_f32p), _stream_ptr(stream)), "sa_gemm_table")
+    return ms

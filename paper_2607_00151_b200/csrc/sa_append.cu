@@ -78,15 +78,7 @@ rope_append_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t tota
     __syncthreads();
     for (int e = tid; e < n_tok * HALF; e += kAppendThreads) {
         const int tl = e / HALF, m = e % HALF;
-        const float2 u = rope_tab[m];
-        const float p = float(s_pos[tl]);          // exact: positions < 2^24
-        const float ph = p * u.x;
-        float pl = fmaf(p, u.x, -ph);              // exact error of the product
-        pl = fmaf(p, u.y, pl);
-        const float fr = (ph - rintf(ph)) + pl;    // turns, |fr| <= 0.5 (+ tiny)
-        float sn, cs;
-        sincospif(2.0f * fr, &sn, &cs);
-        s_cs[tl][m] = make_float2(cs, sn);
+        s_cs[tl][m] = rope_cos_sin(s_pos[tl], rope_tab[m]);
     }
     __syncthreads();
 
@@ -174,10 +166,16 @@ cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
 
 }  // namespace sa
 
-extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
-                                     const int32_t *qo_indptr, const void *k, const void *v, void *q_inout,
-                                     void *stream_) {
-    using namespace sa;
+namespace sa {
+
+// Host half of an append (step a1): validates the batch, allocates pages (copy-on-write of a shared
+// partial page included), grows the sessions, sends the per-request metadata and the new page ids to
+// the device and enqueues the block-table update.  *reqs_dev: the ReqMeta array of the call on the
+// device (kv_len = position of the request's first new token).  Nothing is changed on failure.
+int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
+                       bool have_data, cudaStream_t stream, const ReqMeta **reqs_dev_out, int64_t *total_out) {
+    *reqs_dev_out = nullptr;
+    *total_out = 0;
     if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
     if (n_req == 0) {
         pool->last_launches = 0;
@@ -203,7 +201,7 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
     }
     const int64_t total = qo_indptr[n_req];
     if (need_pages > int64_t(pool->free_pages.size())) return SA_ERR_OUT_OF_PAGES;
-    if (!pool->host_only && total > 0 && (!k || !v)) return SA_ERR_INVALID_ARG;
+    if (!pool->host_only && total > 0 && !have_data) return SA_ERR_INVALID_ARG;
 
     char *mh = nullptr, *md = nullptr;
     if (!pool->host_only) {
@@ -264,7 +262,6 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
     pool->last_launches = 0;
     if (pool->host_only) return SA_OK;
 
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     for (const auto &c : cow)
         if (copy_page_async(pool, c.first, c.second, stream) != cudaSuccess) return SA_ERR_CUDA;
     // slab layout: [ReqMeta x n_req][new page ids x n_list][ReqMeta x n_gain]
@@ -282,6 +279,22 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
         ++pool->last_launches;
     }
     if (cudaGetLastError() != cudaSuccess) return SA_ERR_CUDA;
+    *reqs_dev_out = reqs_dev;
+    *total_out = total;
+    return SA_OK;
+}
+
+}  // namespace sa
+
+extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                     const int32_t *qo_indptr, const void *k, const void *v, void *q_inout,
+                                     void *stream_) {
+    using namespace sa;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const ReqMeta *reqs_dev = nullptr;
+    int64_t total = 0;
+    const int32_t st = append_prepare(pool, n_req, sids, qo_indptr, k && v, stream, &reqs_dev, &total);
+    if (st != SA_OK || !reqs_dev) return st;
     if (launch_rope_append(pool, reqs_dev, n_req, total, k, v, q_inout, stream, &pool->last_launches) != cudaSuccess)
         return SA_ERR_CUDA;
     return SA_OK;

@@ -30,7 +30,7 @@ struct HostPlan {
 // The split of a request depends only on that request (never on its batch), so co-batching
 // cannot change the bits of a row.
 int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
-                   HostPlan *hp) {
+                   HostPlan *hp, bool before_append = false) {
     if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
     if (n_req == 0) return SA_OK;
     if (!sids || !qo_indptr || qo_indptr[0] != 0 || n_req > pool->cfg.max_sessions) return SA_ERR_INVALID_ARG;
@@ -42,8 +42,9 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
         const int32_t sid = sids[r];
         if (sid < 0 || size_t(sid) >= pool->sessions.size() || !pool->sessions[size_t(sid)].open) return SA_ERR_INVALID_ARG;
         const int64_t n = int64_t(qo_indptr[r + 1]) - qo_indptr[r];
-        const int64_t kv = pool->sessions[size_t(sid)].len;
-        if (n < 0 || n > kv) return SA_ERR_INVALID_ARG;  // the request's own tokens must already be appended
+        if (n < 0) return SA_ERR_INVALID_ARG;
+        const int64_t kv = pool->sessions[size_t(sid)].len + (before_append ? n : 0);
+        if (n > kv) return SA_ERR_INVALID_ARG;  // the request's own tokens must already be appended
         if (n == 0) continue;
         ReqMeta m{};
         m.sid = sid;
@@ -122,6 +123,16 @@ void write_sched_payload(const Tc5Schedule &sc, char *dst) {
 }
 
 }  // namespace
+
+int32_t attention_workspace_after_append(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                         const int32_t *qo_indptr, size_t *out_bytes) {
+    HostPlan hp;
+    const int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hp, true);
+    if (st != SA_OK) return st;
+    *out_bytes = workspace_need(pool, hp);
+    return SA_OK;
+}
+
 }  // namespace sa
 
 extern "C" int32_t sa_mixed_attention_workspace_bytes(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,

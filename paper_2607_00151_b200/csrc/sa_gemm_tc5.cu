@@ -1,0 +1,500 @@
+// sa_gemm_tc5.cu -- the dense operators of the layer on the tcgen05 tensor cores (
+// PAPER.md section 4 "GEMM", L299-303: "the projection matrices in attention (QKV and output
+// projections) and the FFN layers", whose cost T_GEMM(M) depends on the forward tokens M only).
+//
+// One persistent warp-specialised kernel, y = x W^T with x [M, K] and W [N, K] both K-major bf16:
+//   warp 0      TMA producer: a 4-stage ring of (A 128 x 64, B 256 x 64) SWIZZLE_128B tiles
+//   warp 1      one lane issues tcgen05.mma 128 x 256 x 16 (cta_group::1), fp32 accumulators in TMEM
+//   warp 2      TMEM allocator (all 512 columns = two 128 x 256 accumulators)
+//   warps 4-7   epilogue: thread = output row, tcgen05.ld of the accumulator while the MMA warp is
+//               already filling the other accumulator with the next tile
+// and three epilogues (template EPI):
+//   EPI_PLAIN   y = acc (+ residual), bf16                            (output / down projection)
+//   EPI_SWIGLU  B tile = 128 gate rows + 128 up rows of the same FFN units:
+//               act = SiLU(acc_gate) * acc_up                         (sa_swiglu)
+//   EPI_QKV     a tile is two heads of the fused QKV projection: Q and K heads are rotated (RoPE,
+//               half-split pairs m / m+64 sit in the same thread's row), K' and V are scattered
+//               into the pool pages through the per-token slot table, Q' goes to q_out
+//               (sa_qkv_rope_append: "KV cache construction", L168)
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "sa_internal.h"
+#include "sa_tc5_ptx.cuh"
+
+namespace sa {
+
+using namespace ptx;
+
+namespace {
+
+constexpr int GBM = 128, GBN = 256, GBK = 64, GSTAGES = 4;
+constexpr uint32_t A_STAGE = GBM * GBK * 2;   // 16 KiB
+constexpr uint32_t B_HALF = 128 * GBK * 2;    // 16 KiB: 128 rows of W
+constexpr uint32_t B_STAGE = 2 * B_HALF;      // 32 KiB
+constexpr uint32_t STAGE_BYTES = A_STAGE + B_STAGE;
+constexpr int kGemmThreads = 256;
+constexpr size_t kSmemGemm = size_t(GSTAGES) * STAGE_BYTES + 1024;
+constexpr int M_GROUP = 16;  // m-tiles walked fastest, so that concurrently running CTAs share W tiles in L2
+
+enum { EPI_PLAIN = 0, EPI_SWIGLU = 1, EPI_QKV = 2 };
+
+struct GemmArgs {
+    int64_t M;
+    int32_t N;        // output features (EPI_SWIGLU: FFN units F)
+    int32_t K;
+    int32_t m_tiles, n_tiles;
+    __nv_bfloat16 *y;
+    const __nv_bfloat16 *residual;
+    int64_t ldy;
+    // EPI_QKV
+    const float2 *cs;          // [T][64] (cos, sin) at the token's absolute position
+    const int64_t *tok_off;    // [T] element offset of (page, head 0, slot, 0) in the K / V page arrays
+    __nv_bfloat16 *k_base, *v_base, *q_out;
+    int64_t stride_head;
+    int32_t Hq, Hkv;
+};
+
+__device__ __forceinline__ void tile_coords(const GemmArgs &a, int t, int &mt, int &nt) {
+    const int per_group = M_GROUP * a.n_tiles;
+    const int g = t / per_group, r = t - g * per_group;
+    const int gm = min(M_GROUP, a.m_tiles - g * M_GROUP);
+    mt = g * M_GROUP + r % gm;
+    nt = r / gm;
+}
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+    __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&p);
+}
+
+// 32 fp32 accumulator values of one row -> 32 bf16 = 64 bytes at dst (16-byte aligned)
+__device__ __forceinline__ void store_row32(__nv_bfloat16 *dst, const float (&f)[32], int n_valid = 32) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (8 * i >= n_valid) break;  // ragged last columns: N is a multiple of 8
+        uint4 u;
+        u.x = pack_bf16x2(f[8 * i + 0], f[8 * i + 1]);
+        u.y = pack_bf16x2(f[8 * i + 2], f[8 * i + 3]);
+        u.z = pack_bf16x2(f[8 * i + 4], f[8 * i + 5]);
+        u.w = pack_bf16x2(f[8 * i + 6], f[8 * i + 7]);
+        *reinterpret_cast<uint4 *>(dst + 8 * i) = u;
+    }
+}
+
+__device__ __forceinline__ void ld_row32(uint32_t taddr, float (&f)[32]) {
+    uint32_t r[32];
+    tmem_ld32(taddr, r);
+    tmem_wait_ld();
+#pragma unroll
+    for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(r[i]);
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b0,
+                const __grid_constant__ CUtensorMap tmap_b1, const GemmArgs a) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const uint32_t s0 = smem_u32(smem);
+    __shared__ uint64_t bars[2 * GSTAGES + 4];
+    __shared__ uint32_t tmem_base_smem;
+    const uint32_t bar0 = smem_u32(&bars[0]);
+    auto bar_full = [&](int s) -> uint32_t { return bar0 + 8u * uint32_t(s); };
+    auto bar_empty = [&](int s) -> uint32_t { return bar0 + 8u * uint32_t(GSTAGES + s); };
+    auto bar_acc_full = [&](int b) -> uint32_t { return bar0 + 8u * uint32_t(2 * GSTAGES + b); };
+    auto bar_acc_empty = [&](int b) -> uint32_t { return bar0 + 8u * uint32_t(2 * GSTAGES + 2 + b); };
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int n_tiles_total = a.m_tiles * a.n_tiles;
+    const int k_steps = a.K / GBK;
+
+    if (tid == 0) {
+        for (int s = 0; s < GSTAGES; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_empty(s), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_acc_full(b), 1);
+            mbar_init(bar_acc_empty(b), 128);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 2) tmem_alloc<512>(smem_u32(&tmem_base_smem));
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base_smem;
+
+    if (warp == 0) {
+        // =========================== TMA producer ===========================
+        if (lane == 0) {
+            prefetch_tmap(&tmap_a);
+            prefetch_tmap(&tmap_b0);
+            prefetch_tmap(&tmap_b1);
+            int kc = 0;
+            for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x) {
+                int mt, nt;
+                tile_coords(a, t, mt, nt);
+                const int m0 = mt * GBM;
+                const int r0 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN;        // rows of W (b0)
+                const int r1 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN + 128;  // rows of the second half (b1)
+                for (int ks = 0; ks < k_steps; ++ks, ++kc) {
+                    const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
+                    mbar_wait(bar_empty(s), ph ^ 1);
+                    const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
+                    mbar_expect_tx(bar_full(s), STAGE_BYTES);
+                    tma_load_2d(sA, &tmap_a, bar_full(s), ks * GBK, m0);
+                    tma_load_2d(sB, &tmap_b0, bar_full(s), ks * GBK, r0);
+                    tma_load_2d(sB + B_HALF, &tmap_b1, bar_full(s), ks * GBK, r1);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer ===========================
+        constexpr uint32_t idesc = umma_idesc_bf16(GBM, GBN, false, false);
+        int kc = 0, tc = 0;
+        for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x, ++tc) {
+            const int b = tc & 1;
+            mbar_wait(bar_acc_empty(b), ((tc >> 1) & 1) ^ 1);  // the epilogue has drained this accumulator
+            tc_fence_after();
+            for (int ks = 0; ks < k_steps; ++ks, ++kc) {
+                const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
+                mbar_wait(bar_full(s), ph);
+                tc_fence_after();
+                if (lane == 0) {
+                    const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
+#pragma unroll
+                    for (int kk = 0; kk < GBK / 16; ++kk)
+                        umma_ss(tmem + b * GBN, umma_desc(sA + kk * 32, 16, 1024), umma_desc(sB + kk * 32, 16, 1024), idesc,
+                                ks > 0 || kk > 0);
+                    umma_commit(bar_empty(s));
+                    if (ks == k_steps - 1) umma_commit(bar_acc_full(b));
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp >= 4) {
+        // =========================== epilogue ===========================
+        const int q4 = warp & 3;                 // TMEM lane quarter this warp may read
+        const int row_in_tile = q4 * 32 + lane;
+        const uint32_t lane_addr = uint32_t(q4 * 32) << 16;
+        int tc = 0;
+        for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x, ++tc) {
+            const int b = tc & 1;
+            int mt, nt;
+            tile_coords(a, t, mt, nt);
+            const int64_t row = int64_t(mt) * GBM + row_in_tile;
+            const bool live = row < a.M;
+            mbar_wait(bar_acc_full(b), (tc >> 1) & 1);
+            tc_fence_after();
+            const uint32_t acc = tmem + lane_addr + b * GBN;
+            if (EPI == EPI_PLAIN) {
+                const int n0 = nt * GBN;
+#pragma unroll 1
+                for (int c = 0; c < GBN / 32; ++c) {
+                    const int col = n0 + c * 32;
+                    if (col >= a.N) break;  // uniform over the CTA
+                    float f[32];
+                    ld_row32(acc + c * 32, f);
+                    if (live) {
+                        __nv_bfloat16 *dst = a.y + row * a.ldy + col;
+                        if (a.residual) {
+                            const __nv_bfloat16 *rs = a.residual + row * a.ldy + col;
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                if (col + 8 * i >= a.N) break;
+                                const uint4 u = *reinterpret_cast<const uint4 *>(rs + 8 * i);
+                                const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) {
+                                    f[8 * i + 2 * j] += __uint_as_float(w[j] << 16);
+                                    f[8 * i + 2 * j + 1] += __uint_as_float(w[j] & 0xffff0000u);
+                                }
+                            }
+                        }
+                        store_row32(dst, f, a.N - col);
+                    }
+                }
+            } else if (EPI == EPI_SWIGLU) {
+                const int f0 = nt * 128;
+#pragma unroll 1
+                for (int c = 0; c < 4; ++c) {
+                    const int col = f0 + c * 32;
+                    if (col >= a.N) break;
+                    float g[32], u[32];
+                    ld_row32(acc + c * 32, g);
+                    ld_row32(acc + 128 + c * 32, u);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const float e = ex2_approx(-1.4426950408889634f * g[i]);
+                        g[i] = __fdividef(g[i], 1.0f + e) * u[i];
+                    }
+                    if (live) {
+                        __nv_bfloat16 *dst = a.y + row * a.ldy + col;
+                        store_row32(dst, g, a.N - col);
+                    }
+                }
+            } else {  // EPI_QKV: two heads of 128 dims per tile
+                const int64_t off = live ? a.tok_off[row] : 0;
+#pragma unroll 1
+                for (int hh = 0; hh < 2; ++hh) {
+                    const int head = nt * 2 + hh;
+                    if (head >= a.Hq + 2 * a.Hkv) break;
+                    const bool rot = head < a.Hq + a.Hkv;
+                    __nv_bfloat16 *dst;
+                    if (head < a.Hq)
+                        dst = a.q_out + (row * a.Hq + head) * 128;
+                    else if (head < a.Hq + a.Hkv)
+                        dst = a.k_base + off + int64_t(head - a.Hq) * a.stride_head;
+                    else
+                        dst = a.v_base + off + int64_t(head - a.Hq - a.Hkv) * a.stride_head;
+#pragma unroll 1
+                    for (int m0 = 0; m0 < 64; m0 += 32) {
+                        float lo[32], hi[32];
+                        ld_row32(acc + hh * 128 + m0, lo);
+                        ld_row32(acc + hh * 128 + 64 + m0, hi);
+                        if (live) {
+                            if (rot) {
+                                const float4 *csp = reinterpret_cast<const float4 *>(a.cs + row * 64 + m0);
+#pragma unroll
+                                for (int i = 0; i < 16; ++i) {
+                                    const float4 c2 = __ldg(csp + i);  // (cos, sin) of dims 2i, 2i+1
+                                    const float x0 = lo[2 * i], x1 = hi[2 * i];
+                                    lo[2 * i] = fmaf(x0, c2.x, -(x1 * c2.y));
+                                    hi[2 * i] = fmaf(x1, c2.x, x0 * c2.y);
+                                    const float z0 = lo[2 * i + 1], z1 = hi[2 * i + 1];
+                                    lo[2 * i + 1] = fmaf(z0, c2.z, -(z1 * c2.w));
+                                    hi[2 * i + 1] = fmaf(z1, c2.z, z0 * c2.w);
+                                }
+                            }
+                            store_row32(dst + m0, lo);
+                            store_row32(dst + 64 + m0, hi);
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(bar_acc_empty(b));
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc<512>(tmem);
+}
+
+// Per token of a fused QKV append: the slot it lands in and (cos, sin) of its absolute position.
+__global__ void __launch_bounds__(256)
+qkv_token_table_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t total_rows,
+                       const int32_t *__restrict__ block_table, int64_t mpps, int32_t log2_page, int64_t stride_page,
+                       const float2 *__restrict__ rope_tab, float2 *__restrict__ cs, int64_t *__restrict__ tok_off) {
+    __shared__ int32_t s_pos[4];
+    const int64_t t0 = int64_t(blockIdx.x) * 4;
+    const int tid = threadIdx.x;
+    if (tid < 4 && t0 + tid < total_rows) {
+        const int64_t t = t0 + tid;
+        int lo = 0, hi = n_req - 1;  // last request with q_start <= t
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (reqs[mid].q_start <= t) lo = mid; else hi = mid - 1;
+        }
+        const ReqMeta r = reqs[lo];
+        const int32_t pos = r.kv_len + int32_t(t - r.q_start);
+        const int32_t page = block_table[int64_t(r.sid) * mpps + (pos >> log2_page)];
+        const int32_t slot = pos & ((1 << log2_page) - 1);
+        s_pos[tid] = pos;
+        tok_off[t] = int64_t(page) * stride_page + int64_t(slot) * 128;
+    }
+    __syncthreads();
+    const int tl = tid >> 6, m = tid & 63;
+    if (t0 + tl < total_rows) cs[(t0 + tl) * 64 + m] = rope_cos_sin(s_pos[tl], rope_tab[m]);
+}
+
+// RMSNorm (reading R22): one warp per row, fp32, the row is read twice (the second pass hits L1).
+__global__ void __launch_bounds__(256)
+rmsnorm_kernel(const __nv_bfloat16 *__restrict__ x, const __nv_bfloat16 *__restrict__ w, float eps,
+               __nv_bfloat16 *__restrict__ y, int64_t M, int32_t H) {
+    const int64_t row = int64_t(blockIdx.x) * 8 + (threadIdx.x >> 5);
+    if (row >= M) return;
+    const int lane = threadIdx.x & 31;
+    const uint4 *xr = reinterpret_cast<const uint4 *>(x + row * H);
+    const uint4 *wr = reinterpret_cast<const uint4 *>(w);
+    uint4 *yr = reinterpret_cast<uint4 *>(y + row * H);
+    const int nv = H / 8;
+    float ss = 0.f;
+    for (int i = lane; i < nv; i += 32) {
+        const uint4 u = xr[i];
+        const uint32_t v[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float a0 = __uint_as_float(v[j] << 16), a1 = __uint_as_float(v[j] & 0xffff0000u);
+            ss = fmaf(a0, a0, ss);
+            ss = fmaf(a1, a1, ss);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    const float inv = rsqrtf(ss / float(H) + eps);
+    for (int i = lane; i < nv; i += 32) {
+        const uint4 u = xr[i], g = wr[i];
+        const uint32_t v[4] = {u.x, u.y, u.z, u.w}, gw[4] = {g.x, g.y, g.z, g.w};
+        uint32_t o[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float a0 = __uint_as_float(v[j] << 16) * inv * __uint_as_float(gw[j] << 16);
+            const float a1 = __uint_as_float(v[j] & 0xffff0000u) * inv * __uint_as_float(gw[j] & 0xffff0000u);
+            o[j] = pack_bf16x2(a0, a1);
+        }
+        yr[i] = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// [rows][K] bf16 row-major, box = 64 columns x 128 rows, SWIZZLE_128B (rows past the end read as zeros)
+bool make_tmap_2d(CUtensorMap *tm, const void *base, int64_t rows, int32_t K) {
+    EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(tensor_map_encode_fn());
+    if (!enc) return false;
+    cuuint64_t dims[2] = {cuuint64_t(K), cuuint64_t(rows > 0 ? rows : 1)};
+    cuuint64_t strides[1] = {cuuint64_t(K) * 2};
+    cuuint32_t box[2] = {64, 128};
+    cuuint32_t es[2] = {1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int device_sms() {
+    static int sms[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+    if (sms[dev] == 0) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+        sms[dev] = n;
+    }
+    return sms[dev];
+}
+
+template <int EPI>
+cudaError_t launch_gemm(const CUtensorMap &ta, const CUtensorMap &tb0, const CUtensorMap &tb1, const GemmArgs &a,
+                        cudaStream_t stream) {
+    static bool attr_done = false;  // (per process; the attribute is set again on every device change below)
+    static int attr_dev = -1;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!attr_done || attr_dev != dev) {
+        cudaError_t e = cudaFuncSetAttribute(gemm_tc5_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemGemm));
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+        attr_dev = dev;
+    }
+    const int sms = device_sms();
+    if (sms <= 0) return cudaErrorNoDevice;
+    const int tiles = a.m_tiles * a.n_tiles;
+    gemm_tc5_kernel<EPI><<<unsigned(std::min(tiles, sms)), kGemmThreads, kSmemGemm, stream>>>(ta, tb0, tb1, a);
+    return cudaGetLastError();
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+}  // namespace
+
+// y[M, N] = x W^T (+ residual): shared by sa_linear and sa_layer_forward
+int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
+                   cudaStream_t stream) {
+    if (M < 0 || N <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
+    if (K % GBK != 0 || N % 8 != 0 || M > (int64_t(1) << 30)) return SA_ERR_UNSUPPORTED;
+    if (M == 0) return SA_OK;
+    if (!x || !w || !y || !aligned16(x) || !aligned16(w) || !aligned16(y) || !aligned16(residual)) return SA_ERR_INVALID_ARG;
+    alignas(64) CUtensorMap ta, tb;
+    if (!make_tmap_2d(&ta, x, M, K) || !make_tmap_2d(&tb, w, N, K)) return SA_ERR_CUDA;
+    GemmArgs a{};
+    a.M = M;
+    a.N = N;
+    a.K = K;
+    a.m_tiles = int32_t((M + GBM - 1) / GBM);
+    a.n_tiles = (N + GBN - 1) / GBN;
+    a.y = static_cast<__nv_bfloat16 *>(y);
+    a.residual = static_cast<const __nv_bfloat16 *>(residual);
+    a.ldy = N;
+    return launch_gemm<EPI_PLAIN>(ta, tb, tb, a, stream) == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+}
+
+int32_t gemm_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
+                    cudaStream_t stream) {
+    if (M < 0 || F <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
+    if (K % GBK != 0 || F % 8 != 0 || M > (int64_t(1) << 30)) return SA_ERR_UNSUPPORTED;
+    if (M == 0) return SA_OK;
+    if (!x || !w_gate || !w_up || !act || !aligned16(x) || !aligned16(w_gate) || !aligned16(w_up) || !aligned16(act))
+        return SA_ERR_INVALID_ARG;
+    alignas(64) CUtensorMap ta, tg, tu;
+    if (!make_tmap_2d(&ta, x, M, K) || !make_tmap_2d(&tg, w_gate, F, K) || !make_tmap_2d(&tu, w_up, F, K)) return SA_ERR_CUDA;
+    GemmArgs a{};
+    a.M = M;
+    a.N = F;
+    a.K = K;
+    a.m_tiles = int32_t((M + GBM - 1) / GBM);
+    a.n_tiles = (F + 127) / 128;
+    a.y = static_cast<__nv_bfloat16 *>(act);
+    a.ldy = F;
+    return launch_gemm<EPI_SWIGLU>(ta, tg, tu, a, stream) == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+}
+
+int32_t rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, cudaStream_t stream) {
+    if (M < 0 || H <= 0) return SA_ERR_INVALID_ARG;
+    if (H % 8 != 0) return SA_ERR_UNSUPPORTED;
+    if (M == 0) return SA_OK;
+    if (!x || !w || !y || !aligned16(x) || !aligned16(w) || !aligned16(y)) return SA_ERR_INVALID_ARG;
+    rmsnorm_kernel<<<unsigned((M + 7) / 8), 256, 0, stream>>>(static_cast<const __nv_bfloat16 *>(x),
+                                                              static_cast<const __nv_bfloat16 *>(w), eps,
+                                                              static_cast<__nv_bfloat16 *>(y), M, H);
+    return cudaGetLastError() == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+}
+
+size_t qkv_workspace_bytes(int64_t total) {
+    const size_t T = size_t(std::max<int64_t>(total, 0));
+    return (T * 64 * sizeof(float2) + 255) / 256 * 256 + (T * sizeof(int64_t) + 255) / 256 * 256 + 256;
+}
+
+// the device half of sa_qkv_rope_append, after append_prepare has placed the tokens
+int32_t qkv_rope_append_device(sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req, int64_t total, const void *h,
+                               const void *w_qkv, int32_t hidden, void *q_out, void *workspace, cudaStream_t stream) {
+    const sa_kv_pool_config &c = pool->cfg;
+    const int32_t N = (c.num_q_heads + 2 * c.num_kv_heads) * 128;
+    uintptr_t w = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255);
+    float2 *cs = reinterpret_cast<float2 *>(w);
+    int64_t *tok_off = reinterpret_cast<int64_t *>(w + (size_t(total) * 64 * sizeof(float2) + 255) / 256 * 256);
+    qkv_token_table_kernel<<<unsigned((total + 3) / 4), 256, 0, stream>>>(reqs_dev, n_req, total, pool->block_table,
+                                                                          pool->max_pages_per_session, pool->log2_page,
+                                                                          pool->stride_page, pool->rope_tab, cs, tok_off);
+    if (cudaGetLastError() != cudaSuccess) return SA_ERR_CUDA;
+    ++pool->last_launches;
+    alignas(64) CUtensorMap ta, tb;
+    if (!make_tmap_2d(&ta, h, total, hidden) || !make_tmap_2d(&tb, w_qkv, N, hidden)) return SA_ERR_CUDA;
+    GemmArgs a{};
+    a.M = total;
+    a.N = N;
+    a.K = hidden;
+    a.m_tiles = int32_t((total + GBM - 1) / GBM);
+    a.n_tiles = (N + GBN - 1) / GBN;
+    a.cs = cs;
+    a.tok_off = tok_off;
+    a.k_base = static_cast<__nv_bfloat16 *>(pool->k_base);
+    a.v_base = static_cast<__nv_bfloat16 *>(pool->v_base);
+    a.q_out = static_cast<__nv_bfloat16 *>(q_out);
+    a.stride_head = pool->stride_head;
+    a.Hq = c.num_q_heads;
+    a.Hkv = c.num_kv_heads;
+    if (launch_gemm<EPI_QKV>(ta, tb, tb, a, stream) != cudaSuccess) return SA_ERR_CUDA;
+    ++pool->last_launches;
+    return SA_OK;
+}
+
+}  // namespace sa
+

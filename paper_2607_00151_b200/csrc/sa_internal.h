@@ -129,6 +129,26 @@ cudaError_t copy_page_async(const sa_kv_pool *pool, int32_t dst_page, int32_t sr
 int32_t acquire_big_meta(sa_kv_pool *pool, size_t bytes, char **host);
 int32_t commit_big_meta(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream);
 
+#ifdef __CUDACC__
+// (cos, sin) of pos * theta_m from the pool's table u = (hi, lo) of theta_m / (2 pi) (reading R9):
+// the position is an exact fp32 integer (< 2^24), the product pos * u is formed error-free, whole
+// turns are dropped and sincospif evaluates the fraction.
+__device__ __forceinline__ float2 rope_cos_sin(int32_t pos, float2 u) {
+    const float p = float(pos);
+    const float ph = p * u.x;
+    float pl = fmaf(p, u.x, -ph);              // exact error of the product
+    pl = fmaf(p, u.y, pl);
+    const float fr = (ph - rintf(ph)) + pl;    // turns, |fr| <= 0.5 (+ tiny)
+    float sn, cs;
+    sincospif(2.0f * fr, &sn, &cs);
+    return make_float2(cs, sn);
+}
+#endif
+
+// Host half of an append: validation, page allocation, metadata upload, block-table update (sa_append.cu).
+int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
+                       bool have_data, cudaStream_t stream, const ReqMeta **reqs_dev_out, int64_t *total_out);
+
 // --- kernel launchers (each returns a cudaError_t from the launch) ---
 cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
                                int64_t total_rows, const void *k, const void *v, void *q,
@@ -147,6 +167,22 @@ cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
 cudaError_t launch_flash_prefill_legacy(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
                                         const AttnPlan &plan, const void *q, void *out, float *lse,
                                         float sm_scale, cudaStream_t stream, int32_t *launches);
+
+// dense operators of the layer (sa_gemm_tc5.cu); each returns an SA_* status
+int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
+                   cudaStream_t stream);
+int32_t gemm_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
+                    cudaStream_t stream);
+int32_t rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, cudaStream_t stream);
+size_t qkv_workspace_bytes(int64_t total);
+int32_t qkv_rope_append_device(sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req, int64_t total, const void *h,
+                               const void *w_qkv, int32_t hidden, void *q_out, void *workspace, cudaStream_t stream);
+// sa_mixed_attention's workspace need for a batch whose q_r tokens are still to be appended (sa_attention.cu)
+int32_t attention_workspace_after_append(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
+                                         const int32_t *qo_indptr, size_t *out_bytes);
+
+// cuTensorMapEncodeTiled resolved through the runtime (no link against libcuda); nullptr if unavailable
+void *tensor_map_encode_fn();
 
 // tcgen05 path (sa_prefill_tc5.cu)
 int32_t tc5_init(sa_kv_pool *pool);  // builds the TMA descriptors; SA_OK or SA_ERR_CUDA

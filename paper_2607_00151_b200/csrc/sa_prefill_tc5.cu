@@ -584,6 +584,8 @@ extern "C" __attribute__((visibility("default"))) int32_t sa_debug_tc5_probe(uns
 }
 #endif
 
+void *tensor_map_encode_fn() { return reinterpret_cast<void *>(get_encode()); }
+
 int32_t tc5_init(sa_kv_pool *pool) {
     pool->tc5_ready = false;
     if (pool->cfg.head_dim != D) return SA_OK;  // head_dim 64 stays on the mma.sync kernel

@@ -145,3 +145,41 @@ def gen_session(w: Workload, idx: int, device="cpu", scale: Optional[float] = No
     v = draw(n_kv, L.num_kv_heads, w.value_scale)
     q = draw(s.new, L.num_q_heads, sc)
     return k, v, q
+
+
+# ---- dense operators of the layer: random-init weights of BASELINE.json's "Llama-3-8B-shaped layer"
+@dataclass
+class LayerShape:
+    hidden: int
+    ffn: int
+    rms_eps: float = 1e-5
+
+
+LLAMA8B_DENSE = LayerShape(4096, 14336)
+
+
+def gen_layer_weights(layer: Layer, shape: LayerShape, seed: int, device="cpu") -> dict:
+    """bf16 tensors, weights [out_features, in_features] ~ N(0,1)/sqrt(in_features), norm gains ~ 1 + 0.1 N(0,1).
+    Draw order: norm1, w_qkv, w_o, norm2, w_gate, w_up, w_down from one torch generator seeded seed*1000003 + 999."""
+    dev = torch.device(device)
+    g = torch.Generator(device=dev)
+    g.manual_seed(seed * 1000003 + 999)
+    H, F, D = shape.hidden, shape.ffn, layer.head_dim
+    QD, NQKV = layer.num_q_heads * D, (layer.num_q_heads + 2 * layer.num_kv_heads) * D
+
+    def mat(n, k):
+        return (torch.randn((n, k), generator=g, device=dev, dtype=torch.float32) * k ** -0.5).to(torch.bfloat16)
+
+    def gain(n):
+        return (1.0 + 0.1 * torch.randn((n,), generator=g, device=dev, dtype=torch.float32)).to(torch.bfloat16)
+
+    return {"norm1": gain(H), "w_qkv": mat(NQKV, H), "w_o": mat(H, QD), "norm2": gain(H), "w_gate": mat(F, H),
+            "w_up": mat(F, H), "w_down": mat(H, F)}
+
+
+def gen_hidden(n_tokens: int, hidden: int, seed: int, device="cpu", scale: float = 1.0):
+    """Hidden states x [n_tokens, hidden] ~ N(0, scale^2), bf16."""
+    dev = torch.device(device)
+    g = torch.Generator(device=dev)
+    g.manual_seed(seed * 1000003 + 555)
+    return (torch.randn((n_tokens, hidden), generator=g, device=dev, dtype=torch.float32) * scale).to(torch.bfloat16)
