@@ -278,6 +278,66 @@ def measure_parts(local: int, peaks, iters: int = 10):
     return decode, app, mixed
 
 
+# --------------------------------------------------------------------------------- whole layer (N3)
+def measure_layer(local: int, peaks, iters: int = 10):
+    """Re-prefill of config 2's segment through sa_layer_forward (RMSNorm, fused QKV+RoPE+append, paged
+    attention, output projection, SwiGLU FFN: PAPER.md L299-303 plus the attention path), Llama-3-8B
+    layer shape (hidden 4096, FFN 14336).  One step = the four 2048-token chunks; tensor roofline over
+    GEMM + causal attention flops."""
+    from paper_2607_00151_b200 import binding as sa
+    from paper_2607_00151_b200.harness import Runner, make_pool
+    w = get_workload(2)
+    L = w.layer
+    H, F = 4096, 14336
+    dev = torch.device("cuda:%d" % local)
+    stream = torch.cuda.current_stream()
+    pool = make_pool(w, local, "random")
+    r = Runner(w, pool, None, local, want_lse=False)
+    r.fill_prefixes()
+    g = torch.Generator(device=dev)
+    g.manual_seed(11)
+    rnd = lambda *s, sc=0.02: (torch.randn(*s, device=dev, generator=g, dtype=torch.float32) * sc).to(torch.bfloat16)
+    nqkv = (L.num_q_heads + 2 * L.num_kv_heads) * L.head_dim
+    lw = sa.LayerWeights(rnd(H, sc=1.0), rnd(nqkv, H), rnd(H, L.num_q_heads * L.head_dim), rnd(H, sc=1.0),
+                         rnd(F, H), rnd(F, H), rnd(H, F), 1e-5)
+    xs = [rnd(int(rd.indptr[-1]), H, sc=1.0) for rd in r.rounds]
+    ys = [torch.empty_like(x) for x in xs]
+    wss = [torch.empty(sa.sa_layer_workspace_bytes(pool, lw, rd.sids, rd.indptr), dtype=torch.uint8, device=dev) for rd in r.rounds]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        r.truncate_to_prefix()
+        n = 0
+        for rd, x, y, ws in zip(r.rounds, xs, ys, wss):
+            sa.sa_layer_forward(pool, lw, rd.sids, rd.indptr, x, y, ws)
+            n += sa.sa_last_launch_count(pool)
+        return n
+    for _ in range(3):
+        launches = step()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(iters):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    ms = float(np.median(ts))
+    tokens = sum(s.new for s in w.sessions)
+    gemm_flops = 2.0 * tokens * H * (nqkv + L.num_q_heads * L.head_dim + 3 * F)
+    attn_flops = 4.0 * L.head_dim * L.num_q_heads * w.pair_count()
+    tf = (gemm_flops + attn_flops) / (ms * 1e-3) / 1e12
+    out = {"workload": "cfg2_summarize through sa_layer_forward, hidden %d ffn %d" % (H, F), "tokens_per_s": tokens / (ms * 1e-3),
+           "ms_per_step": ms, "ms_min": float(min(ts)), "gemm_flops": gemm_flops, "attention_flops": attn_flops,
+           "bound": "tensor", "achieved": tf, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": tf / peaks["bf16_tflops"],
+           "launches_per_step": launches, "note": "whole decoder layer per chunk (7 operators), L2 flushed between steps"}
+    r.close()
+    sa.sa_kv_pool_destroy(pool)
+    return out
+
+
 # --------------------------------------------------------------------------------- our arm
 def run_ours(args, world, rank, local):
     if not torch.cuda.is_available():
@@ -447,6 +507,7 @@ def run_ours(args, world, rank, local):
         line["roofline_decode"] = dec_roof
         line["roofline_append"] = app_roof
         line["mixed_config4"] = mixed
+        line["layer"] = measure_layer(local, peaks)
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_sample(w, 15.0)
@@ -467,7 +528,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parts", action="store_true", help="skip the decode / append bandwidth measurements on config 4")
     ap.add_argument("--parts-only", action="store_true", help="only the decode / append measurements (for profiling them)")
+    ap.add_argument("--layer-only", action="store_true", help="only the whole-layer measurement (for profiling the GEMMs)")
     args = ap.parse_args()
+    if args.layer_only:
+        import __graft_entry__
+        __graft_entry__.build()
+        print(json.dumps({"layer": measure_layer(0, load_peaks(), iters=3)}))
+        return
     if args.impl == "reference":
         world = int(os.environ.get("WORLD_SIZE", "1"))
         rank = int(os.environ.get("RANK", "0"))

@@ -11,7 +11,7 @@ A prefill chunk is a pair (q, prefix): q query tokens over prefix cached tokens 
 request is its cache length L (L305).  A model is a dict
 ``{"c0": ms, "alpha_d": ms per KV token, "alpha_p": ms per causal pair, "gemm": [(M, ms), ...]}``.
 
-Readings (R19/R21-R23):
+Readings (R19 and R25-R28, in this order):
 * Algorithm 1, lines 15-17 lost their text in the PDF extraction: on budget overflow the loop
   BREAKS (as Algorithm 2 does at L374-384, and as the in-order lookahead queue of L168 requires).
 * ``EstPrefillLatency(r)`` (Alg. 1 line 6) = Eq. 1 of the batch holding r's remaining prefill alone.
