@@ -260,24 +260,26 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
         constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
+        // descriptors are built once; an operand at a fixed offset is one 64-bit add away
+        const uint64_t dq0 = umma_desc(sQ, 16, 1024), dk0 = umma_desc(sK, 16, 1024), dv0 = umma_desc(sV, HALF_BYTES, 1024);
         auto issue_qk = [&](int t, int s) {
+            const uint64_t dq = umma_desc_adv(dq0, t * TILE_BYTES), dk = umma_desc_adv(dk0, s * TILE_BYTES);
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
                 const uint32_t off = (ks >> 2) * HALF_BYTES + (ks & 3) * 32;
-                umma_ss(tmem + t * BN, umma_desc(sQ + t * TILE_BYTES + off, 16, 1024),
-                        umma_desc(sK + s * TILE_BYTES + off, 16, 1024), idesc_qk, ks > 0);
+                umma_ss(tmem + t * BN, umma_desc_adv(dq, off), umma_desc_adv(dk, off), idesc_qk, ks > 0);
             }
         };
         auto issue_pv = [&](int t, int s, int ks0, bool acc) {  // 4 k-steps = 64 keys
+            const uint64_t dv = umma_desc_adv(dv0, s * TILE_BYTES);
 #pragma unroll
             for (int ks = ks0; ks < ks0 + 4; ++ks)
-                umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8,
-                        umma_desc(sV + s * TILE_BYTES + ks * 2048, HALF_BYTES, 1024), idesc_pv, acc || ks > ks0);
+                umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8, umma_desc_adv(dv, ks * 2048), idesc_pv, acc || ks > ks0);
         };
         // S_t of the first KV tile of a part; `single`: that tile is also the part's last, so its
         // second QK product is the last reader of the part's Q
         auto issue_first_qk = [&](int t, int s, bool single) {
-            if (lane == 0) {
+            if (elect_one()) {
                 issue_qk(t, s);
                 umma_commit(bar(BAR_S_FULL + t));
                 if (t == 1) {
@@ -285,6 +287,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                     if (single) umma_commit(bar(BAR_Q_EMPTY));
                 }
             }
+            __syncwarp();
         };
         int kc = 0;
         PartGeom gm = load_part<LOG2B>(a, pb);
@@ -320,13 +323,15 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                     // P arrives in two halves so that the first 64 keys' PV runs under the last exponentials
                     mbar_wait(bar(BAR_P_LO + t), kc & 1);
                     tc_fence_after();
-                    if (lane == 0) issue_pv(t, s, 0, j > gm.u0);
+                    if (elect_one()) issue_pv(t, s, 0, j > gm.u0);
+                    __syncwarp();
                     mbar_wait(bar(BAR_P_HI + t), kc & 1);
                     tc_fence_after();
-                    if (lane == 0) {
+                    if (elect_one()) {
                         issue_pv(t, s, 4, true);
                         if (t == 1) umma_commit(bar(BAR_V_EMPTY + s));
                     }
+                    __syncwarp();
                     if (!last) {
                         if (t == 0) {
                             mbar_wait(bar(BAR_K_FULL + sn), phn);
@@ -334,7 +339,8 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                         }
                         issue_first_qk(t, sn, j + 1 == gm.u1 - 1);
                     } else {
-                        if (lane == 0) umma_commit(bar(BAR_O_FULL + t));
+                        if (elect_one()) umma_commit(bar(BAR_O_FULL + t));
+                        __syncwarp();
                         if (has_next_part) {  // keep the tensor pipe fed across the part boundary
                             if (t == 0) {
                                 mbar_wait(bar(BAR_Q_FULL), (p + 1 - pb) & 1);
