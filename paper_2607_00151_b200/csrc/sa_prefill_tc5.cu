@@ -15,7 +15,8 @@
 //               the V rows past the end of the session in an item's last tile
 //   warp 2      TMEM allocator
 //   warps 4-7   softmax of Q tile 0 (thread = row): S from TMEM, mask, lazy-rescaled online
-//   warps 8-11  softmax of Q tile 1   softmax, P (bf16) back into the S columns, epilogue
+//   warps 8-11  softmax of Q tile 1   softmax, P (bf16) back into the S columns in three pieces (64 + 32 + 32
+//               keys, so that only two PV k-steps are left after the last exponential), epilogue
 // TMEM (512 columns): S0/P0 [0,128)  S1/P1 [128,256)  O0 [256,384)  O1 [384,512).
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -74,11 +75,12 @@ enum Bar {
     BAR_V_FULL = 6,   // [2]
     BAR_V_EMPTY = 8,  // [2]
     BAR_S_FULL = 10,  // [2] per Q tile
-    BAR_P_LO = 12,    // [2] P columns of keys 0..63 of the tile are in TMEM
-    BAR_P_HI = 14,    // [2] ... keys 64..127
-    BAR_O_FULL = 16,  // [2] all PV products of the part have landed in O_t
-    BAR_O_EMPTY = 18, // [2] the epilogue has read O_t out of TMEM
-    BAR_COUNT = 20
+    BAR_P_A = 12,     // [2] P columns of keys 0..63 of the tile are in TMEM
+    BAR_P_B = 14,     // [2] ... keys 64..95
+    BAR_P_C = 16,     // [2] ... keys 96..127
+    BAR_O_FULL = 18,  // [2] all PV products of the part have landed in O_t
+    BAR_O_EMPTY = 20, // [2] the epilogue has read O_t out of TMEM
+    BAR_COUNT = 22
 };
 
 // Everything a role needs to know about one part; every role derives the same values.
@@ -118,11 +120,16 @@ __device__ __forceinline__ void chunk_mask(uint32_t (&s)[32], int key0, int lim)
     for (int i = 0; i < 32; ++i)
         if (key0 + i > lim) s[i] = 0xff800000u;  // -inf: selected, never added
 }
+__device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }  // one FMNMX3
+// max of the 32 columns of a chunk as a tree of depth 4 (a serial chain would expose the FMNMX3 latency 16 times)
 __device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
-    float m = __uint_as_float(s[0]);
+    float l1[10];
 #pragma unroll
-    for (int i = 1; i < 31; i += 2) m = fmaxf(fmaxf(m, __uint_as_float(s[i])), __uint_as_float(s[i + 1]));
-    return fmaxf(m, __uint_as_float(s[31]));
+    for (int i = 0; i < 10; ++i)
+        l1[i] = max3(__uint_as_float(s[3 * i]), __uint_as_float(s[3 * i + 1]), __uint_as_float(s[3 * i + 2]));
+    const float a0 = max3(l1[0], l1[1], l1[2]), a1 = max3(l1[3], l1[4], l1[5]), a2 = max3(l1[6], l1[7], l1[8]);
+    const float a3 = max3(l1[9], __uint_as_float(s[30]), __uint_as_float(s[31]));
+    return fmaxf(max3(a0, a1, a2), a3);
 }
 // exp2 of one chunk, row sums, bf16 P into 16 TMEM columns.  SA_POLY_SHARE of every four column
 // pairs take the packed cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
@@ -188,8 +195,9 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             mbar_init(bar(BAR_V_FULL + s), 1);
             mbar_init(bar(BAR_V_EMPTY + s), 1);
             mbar_init(bar(BAR_S_FULL + s), 1);
-            mbar_init(bar(BAR_P_LO + s), BM);
-            mbar_init(bar(BAR_P_HI + s), BM);
+            mbar_init(bar(BAR_P_A + s), BM);
+            mbar_init(bar(BAR_P_B + s), BM);
+            mbar_init(bar(BAR_P_C + s), BM);
             mbar_init(bar(BAR_O_FULL + s), 1);
             mbar_init(bar(BAR_O_EMPTY + s), BM);
         }
@@ -270,10 +278,10 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 umma_ss(tmem + t * BN, umma_desc_adv(dq, off), umma_desc_adv(dk, off), idesc_qk, ks > 0);
             }
         };
-        auto issue_pv = [&](int t, int s, int ks0, bool acc) {  // 4 k-steps = 64 keys
+        auto issue_pv = [&](int t, int s, int ks0, int nks, bool acc) {  // nks k-steps of 16 keys from k-step ks0
             const uint64_t dv = umma_desc_adv(dv0, s * TILE_BYTES);
 #pragma unroll
-            for (int ks = ks0; ks < ks0 + 4; ++ks)
+            for (int ks = ks0; ks < ks0 + nks; ++ks)
                 umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8, umma_desc_adv(dv, ks * 2048), idesc_pv, acc || ks > ks0);
         };
         // S_t of the first KV tile of a part; `single`: that tile is also the part's last, so its
@@ -320,15 +328,20 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 for (int t = 0; t < 2; ++t) {
                     // the first PV product of a part overwrites O_t: the previous part's epilogue must have read it
                     if (j == gm.u0 && p > pb) mbar_wait(bar(BAR_O_EMPTY + t), (p - pb - 1) & 1);
-                    // P arrives in two halves so that the first 64 keys' PV runs under the last exponentials
-                    mbar_wait(bar(BAR_P_LO + t), kc & 1);
+                    // P arrives in three pieces (64 + 32 + 32 keys): the products of the first 96 keys run under
+                    // the remaining exponentials and only two k-steps are left after the last one
+                    mbar_wait(bar(BAR_P_A + t), kc & 1);
                     tc_fence_after();
-                    if (elect_one()) issue_pv(t, s, 0, j > gm.u0);
+                    if (elect_one()) issue_pv(t, s, 0, 4, j > gm.u0);
                     __syncwarp();
-                    mbar_wait(bar(BAR_P_HI + t), kc & 1);
+                    mbar_wait(bar(BAR_P_B + t), kc & 1);
+                    tc_fence_after();
+                    if (elect_one()) issue_pv(t, s, 4, 2, true);
+                    __syncwarp();
+                    mbar_wait(bar(BAR_P_C + t), kc & 1);
                     tc_fence_after();
                     if (elect_one()) {
-                        issue_pv(t, s, 4, true);
+                        issue_pv(t, s, 6, 2, true);
                         if (t == 1) umma_commit(bar(BAR_V_EMPTY + s));
                     }
                     __syncwarp();
@@ -421,20 +434,23 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 if (masked) {
                     chunk_exp_store<true>(s0, sl2_2, neg_2, lsum, tS);
                     chunk_exp_store<true>(s1, sl2_2, neg_2, lsum, tS + 16);
-                    chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
                 } else {
                     chunk_exp_store<false>(s0, sl2_2, neg_2, lsum, tS);
                     chunk_exp_store<false>(s1, sl2_2, neg_2, lsum, tS + 16);
-                    chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
                 }
-                tmem_wait_st();  // chunks 0..2 are in TMEM (the wait costs nothing: chunk 2's math ran meanwhile)
+                tmem_wait_st();
                 tc_fence_before();
-                mbar_arrive(bar(BAR_P_LO + t));
+                mbar_arrive(bar(BAR_P_A + t));
+                if (masked) chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
+                else chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(bar(BAR_P_B + t));
                 if (masked) chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
                 else chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
                 tmem_wait_st();
                 tc_fence_before();
-                mbar_arrive(bar(BAR_P_HI + t));
+                mbar_arrive(bar(BAR_P_C + t));
             }
             float l;
             {
