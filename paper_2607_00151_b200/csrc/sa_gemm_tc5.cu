@@ -156,6 +156,7 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
         constexpr uint32_t idesc = umma_idesc_bf16(GBM, GBN, false, false);
+        const uint64_t dA0 = umma_desc(s0, 16, 1024), dB0 = umma_desc(s0 + A_STAGE, 16, 1024);
         int kc = 0, tc = 0;
         for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x, ++tc) {
             const int b = tc & 1;
@@ -165,12 +166,11 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
                 const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
                 mbar_wait(bar_full(s), ph);
                 tc_fence_after();
-                if (lane == 0) {
-                    const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
+                if (elect_one()) {  // one lane, known to the compiler: the four tcgen05.mma go out back to back
+                    const uint64_t dA = umma_desc_adv(dA0, s * STAGE_BYTES), dB = umma_desc_adv(dB0, s * STAGE_BYTES);
 #pragma unroll
                     for (int kk = 0; kk < GBK / 16; ++kk)
-                        umma_ss(tmem + b * GBN, umma_desc(sA + kk * 32, 16, 1024), umma_desc(sB + kk * 32, 16, 1024), idesc,
-                                ks > 0 || kk > 0);
+                        umma_ss(tmem + b * GBN, umma_desc_adv(dA, kk * 32), umma_desc_adv(dB, kk * 32), idesc, ks > 0 || kk > 0);
                     umma_commit(bar_empty(s));
                     if (ks == k_steps - 1) umma_commit(bar_acc_full(b));
                 }
