@@ -366,6 +366,29 @@ SA_API int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_heads, i
                       const int32_t *m_list, int32_t n_m, int32_t warmup, int32_t iters, float *out_ms,
                       void *stream);
 
+/* ---- KV hand-over between pools ----------------------------------------------------
+ * in PD-disaggregated serving "KV transfer" moves a request's cache from the prefill
+ * instance to the decode instance (L456: 4 prefill + 4 decode GPUs); L424: tensor parallelism shards
+ * the kv heads over GPUs.  A session's tokens travel as a WIRE IMAGE: dense bf16
+ *     image[c][h][t][d],  c in {0: K' (rotated, as stored), 1: V},  h < Hkv,  t < n_tokens,  d < D,
+ * so the image of one kv head is contiguous and a head-sharded receiver imports its own heads only.
+ * `image` is a DEVICE pointer, 16-byte aligned: local memory, or a peer GPU's memory mapped into this
+ * process (NVLink P2P), which makes export a direct remote write and import a direct remote read.
+ * Both calls enqueue one gather / scatter kernel on `stream` and never synchronise.  The bits of K', V
+ * are copied unchanged; positions are implicit (token t of the image is session token tok_begin + t on
+ * export and session_len + t on import), so a receiver must import a session's images in order. */
+SA_API int32_t sa_kv_wire_bytes(const sa_kv_pool *pool, int64_t n_tokens, size_t *out_bytes);
+/* Tokens [tok_begin, tok_begin + n_tokens) of session `sid` -> image.  The session is not changed.
+ * SA_ERR_INVALID_ARG if the range is not inside the session, SA_ERR_WORKSPACE_TOO_SMALL if
+ * image_bytes < sa_kv_wire_bytes(n_tokens). */
+SA_API int32_t sa_kv_session_export(sa_kv_pool *pool, int32_t sid, int64_t tok_begin, int64_t n_tokens, void *image,
+                             size_t image_bytes, void *stream);
+/* Appends n_tokens tokens to session `sid` from an image that holds `src_heads` kv heads, taking heads
+ * [head_begin, head_begin + pool's Hkv).  Page allocation, copy-on-write of a shared partial page and
+ * failure behaviour are sa_rope_kv_append's (SA_ERR_OUT_OF_PAGES changes nothing); nothing is rotated. */
+SA_API int32_t sa_kv_session_import(sa_kv_pool *pool, int32_t sid, int64_t n_tokens, const void *image, int32_t src_heads,
+                             int32_t head_begin, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -18,6 +18,9 @@ Entry points:
   re-prefill of a segment over an already rotated, stored prefix
                                                      PAPER.md L311-313, L186-187
 Decode row = ``oracle_cached`` with a one-token segment
+* ``wire_image(k_rot, v, head_begin, head_count)``   the KV hand-over image (N4;
+  PAPER.md L426 "KV transfer", L424 tensor parallelism): a pure re-indexing of
+  the stored cache, image[c][h][t][d] = (K' if c == 0 else V)[t][head_begin+h][d]
 
 Parity pins live in tests/test_oracle_pins.py.  Absolute output values are
 otherwise unpinned (the paper prints no tensor).
@@ -175,3 +178,23 @@ def oracle_cached(k_rot_prefix, v_prefix, q_seg, k_seg, v_seg, P: int, base: flo
     res["k_rot_seg"] = k_rot_seg
     res["q_rot"] = q_rot
     return res
+
+
+def wire_image(k_rot, v, head_begin: int = 0, head_count: Optional[int] = None) -> np.ndarray:
+    """Hand-over image of a cached token range (N4; PAPER.md L426 / L424).
+
+    k_rot, v: [n, Hkv, D], the rotated keys and the values as the cache stores them.  Returns
+    image[2][head_count][n][D] with image[0][h][t][d] = k_rot[t][head_begin + h][d] and
+    image[1][h][t][d] = v[t][head_begin + h][d]: no arithmetic, only the index order (written as
+    explicit loops over c and h so that it can be checked against that sentence by eye)."""
+    k_rot = np.asarray(k_rot)
+    v = np.asarray(v)
+    n, hkv, d = k_rot.shape
+    if head_count is None:
+        head_count = hkv - head_begin
+    img = np.empty((2, head_count, n, d), dtype=k_rot.dtype)
+    for h in range(head_count):
+        for t in range(n):
+            img[0, h, t, :] = k_rot[t, head_begin + h, :]
+            img[1, h, t, :] = v[t, head_begin + h, :]
+    return img

@@ -135,6 +135,9 @@ PROTOTYPES = {
                                           ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
     "sa_gemm_table": (ctypes.c_int32, [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p,
                                        ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _f32p, _vp]),
+    "sa_kv_wire_bytes": (ctypes.c_int32, [_vp, ctypes.c_int64, ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_kv_session_export": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, _vp, ctypes.c_size_t, _vp]),
+    "sa_kv_session_import": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, _vp, ctypes.c_int32, ctypes.c_int32, _vp]),
 }
 
 _lib = None
@@ -475,6 +478,26 @@ def sa_dynamic_chunk(model: LatencyModel, decode_L, chunks, prefix: int, remaini
                                            int(remaining), int(max_chunk), int(granularity), float(budget_ms), ctypes.byref(out)),
            "sa_dynamic_chunk")
     return int(out.value)
+
+
+# ---------------------------------------------------------------- KV hand-over between pools (N4)
+def sa_kv_wire_bytes(pool: Pool, n_tokens: int) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_kv_wire_bytes(pool.handle, n_tokens, ctypes.byref(out)), "sa_kv_wire_bytes")
+    return int(out.value)
+
+
+def sa_kv_session_export(pool: Pool, sid: int, tok_begin: int, n_tokens: int, image, stream=None) -> None:
+    """image: device bf16 tensor with >= 2*Hkv*n_tokens*D elements (local or peer-mapped)."""
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_kv_session_export(pool.handle, sid, tok_begin, n_tokens, _ptr(image), _nbytes(image), sp),
+           "sa_kv_session_export")
+
+
+def sa_kv_session_import(pool: Pool, sid: int, n_tokens: int, image, src_heads: int, head_begin: int = 0, stream=None) -> None:
+    sp = None if pool.storage is None else _stream_ptr(stream)
+    _check(load_library().sa_kv_session_import(pool.handle, sid, n_tokens, _ptr(image), src_heads, head_begin, sp),
+           "sa_kv_session_import")
 
 
 # ---------------------------------------------------------------- dense operators of the layer (N3)

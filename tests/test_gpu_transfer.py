@@ -1,0 +1,184 @@
+"""GPU tests of the KV hand-over between pools ("KV transfer" between
+prefill and decode instances, L424 tensor parallelism): a session leaves one pool as a wire image
+[2][Hkv][n][D] and enters another pool -- with another page size, another page order, or only a
+slice of the kv heads -- from it.  The image is compared with the oracle's re-indexing of the
+logical cache (V bit for bit, K' within the RoPE gate), and everything downstream bit for bit
+with the session it came from."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2607_00151_b200 import binding as sa
+from paper_2607_00151_b200.harness import gather_kv, pool_views
+from paper_2607_00151_b200.workloads import Layer
+
+pytestmark = pytest.mark.gpu
+
+SENT = 0x7FC1
+
+
+def _bits(t):
+    return t.contiguous().view(torch.int16)
+
+
+def _mk_pool(L: Layer, num_pages, max_tokens, seed, sentinel=SENT):
+    cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, num_pages, 8, max_tokens, L.rope_base, 0)
+    nbytes = sa.sa_kv_pool_storage_bytes(cfg)
+    storage = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    storage.view(torch.int16)[: nbytes // 2].fill_(np.array(sentinel, dtype=np.uint16).view(np.int16).item())
+    order = np.random.default_rng(seed).permutation(num_pages).astype(np.int32)
+    return sa.sa_kv_pool_create(cfg, storage, order)
+
+
+def _rand(n, h, d, gen, scale):
+    return (torch.randn((n, h, d), generator=gen, device="cuda", dtype=torch.float32) * scale).to(torch.bfloat16)
+
+
+def _attend(pool, sid, q_rot):
+    n = q_rot.shape[0]
+    out = torch.empty_like(q_rot)
+    lse = torch.empty((n, q_rot.shape[1]), dtype=torch.float32, device="cuda")
+    ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(pool, [sid], [0, n]), 256), dtype=torch.uint8, device="cuda")
+    sa.sa_mixed_attention(pool, [sid], [0, n], q_rot, out, lse, 0.0, ws)
+    torch.cuda.synchronize()
+    return out, lse
+
+
+def _source(L: Layer, n, seed, scale):
+    """A pool with one session of n cached tokens; returns (pool, sid, k_raw, v_raw)."""
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(seed)
+    pages = (n + L.page_size - 1) // L.page_size + 3
+    pool = _mk_pool(L, pages, n + 2 * L.page_size, seed + 1)
+    sid = sa.sa_kv_session_open(pool)
+    k, v = _rand(n, L.num_kv_heads, L.head_dim, gen, scale), _rand(n, L.num_kv_heads, L.head_dim, gen, scale)
+    sa.sa_rope_kv_append(pool, [sid], [0, n], k, v, None)
+    torch.cuda.synchronize()
+    return pool, sid, k, v
+
+
+def _export(pool, sid, t0, n):
+    L = pool.cfg
+    img = torch.full((2, L.num_kv_heads, n, L.head_dim), float("nan"), dtype=torch.bfloat16, device="cuda")
+    assert sa.sa_kv_wire_bytes(pool, n) == img.numel() * 2
+    sa.sa_kv_session_export(pool, sid, t0, n, img)
+    torch.cuda.synchronize()
+    return img
+
+
+@pytest.mark.parametrize("shape", ["llama", "tiny"])
+def test_export_image_matches_the_oracle_reindexing(shape):
+    L, n, scale = (Layer(32, 8, 128, 64, 500000.0), 333, 128 ** -0.5) if shape == "llama" else (Layer(8, 2, 64, 16, 10000.0), 77, 1.0)
+    pool, sid, k, v = _source(L, n, 11, scale)
+    t0, m = 5, n - 9  # a range that starts and ends inside pages
+    img = _export(pool, sid, t0, m)
+    k_rot = orc.rope(k.cpu(), np.arange(n), L.rope_base)       # fp64 K' of the logical cache
+    ref = orc.wire_image(k_rot[t0:t0 + m], orc.widen(v.cpu())[t0:t0 + m])
+    got = img.double().cpu().numpy()
+    assert np.array_equal(got[1], ref[1]), "V part of the image must be a bit copy"
+    # RoPE gate of BASELINE.json (1e-2) where a correctly rounded bf16 can meet it, one bf16 ulp elsewhere (DESIGN.md T-B)
+    assert (np.abs(got[0] - ref[0]) <= np.maximum(1e-2, 2.0 ** -7 * np.abs(ref[0]))).all()
+    # and the K' part is exactly what the pool stores (the hand-over rounds nothing again)
+    length, page_ids = sa.sa_kv_session_query(pool, sid)
+    ks, vs = gather_kv(pool, list(page_ids), length)
+    assert torch.equal(_bits(img[0]), _bits(ks[t0:t0 + m].permute(1, 0, 2)))
+    assert torch.equal(_bits(img[1]), _bits(vs[t0:t0 + m].permute(1, 0, 2)))
+    sa.sa_kv_pool_destroy(pool)
+
+
+def test_roundtrip_into_other_page_size_and_order_is_bit_exact():
+    L = Layer(32, 8, 128, 64, 500000.0)
+    n = 700
+    pool, sid, k, v = _source(L, n, 21, 128 ** -0.5)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    q = _rand(200, L.num_q_heads, L.head_dim, gen, 128 ** -0.5)
+    # the last 200 cached tokens double as the queries' own positions: a re-prefill chunk over the handed-over cache
+    o_src, lse_src = _attend(pool, sid, q)
+    for B2, seed in ((64, 3), (16, 4)):
+        L2 = Layer(L.num_q_heads, L.num_kv_heads, L.head_dim, B2, L.rope_base)
+        dst = _mk_pool(L2, (n + B2 - 1) // B2 + 5, n + 128, seed)
+        sid2 = sa.sa_kv_session_open(dst)
+        free0 = sa.sa_kv_pool_free_pages(dst)
+        # in order, in three uneven pieces that do not end on page boundaries
+        for t0, m in ((0, 100), (100, 233), (333, n - 333)):
+            sa.sa_kv_session_import(dst, sid2, m, _export(pool, sid, t0, m), L.num_kv_heads, 0)
+        torch.cuda.synchronize()
+        length, page_ids = sa.sa_kv_session_query(dst, sid2)
+        assert length == n and sa.sa_kv_pool_free_pages(dst) == free0 - (n + B2 - 1) // B2
+        k2, v2 = gather_kv(dst, list(page_ids), n)
+        ls, ps = sa.sa_kv_session_query(pool, sid)
+        k1, v1 = gather_kv(pool, list(ps), n)
+        assert torch.equal(_bits(k1), _bits(k2)) and torch.equal(_bits(v1), _bits(v2))
+        # slots the session does not own keep the sentinel (last page's tail and every unused page)
+        kp, vp = pool_views(dst)
+        used = set(int(p) for p in page_ids)
+        for pg in range(dst.cfg.num_pages):
+            lo = 0 if pg not in used else (n % B2 if pg == int(page_ids[-1]) and n % B2 else B2)
+            if lo < B2:
+                assert (_bits(kp[pg, :, lo:, :]) == np.array(SENT, dtype=np.uint16).view(np.int16).item()).all()
+                assert (_bits(vp[pg, :, lo:, :]) == np.array(SENT, dtype=np.uint16).view(np.int16).item()).all()
+        o2, lse2 = _attend(dst, sid2, q)
+        if B2 == L.page_size:
+            assert torch.equal(_bits(o_src), _bits(o2)) and torch.equal(lse_src, lse2)
+        else:  # another page size: same logical tiles, the bits still agree (tiles are 128 logical keys)
+            assert torch.equal(_bits(o_src), _bits(o2))
+        sa.sa_kv_pool_destroy(dst)
+    sa.sa_kv_pool_destroy(pool)
+
+
+def test_head_sharded_receivers_reproduce_the_unsharded_attention():
+    """Tensor-parallel receivers: rank r of 2 holds kv heads [4r, 4r+4) and q heads [16r, 16r+16)."""
+    L = Layer(32, 8, 128, 64, 500000.0)
+    n = 515
+    pool, sid, k, v = _source(L, n, 31, 128 ** -0.5)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(6)
+    q = _rand(130, L.num_q_heads, L.head_dim, gen, 128 ** -0.5)
+    o_full, lse_full = _attend(pool, sid, q)
+    img = _export(pool, sid, 0, n)
+    world = 2
+    Ls = Layer(L.num_q_heads // world, L.num_kv_heads // world, L.head_dim, L.page_size, L.rope_base)
+    outs, lses = [], []
+    for r in range(world):
+        shard = _mk_pool(Ls, n // 64 + 4, n + 64, 40 + r)
+        s2 = sa.sa_kv_session_open(shard)
+        sa.sa_kv_session_import(shard, s2, n, img, L.num_kv_heads, r * Ls.num_kv_heads)
+        qs = q[:, r * Ls.num_q_heads:(r + 1) * Ls.num_q_heads].contiguous()
+        o, l = _attend(shard, s2, qs)
+        outs.append(o)
+        lses.append(l)
+        # the oracle's head slice of the image is what this rank stored
+        length, page_ids = sa.sa_kv_session_query(shard, s2)
+        ks, vs = gather_kv(shard, list(page_ids), n)
+        ref_v = orc.wire_image(orc.widen(k.cpu()), orc.widen(v.cpu()), r * Ls.num_kv_heads, Ls.num_kv_heads)[1]
+        assert np.array_equal(vs.permute(1, 0, 2).double().cpu().numpy(), ref_v)
+        sa.sa_kv_pool_destroy(shard)
+    assert torch.equal(_bits(torch.cat(outs, dim=1)), _bits(o_full))
+    assert torch.equal(torch.cat(lses, dim=1), lse_full)
+    sa.sa_kv_pool_destroy(pool)
+
+
+def test_errors_change_nothing():
+    L = Layer(8, 2, 64, 16, 10000.0)
+    pool, sid, k, v = _source(L, 40, 51, 1.0)
+    img = torch.zeros((2, 2, 40, 64), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_export(pool, sid, 10, 31, img)               # range leaves the session
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_export(pool, sid, 0, 40, img.view(-1)[: 2 * 2 * 39 * 64])  # image too small
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_export(pool, sid, 0, 8, img.view(-1)[4:])    # not 16-byte aligned
+    with pytest.raises(sa.SAError):
+        sa.sa_kv_session_import(pool, sid, 8, img, 2, 1)              # head slice leaves the image
+    free0 = sa.sa_kv_pool_free_pages(pool)
+    big = torch.zeros((2, 2, 16 * (free0 + 2), 64), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(sa.SAError) as ei:
+        sa.sa_kv_session_import(pool, sid, big.shape[2], big, 2, 0)
+    assert ei.value.status in (sa.SA_ERR_OUT_OF_PAGES, sa.SA_ERR_INVALID_ARG)
+    assert sa.sa_kv_pool_free_pages(pool) == free0 and sa.sa_kv_session_query(pool, sid)[0] == 40
+    sa.sa_kv_session_export(pool, sid, 0, 0, img)                     # empty range: legal, no launch
+    sa.sa_kv_session_import(pool, sid, 0, img, 2, 0)
+    assert sa.sa_kv_session_query(pool, sid)[0] == 40
+    sa.sa_kv_pool_destroy(pool)

@@ -311,3 +311,24 @@ def test_widen_bf16_is_exact():
     w = orc.widen(t)
     assert w.dtype == np.float64
     assert np.array_equal(w.astype(np.float32), t.float().numpy())
+
+
+def test_wire_image_is_the_stated_reindexing():
+    """N4 hand-over image (PAPER.md L426 / L424): image[c][h][t][d] = (K', V)[c][t][head_begin + h][d].
+    Hand-written tiny case, the library transpose, and the head slice of a sharded receiver."""
+    # n = 2 tokens, Hkv = 2, D = 2; entries encode (tensor, token, head, dim) so a wrong index order shows
+    k = np.array([[[100, 101], [110, 111]], [[200, 201], [210, 211]]], dtype=np.float64)        # [t][h][d]
+    v = -k
+    img = orc.wire_image(k, v)
+    expect_k = [[[100, 101], [200, 201]], [[110, 111], [210, 211]]]                                # [h][t][d]
+    assert img.shape == (2, 2, 2, 2)
+    assert img[0].tolist() == expect_k and img[1].tolist() == (-np.array(expect_k)).tolist()
+    rng = np.random.default_rng(0)
+    k, v = rng.standard_normal((7, 4, 6)), rng.standard_normal((7, 4, 6))
+    img = orc.wire_image(k, v)
+    assert np.array_equal(img[0], np.transpose(k, (1, 0, 2))) and np.array_equal(img[1], np.transpose(v, (1, 0, 2)))
+    part = orc.wire_image(k, v, head_begin=1, head_count=2)
+    assert np.array_equal(part, img[:, 1:3])
+    # concatenating token ranges of images = image of the concatenation (in-order import)
+    a, b = orc.wire_image(k[:3], v[:3]), orc.wire_image(k[3:], v[3:])
+    assert np.array_equal(np.concatenate([a, b], axis=2), img)

@@ -259,3 +259,34 @@ def test_commit_swaps_block_tables_and_releases_superseded_pages():
     assert all(sa.sa_kv_page_refcount(p, x) == 0 for x in pg_main[3:])
     with pytest.raises(sa.SAError):
         sa.sa_kv_session_commit(p, main, main)
+
+
+def test_import_books_pages_like_an_append_and_validates_the_head_slice():
+    """N4 (PAPER.md L426 KV transfer, L424 head sharding): the host half of sa_kv_session_import on a
+    host-only pool: same page arithmetic as an append, copy-on-write of a shared partial page, all-or-nothing."""
+    order = np.random.default_rng(1).permutation(32).astype(np.int32)
+    p = _pool(num_pages=32, order=order, Hkv=2)
+    assert sa.sa_kv_wire_bytes(p, 10) == 2 * 2 * 10 * 64 * 2 and sa.sa_kv_wire_bytes(p, 0) == 0
+    s = sa.sa_kv_session_open(p)
+    sa.sa_kv_session_import(p, s, 40, None, 8, 6)          # heads [6, 8) of an 8-head image: legal
+    assert sa.sa_kv_session_query(p, s) == (40, order[:3].tolist())
+    sa.sa_kv_session_import(p, s, 9, None, 2, 0)           # crosses into a 4th page
+    assert sa.sa_kv_session_query(p, s) == (49, order[:4].tolist())
+    for src_heads, head_begin in ((8, 7), (1, 0), (2, -1), (0, 0)):
+        with pytest.raises(sa.SAError) as ei:
+            sa.sa_kv_session_import(p, s, 4, None, src_heads, head_begin)
+        assert ei.value.status == sa.SA_ERR_INVALID_ARG
+    free0 = sa.sa_kv_pool_free_pages(p)
+    with pytest.raises(sa.SAError) as ei:
+        sa.sa_kv_session_import(p, s, 16 * free0 + 16, None, 2, 0)
+    assert ei.value.status in (sa.SA_ERR_OUT_OF_PAGES, sa.SA_ERR_INVALID_ARG)
+    assert sa.sa_kv_pool_free_pages(p) == free0 and sa.sa_kv_session_query(p, s)[0] == 49
+    # a fork holds its own copy of the partial 4th page: importing into the fork leaves the source session's page alone
+    f = sa.sa_kv_session_fork(p, s, 49)
+    shared = sa.sa_kv_session_query(p, s)[1][3]
+    sa.sa_kv_session_import(p, f, 3, None, 2, 0)
+    assert sa.sa_kv_session_query(p, f)[0] == 52 and sa.sa_kv_session_query(p, s)[1][3] == shared
+    # export on a host-only pool: argument checks run, the copy itself needs a device
+    with pytest.raises(sa.SAError) as ei:
+        sa.sa_kv_session_export(p, s, 40, 10, None)
+    assert ei.value.status == sa.SA_ERR_INVALID_ARG
