@@ -273,9 +273,40 @@ def measure_parts(local: int, peaks, iters: int = 10):
     flops = 4.0 * L.head_dim * L.num_q_heads * w.pair_count()
     mixed = {"ms": ms_mix, "prefill_tflops_if_alone": flops / (ms_mix * 1e-3) / 1e12, "prefill_flops": flops,
              "decode_bytes": dec_bytes, "note": "config 4 mixed lookahead batch: one sa_mixed_attention call"}
+    # ---- KV hand-over (N4): every session's cached tokens out as wire images, and into a second pool
+    lens = [sa.sa_kv_session_query(pool, sid)[0] for sid in r.sids]
+    imgs = [torch.empty((2, L.num_kv_heads, n, L.head_dim), dtype=torch.bfloat16, device=dev) for n in lens]
+    pool2 = make_pool(w, local, "identity")
+    sids2 = [sa.sa_kv_session_open(pool2) for _ in lens]
+
+    def run_export():
+        for sid, n, im in zip(r.sids, lens, imgs):
+            sa.sa_kv_session_export(pool, sid, 0, n, im)
+
+    def run_import():
+        for sid in sids2:
+            sa.sa_kv_session_truncate(pool2, sid, 0)
+        for sid, n, im in zip(sids2, lens, imgs):
+            sa.sa_kv_session_import(pool2, sid, n, im, L.num_kv_heads, 0)
+    run_export()
+    run_import()
+    torch.cuda.synchronize()
+    ms_ex, _ = timed(run_export, max(3, iters // 2))
+    ms_im, _ = timed(run_import, max(3, iters // 2))
+    xbytes = 2.0 * kappa * sum(lens)
+    transfer = {"bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "tokens": int(sum(lens)), "sessions": len(lens),
+                "export_ms": ms_ex, "export_gbs": xbytes / (ms_ex * 1e-3) / 1e9, "import_ms": ms_im,
+                "import_gbs": xbytes / (ms_im * 1e-3) / 1e9, "bytes_per_pass": xbytes,
+                "note": "config 4's 68 sessions, one sa_kv_session_export / sa_kv_session_import call per session "
+                        "(read kappa + write kappa per token; import includes page allocation and block-table update)"}
+    transfer["frac"] = min(transfer["export_gbs"], transfer["import_gbs"]) / peaks["hbm_gbs"]
+    for sid in sids2:
+        sa.sa_kv_session_close(pool2, sid)
+    sa.sa_kv_pool_destroy(pool2)
+    del imgs
     r.close()
     sa.sa_kv_pool_destroy(pool)
-    return decode, app, mixed
+    return decode, app, mixed, transfer
 
 
 # --------------------------------------------------------------------------------- whole layer (N3)
@@ -503,10 +534,11 @@ def run_ours(args, world, rank, local):
         sa.sa_kv_pool_destroy(pool)
         del r, pool, flush
         torch.cuda.empty_cache()
-        dec_roof, app_roof, mixed = measure_parts(local, peaks)
+        dec_roof, app_roof, mixed, xfer = measure_parts(local, peaks)
         line["roofline_decode"] = dec_roof
         line["roofline_append"] = app_roof
         line["mixed_config4"] = mixed
+        line["transfer_config4"] = xfer
         line["layer"] = measure_layer(local, peaks)
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
@@ -543,8 +575,8 @@ def main():
     if args.parts_only:
         import __graft_entry__
         __graft_entry__.build()
-        dec, app, mixed = measure_parts(0, load_peaks(), iters=3)
-        print(json.dumps({"roofline_decode": dec, "roofline_append": app, "mixed_config4": mixed}))
+        dec, app, mixed, xfer = measure_parts(0, load_peaks(), iters=3)
+        print(json.dumps({"roofline_decode": dec, "roofline_append": app, "mixed_config4": mixed, "transfer_config4": xfer}))
         return
     world, rank, local = dist_setup(args.gpus)
     run_ours(args, world, rank, local)
