@@ -313,6 +313,19 @@ SA_API int32_t sa_linear(const void *x, const void *w, const void *residual, voi
 SA_API int32_t sa_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F,
                   int32_t K, void *stream);
 
+/* The same two operators with a scratch buffer.  With few rows (decode batches: the "near-constant latency"
+ * regime of L301) the 128 x 256 tiles alone are too few to keep every SM streaming weights, so the K loop of a
+ * tile is cut into slices that run on different SMs (split-K); fp32 partials go through `workspace` and a second
+ * kernel sums them IN SLICE ORDER and applies the epilogue, so the result is bit-reproducible run to run (it may
+ * differ in the last bit from the unsplit call: another summation order).  *_workspace_bytes returns 0 when the
+ * shape will not be split; a null or too small workspace falls back to the unsplit kernel, never to an error. */
+SA_API int32_t sa_linear_workspace_bytes(int64_t M, int32_t N, int32_t K, size_t *out_bytes);
+SA_API int32_t sa_linear_ws(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
+                     void *workspace, size_t workspace_bytes, void *stream);
+SA_API int32_t sa_swiglu_workspace_bytes(int64_t M, int32_t F, int32_t K, size_t *out_bytes);
+SA_API int32_t sa_swiglu_ws(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
+                     void *workspace, size_t workspace_bytes, void *stream);
+
 /* y[M, H] = x / sqrt(mean_j x_j^2 + eps) * w  (fp32 arithmetic, one rounding). */
 SA_API int32_t sa_rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, void *stream);
 
@@ -323,7 +336,8 @@ SA_API int32_t sa_rmsnorm(const void *x, const void *w, float eps, void *y, int6
  *   h      : device bf16 [T, hidden]  (the normalised hidden states of the batch's new tokens)
  *   w_qkv  : device bf16 [(Hq + 2 Hkv) * D, hidden]
  *   q_out  : device bf16 [T, Hq, D], rotated queries for sa_mixed_attention
- *   workspace : device, >= sa_qkv_rope_append_workspace_bytes(T) (per-token cos/sin and slot table)
+ *   workspace : device, >= sa_qkv_rope_append_workspace_bytes(T) (per-token cos/sin and slot table, plus the
+ *               split-K scratch of a small batch)
  * Only head_dim 128 (SA_ERR_UNSUPPORTED otherwise). */
 SA_API int32_t sa_qkv_rope_append_workspace_bytes(const sa_kv_pool *pool, int64_t total_tokens, size_t *out_bytes);
 SA_API int32_t sa_qkv_rope_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,

@@ -135,6 +135,10 @@ PROTOTYPES = {
                                           ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
     "sa_gemm_table": (ctypes.c_int32, [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p,
                                        ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _f32p, _vp]),
+    "sa_linear_workspace_bytes": (ctypes.c_int32, [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_linear_ws": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp, ctypes.c_size_t, _vp]),
+    "sa_swiglu_workspace_bytes": (ctypes.c_int32, [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_swiglu_ws": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp, ctypes.c_size_t, _vp]),
     "sa_kv_wire_bytes": (ctypes.c_int32, [_vp, ctypes.c_int64, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_kv_session_export": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, _vp, ctypes.c_size_t, _vp]),
     "sa_kv_session_import": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, _vp, ctypes.c_int32, ctypes.c_int32, _vp]),
@@ -518,6 +522,35 @@ def sa_swiglu(x, w_gate, w_up, act, stream=None) -> None:
     F = w_gate.shape[0]
     assert w_gate.shape == w_up.shape and w_gate.shape[1] == K and tuple(act.shape) == (M, F)
     _check(load_library().sa_swiglu(_ptr(x), _ptr(w_gate), _ptr(w_up), _ptr(act), M, F, K, _stream_ptr(stream)), "sa_swiglu")
+
+
+def sa_linear_workspace_bytes(M: int, N: int, K: int) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_linear_workspace_bytes(M, N, K, ctypes.byref(out)), "sa_linear_workspace_bytes")
+    return int(out.value)
+
+
+def sa_linear_ws(x, w, y, workspace, residual=None, stream=None) -> None:
+    """sa_linear with a split-K scratch (small M)."""
+    M, K = x.shape
+    N = w.shape[0]
+    assert w.shape[1] == K and tuple(y.shape) == (M, N)
+    _check(load_library().sa_linear_ws(_ptr(x), _ptr(w), _ptr(residual), _ptr(y), M, N, K, _ptr(workspace), _nbytes(workspace),
+                                       _stream_ptr(stream)), "sa_linear_ws")
+
+
+def sa_swiglu_workspace_bytes(M: int, F: int, K: int) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_swiglu_workspace_bytes(M, F, K, ctypes.byref(out)), "sa_swiglu_workspace_bytes")
+    return int(out.value)
+
+
+def sa_swiglu_ws(x, w_gate, w_up, act, workspace, stream=None) -> None:
+    M, K = x.shape
+    F = w_gate.shape[0]
+    assert w_gate.shape == w_up.shape and w_gate.shape[1] == K and tuple(act.shape) == (M, F)
+    _check(load_library().sa_swiglu_ws(_ptr(x), _ptr(w_gate), _ptr(w_up), _ptr(act), M, F, K, _ptr(workspace), _nbytes(workspace),
+                                       _stream_ptr(stream)), "sa_swiglu_ws")
 
 
 def sa_rmsnorm(x, w, eps: float, y, stream=None) -> None:

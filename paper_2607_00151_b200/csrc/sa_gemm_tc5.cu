@@ -56,7 +56,11 @@ struct GemmArgs {
     __nv_bfloat16 *k_base, *v_base, *q_out;
     int64_t stride_head;
     int32_t Hq, Hkv;
+    // split-K (small M: too few tiles to stream the weights at HBM rate): a work unit is (tile, k slice)
+    int32_t k_splits;          // >= 1
+    float *partial;            // [tiles * k_splits][128 rows][256 columns] fp32 when k_splits > 1
 };
+constexpr size_t kPartialFloats = size_t(GBN) * GBM;  // per work unit
 
 __device__ __forceinline__ void tile_coords(const GemmArgs &a, int t, int &mt, int &nt) {
     const int per_group = M_GROUP * a.n_tiles;
@@ -93,6 +97,86 @@ __device__ __forceinline__ void ld_row32(uint32_t taddr, float (&f)[32]) {
     for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(r[i]);
 }
 
+// One chunk of one output row, from 32-column pieces of the fp32 accumulator row that `ld(column, f)` supplies
+// (TMEM in the GEMM kernel, the sum of the k-slice partials in the split-K reduction).
+//   EPI_PLAIN : chunk c in 0..7 = columns 32c..32c+31          y = acc (+ residual)
+//   EPI_SWIGLU: chunk c in 0..3 = FFN units 32c..32c+31         act = SiLU(acc[gate]) * acc[128 + up]
+//   EPI_QKV   : chunk c in 0..3 = head c>>1, dims m0..m0+31 and 64+m0.. with m0 = 32 (c & 1): RoPE, scatter
+template <int EPI> constexpr int epi_chunks() { return EPI == EPI_PLAIN ? 8 : 4; }
+
+template <int EPI, class Load>
+__device__ __forceinline__ void epi_chunk(const GemmArgs &a, int nt, int64_t row, bool live, int c, Load ld) {
+    if (EPI == EPI_PLAIN) {
+        const int col = nt * GBN + c * 32;
+        if (col >= a.N) return;  // uniform over the CTA
+        float f[32];
+        ld(c * 32, f);
+        if (live) {
+            __nv_bfloat16 *dst = a.y + row * a.ldy + col;
+            if (a.residual) {
+                const __nv_bfloat16 *rs = a.residual + row * a.ldy + col;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    if (col + 8 * i >= a.N) break;
+                    const uint4 u = *reinterpret_cast<const uint4 *>(rs + 8 * i);
+                    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        f[8 * i + 2 * j] += __uint_as_float(w[j] << 16);
+                        f[8 * i + 2 * j + 1] += __uint_as_float(w[j] & 0xffff0000u);
+                    }
+                }
+            }
+            store_row32(dst, f, a.N - col);
+        }
+    } else if (EPI == EPI_SWIGLU) {
+        const int col = nt * 128 + c * 32;
+        if (col >= a.N) return;
+        float g[32], u[32];
+        ld(c * 32, g);
+        ld(128 + c * 32, u);
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            const float e = ex2_approx(-1.4426950408889634f * g[i]);
+            g[i] = __fdividef(g[i], 1.0f + e) * u[i];
+        }
+        if (live) store_row32(a.y + row * a.ldy + col, g, a.N - col);
+    } else {  // EPI_QKV: two heads of 128 dims per tile
+        const int hh = c >> 1, m0 = (c & 1) * 32;
+        const int head = nt * 2 + hh;
+        if (head >= a.Hq + 2 * a.Hkv) return;
+        const bool rot = head < a.Hq + a.Hkv;
+        const int64_t off = live ? a.tok_off[row] : 0;
+        __nv_bfloat16 *dst;
+        if (head < a.Hq)
+            dst = a.q_out + (row * a.Hq + head) * 128;
+        else if (head < a.Hq + a.Hkv)
+            dst = a.k_base + off + int64_t(head - a.Hq) * a.stride_head;
+        else
+            dst = a.v_base + off + int64_t(head - a.Hq - a.Hkv) * a.stride_head;
+        float lo[32], hi[32];
+        ld(hh * 128 + m0, lo);
+        ld(hh * 128 + 64 + m0, hi);
+        if (live) {
+            if (rot) {
+                const float4 *csp = reinterpret_cast<const float4 *>(a.cs + row * 64 + m0);
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float4 c2 = __ldg(csp + i);  // (cos, sin) of dims 2i, 2i+1
+                    const float x0 = lo[2 * i], x1 = hi[2 * i];
+                    lo[2 * i] = fmaf(x0, c2.x, -(x1 * c2.y));
+                    hi[2 * i] = fmaf(x1, c2.x, x0 * c2.y);
+                    const float z0 = lo[2 * i + 1], z1 = hi[2 * i + 1];
+                    lo[2 * i + 1] = fmaf(z0, c2.z, -(z1 * c2.w));
+                    hi[2 * i + 1] = fmaf(z1, c2.z, z0 * c2.w);
+                }
+            }
+            store_row32(dst + m0, lo);
+            store_row32(dst + 64 + m0, hi);
+        }
+    }
+}
+
 template <int EPI>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b0,
@@ -109,8 +193,15 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
     auto bar_acc_empty = [&](int b) -> uint32_t { return bar0 + 8u * uint32_t(2 * GSTAGES + 2 + b); };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int n_tiles_total = a.m_tiles * a.n_tiles;
     const int k_steps = a.K / GBK;
+    const int KS = a.k_splits;
+    const int n_units = a.m_tiles * a.n_tiles * KS;  // unit u = (tile u / KS, k slice u % KS)
+    auto k_range = [&](int u, int &t, int &k0, int &k1) {
+        t = u / KS;
+        const int sl = u - t * KS;
+        k0 = int(int64_t(sl) * k_steps / KS);
+        k1 = int(int64_t(sl + 1) * k_steps / KS);
+    };
 
     if (tid == 0) {
         for (int s = 0; s < GSTAGES; ++s) {
@@ -136,13 +227,14 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
             prefetch_tmap(&tmap_b0);
             prefetch_tmap(&tmap_b1);
             int kc = 0;
-            for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x) {
-                int mt, nt;
+            for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+                int t, k0, k1, mt, nt;
+                k_range(u, t, k0, k1);
                 tile_coords(a, t, mt, nt);
                 const int m0 = mt * GBM;
                 const int r0 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN;        // rows of W (b0)
                 const int r1 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN + 128;  // rows of the second half (b1)
-                for (int ks = 0; ks < k_steps; ++ks, ++kc) {
+                for (int ks = k0; ks < k1; ++ks, ++kc) {
                     const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
                     mbar_wait(bar_empty(s), ph ^ 1);
                     const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
@@ -158,11 +250,13 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
         constexpr uint32_t idesc = umma_idesc_bf16(GBM, GBN, false, false);
         const uint64_t dA0 = umma_desc(s0, 16, 1024), dB0 = umma_desc(s0 + A_STAGE, 16, 1024);
         int kc = 0, tc = 0;
-        for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x, ++tc) {
+        for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++tc) {
+            int t, k0, k1;
+            k_range(u, t, k0, k1);
             const int b = tc & 1;
             mbar_wait(bar_acc_empty(b), ((tc >> 1) & 1) ^ 1);  // the epilogue has drained this accumulator
             tc_fence_after();
-            for (int ks = 0; ks < k_steps; ++ks, ++kc) {
+            for (int ks = k0; ks < k1; ++ks, ++kc) {
                 const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
                 mbar_wait(bar_full(s), ph);
                 tc_fence_after();
@@ -170,9 +264,9 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
                     const uint64_t dA = umma_desc_adv(dA0, s * STAGE_BYTES), dB = umma_desc_adv(dB0, s * STAGE_BYTES);
 #pragma unroll
                     for (int kk = 0; kk < GBK / 16; ++kk)
-                        umma_ss(tmem + b * GBN, umma_desc_adv(dA, kk * 32), umma_desc_adv(dB, kk * 32), idesc, ks > 0 || kk > 0);
+                        umma_ss(tmem + b * GBN, umma_desc_adv(dA, kk * 32), umma_desc_adv(dB, kk * 32), idesc, ks > k0 || kk > 0);
                     umma_commit(bar_empty(s));
-                    if (ks == k_steps - 1) umma_commit(bar_acc_full(b));
+                    if (ks == k1 - 1) umma_commit(bar_acc_full(b));
                 }
                 __syncwarp();
             }
@@ -183,99 +277,32 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
         const int row_in_tile = q4 * 32 + lane;
         const uint32_t lane_addr = uint32_t(q4 * 32) << 16;
         int tc = 0;
-        for (int t = blockIdx.x; t < n_tiles_total; t += gridDim.x, ++tc) {
+        for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++tc) {
             const int b = tc & 1;
-            int mt, nt;
+            int t, k0, k1, mt, nt;
+            k_range(u, t, k0, k1);
             tile_coords(a, t, mt, nt);
             const int64_t row = int64_t(mt) * GBM + row_in_tile;
             const bool live = row < a.M;
             mbar_wait(bar_acc_full(b), (tc >> 1) & 1);
             tc_fence_after();
             const uint32_t acc = tmem + lane_addr + b * GBN;
-            if (EPI == EPI_PLAIN) {
-                const int n0 = nt * GBN;
+            if (a.k_splits > 1) {
+                // a k slice of the tile: the raw fp32 accumulator row goes to this unit's partial [128 rows][256 columns]
+                float4 *dstp = reinterpret_cast<float4 *>(a.partial + size_t(u) * kPartialFloats + size_t(row_in_tile) * GBN);
 #pragma unroll 1
                 for (int c = 0; c < GBN / 32; ++c) {
-                    const int col = n0 + c * 32;
-                    if (col >= a.N) break;  // uniform over the CTA
                     float f[32];
                     ld_row32(acc + c * 32, f);
                     if (live) {
-                        __nv_bfloat16 *dst = a.y + row * a.ldy + col;
-                        if (a.residual) {
-                            const __nv_bfloat16 *rs = a.residual + row * a.ldy + col;
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                if (col + 8 * i >= a.N) break;
-                                const uint4 u = *reinterpret_cast<const uint4 *>(rs + 8 * i);
-                                const uint32_t w[4] = {u.x, u.y, u.z, u.w};
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) {
-                                    f[8 * i + 2 * j] += __uint_as_float(w[j] << 16);
-                                    f[8 * i + 2 * j + 1] += __uint_as_float(w[j] & 0xffff0000u);
-                                }
-                            }
-                        }
-                        store_row32(dst, f, a.N - col);
+                        for (int i = 0; i < 8; ++i) dstp[c * 8 + i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
                     }
                 }
-            } else if (EPI == EPI_SWIGLU) {
-                const int f0 = nt * 128;
+            } else {
 #pragma unroll 1
-                for (int c = 0; c < 4; ++c) {
-                    const int col = f0 + c * 32;
-                    if (col >= a.N) break;
-                    float g[32], u[32];
-                    ld_row32(acc + c * 32, g);
-                    ld_row32(acc + 128 + c * 32, u);
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        const float e = ex2_approx(-1.4426950408889634f * g[i]);
-                        g[i] = __fdividef(g[i], 1.0f + e) * u[i];
-                    }
-                    if (live) {
-                        __nv_bfloat16 *dst = a.y + row * a.ldy + col;
-                        store_row32(dst, g, a.N - col);
-                    }
-                }
-            } else {  // EPI_QKV: two heads of 128 dims per tile
-                const int64_t off = live ? a.tok_off[row] : 0;
-#pragma unroll 1
-                for (int hh = 0; hh < 2; ++hh) {
-                    const int head = nt * 2 + hh;
-                    if (head >= a.Hq + 2 * a.Hkv) break;
-                    const bool rot = head < a.Hq + a.Hkv;
-                    __nv_bfloat16 *dst;
-                    if (head < a.Hq)
-                        dst = a.q_out + (row * a.Hq + head) * 128;
-                    else if (head < a.Hq + a.Hkv)
-                        dst = a.k_base + off + int64_t(head - a.Hq) * a.stride_head;
-                    else
-                        dst = a.v_base + off + int64_t(head - a.Hq - a.Hkv) * a.stride_head;
-#pragma unroll 1
-                    for (int m0 = 0; m0 < 64; m0 += 32) {
-                        float lo[32], hi[32];
-                        ld_row32(acc + hh * 128 + m0, lo);
-                        ld_row32(acc + hh * 128 + 64 + m0, hi);
-                        if (live) {
-                            if (rot) {
-                                const float4 *csp = reinterpret_cast<const float4 *>(a.cs + row * 64 + m0);
-#pragma unroll
-                                for (int i = 0; i < 16; ++i) {
-                                    const float4 c2 = __ldg(csp + i);  // (cos, sin) of dims 2i, 2i+1
-                                    const float x0 = lo[2 * i], x1 = hi[2 * i];
-                                    lo[2 * i] = fmaf(x0, c2.x, -(x1 * c2.y));
-                                    hi[2 * i] = fmaf(x1, c2.x, x0 * c2.y);
-                                    const float z0 = lo[2 * i + 1], z1 = hi[2 * i + 1];
-                                    lo[2 * i + 1] = fmaf(z0, c2.z, -(z1 * c2.w));
-                                    hi[2 * i + 1] = fmaf(z1, c2.z, z0 * c2.w);
-                                }
-                            }
-                            store_row32(dst + m0, lo);
-                            store_row32(dst + 64 + m0, hi);
-                        }
-                    }
-                }
+                for (int c = 0; c < epi_chunks<EPI>(); ++c)
+                    epi_chunk<EPI>(a, nt, row, live, c, [&](int col_off, float (&f)[32]) { ld_row32(acc + col_off, f); });
             }
             tc_fence_before();
             mbar_arrive(bar_acc_empty(b));
@@ -284,6 +311,88 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
     tc_fence_before();
     __syncthreads();
     if (warp == 2) tmem_dealloc<512>(tmem);
+}
+
+// inverse of tile_coords
+__device__ __forceinline__ int tile_index(const GemmArgs &a, int mt, int nt) {
+    const int g = mt / M_GROUP;
+    const int gm = min(M_GROUP, a.m_tiles - g * M_GROUP);
+    return g * M_GROUP * a.n_tiles + nt * gm + (mt - g * M_GROUP);
+}
+
+// sum over the k slices, in slice order, of four consecutive accumulator columns of one row
+__device__ __forceinline__ float4 splitk_sum4(const GemmArgs &a, int t, int row_in_tile, int col) {
+    const float4 *p = reinterpret_cast<const float4 *>(a.partial + size_t(t) * a.k_splits * kPartialFloats + size_t(row_in_tile) * GBN + col);
+    float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int sl = 0; sl < a.k_splits; ++sl) {
+        const float4 v = p[size_t(sl) * (kPartialFloats / 4)];
+        s.x += v.x;
+        s.y += v.y;
+        s.z += v.z;
+        s.w += v.w;
+    }
+    return s;
+}
+
+__device__ __forceinline__ uint2 pack4(float a, float b, float c, float d) { return make_uint2(pack_bf16x2(a, b), pack_bf16x2(c, d)); }
+
+// Split-K reduction + epilogue, elementwise: one thread = one row and four consecutive output columns (PLAIN: of
+// y; SWIGLU: four FFN units; QKV: dims m..m+3 and 64+m..64+m+3 of one head).  Slices are summed in slice order,
+// fixed, so the bits do not depend on which CTA ran which slice.
+template <int EPI>
+__global__ void __launch_bounds__(256) gemm_splitk_reduce_kernel(const GemmArgs a, int64_t n_items, int32_t items_per_row) {
+    const int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (e >= n_items) return;
+    const int64_t row = e / items_per_row;
+    const int j = int(e - row * items_per_row);
+    const int mt = int(row / GBM), rit = int(row - int64_t(mt) * GBM);
+    if (EPI == EPI_PLAIN) {
+        const int n = j * 4, nt = n / GBN, col = n - nt * GBN;
+        float4 v = splitk_sum4(a, tile_index(a, mt, nt), rit, col);
+        if (a.residual) {
+            const uint2 r = *reinterpret_cast<const uint2 *>(a.residual + row * a.ldy + n);
+            v.x += __uint_as_float(r.x << 16);
+            v.y += __uint_as_float(r.x & 0xffff0000u);
+            v.z += __uint_as_float(r.y << 16);
+            v.w += __uint_as_float(r.y & 0xffff0000u);
+        }
+        *reinterpret_cast<uint2 *>(a.y + row * a.ldy + n) = pack4(v.x, v.y, v.z, v.w);
+    } else if (EPI == EPI_SWIGLU) {
+        const int f = j * 4, nt = f / 128, col = f - nt * 128;
+        const int t = tile_index(a, mt, nt);
+        const float4 g = splitk_sum4(a, t, rit, col), u = splitk_sum4(a, t, rit, 128 + col);
+        const float gg[4] = {g.x, g.y, g.z, g.w}, uu[4] = {u.x, u.y, u.z, u.w};
+        float o[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float ex = ex2_approx(-1.4426950408889634f * gg[i]);
+            o[i] = __fdividef(gg[i], 1.0f + ex) * uu[i];
+        }
+        *reinterpret_cast<uint2 *>(a.y + row * a.ldy + f) = pack4(o[0], o[1], o[2], o[3]);
+    } else {
+        const int head = j / 16, m = (j - head * 16) * 4;   // 16 items of 4 + 4 dims per head
+        const int nt = head >> 1, hh = head & 1;
+        const int t = tile_index(a, mt, nt);
+        float4 lo = splitk_sum4(a, t, rit, hh * 128 + m), hi = splitk_sum4(a, t, rit, hh * 128 + 64 + m);
+        __nv_bfloat16 *dst;
+        if (head < a.Hq)
+            dst = a.q_out + (row * a.Hq + head) * 128;
+        else if (head < a.Hq + a.Hkv)
+            dst = a.k_base + a.tok_off[row] + int64_t(head - a.Hq) * a.stride_head;
+        else
+            dst = a.v_base + a.tok_off[row] + int64_t(head - a.Hq - a.Hkv) * a.stride_head;
+        if (head < a.Hq + a.Hkv) {
+            const float4 *csp = reinterpret_cast<const float4 *>(a.cs + row * 64 + m);
+            const float4 c01 = __ldg(csp), c23 = __ldg(csp + 1);  // (cos, sin) of dims m, m+1 | m+2, m+3
+            float x0, x1;
+            x0 = lo.x, x1 = hi.x, lo.x = fmaf(x0, c01.x, -(x1 * c01.y)), hi.x = fmaf(x1, c01.x, x0 * c01.y);
+            x0 = lo.y, x1 = hi.y, lo.y = fmaf(x0, c01.z, -(x1 * c01.w)), hi.y = fmaf(x1, c01.z, x0 * c01.w);
+            x0 = lo.z, x1 = hi.z, lo.z = fmaf(x0, c23.x, -(x1 * c23.y)), hi.z = fmaf(x1, c23.x, x0 * c23.y);
+            x0 = lo.w, x1 = hi.w, lo.w = fmaf(x0, c23.z, -(x1 * c23.w)), hi.w = fmaf(x1, c23.z, x0 * c23.w);
+        }
+        *reinterpret_cast<uint2 *>(dst + m) = pack4(lo.x, lo.y, lo.z, lo.w);
+        *reinterpret_cast<uint2 *>(dst + 64 + m) = pack4(hi.x, hi.y, hi.z, hi.w);
+    }
 }
 
 // Per token of a fused QKV append: the slot it lands in and (cos, sin) of its absolute position.
@@ -381,9 +490,17 @@ int device_sms() {
     return sms[dev];
 }
 
+// Split-K pays when the tiles alone cannot keep the SMs streaming weights (small M: decode batches, L301
+// "near-constant latency" regime): k slices per tile so that tiles x slices is about one wave.
+int choose_splits(int tiles, int k_steps, int sms) {
+    if (tiles <= 0 || tiles * 2 > sms) return 1;
+    const int s = std::min(std::min(sms / tiles, k_steps / 2), 32);
+    return s >= 2 ? s : 1;
+}
+
 template <int EPI>
-cudaError_t launch_gemm(const CUtensorMap &ta, const CUtensorMap &tb0, const CUtensorMap &tb1, const GemmArgs &a,
-                        cudaStream_t stream) {
+cudaError_t launch_gemm(const CUtensorMap &ta, const CUtensorMap &tb0, const CUtensorMap &tb1, GemmArgs a, void *splitk_ws,
+                        size_t splitk_bytes, cudaStream_t stream, int32_t *launches) {
     static bool attr_done = false;  // (per process; the attribute is set again on every device change below)
     static int attr_dev = -1;
     int dev = 0;
@@ -397,7 +514,21 @@ cudaError_t launch_gemm(const CUtensorMap &ta, const CUtensorMap &tb0, const CUt
     const int sms = device_sms();
     if (sms <= 0) return cudaErrorNoDevice;
     const int tiles = a.m_tiles * a.n_tiles;
-    gemm_tc5_kernel<EPI><<<unsigned(std::min(tiles, sms)), kGemmThreads, kSmemGemm, stream>>>(ta, tb0, tb1, a);
+    int ks = choose_splits(tiles, a.K / GBK, sms);
+    uintptr_t w = (reinterpret_cast<uintptr_t>(splitk_ws) + 255) & ~uintptr_t(255);
+    const size_t need = size_t(tiles) * ks * kPartialFloats * sizeof(float) + 256;
+    if (ks > 1 && (!splitk_ws || splitk_bytes < need)) ks = 1;  // no scratch: the unsplit kernel is always correct
+    a.k_splits = ks;
+    a.partial = ks > 1 ? reinterpret_cast<float *>(w) : nullptr;
+    gemm_tc5_kernel<EPI><<<unsigned(std::min(tiles * ks, sms)), kGemmThreads, kSmemGemm, stream>>>(ta, tb0, tb1, a);
+    if (launches) ++*launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess || ks == 1) return e;
+    // items of four output columns per row: PLAIN N/4 (N is a multiple of 8), SWIGLU F/4, QKV 16 per head
+    const int32_t per_row = EPI == EPI_QKV ? (a.Hq + 2 * a.Hkv) * 16 : a.N / 4;
+    const int64_t n_items = a.M * per_row;
+    gemm_splitk_reduce_kernel<EPI><<<unsigned((n_items + 255) / 256), 256, 0, stream>>>(a, n_items, per_row);
+    if (launches) ++*launches;
     return cudaGetLastError();
 }
 
@@ -405,9 +536,21 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 
 
 }  // namespace
 
+// scratch a GEMM of M rows and `n_tiles` column tiles over K wants for split-K (0: it will not split)
+size_t gemm_splitk_bytes(int64_t M, int32_t n_tiles, int32_t K) {
+    const int sms = device_sms();
+    if (M <= 0 || n_tiles <= 0 || K < GBK || sms <= 0) return 0;
+    const int64_t tiles = (M + GBM - 1) / GBM * n_tiles;
+    if (tiles * 2 > sms) return 0;
+    const int ks = choose_splits(int(tiles), K / GBK, sms);
+    return ks > 1 ? size_t(tiles) * ks * kPartialFloats * sizeof(float) + 512 : 0;
+}
+size_t gemm_plain_splitk_bytes(int64_t M, int32_t N, int32_t K) { return gemm_splitk_bytes(M, (N + GBN - 1) / GBN, K); }
+size_t gemm_swiglu_splitk_bytes(int64_t M, int32_t F, int32_t K) { return gemm_splitk_bytes(M, (F + 127) / 128, K); }
+
 // y[M, N] = x W^T (+ residual): shared by sa_linear and sa_layer_forward
 int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
-                   cudaStream_t stream) {
+                   void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches) {
     if (M < 0 || N <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
     if (K % GBK != 0 || N % 8 != 0 || M > (int64_t(1) << 30)) return SA_ERR_UNSUPPORTED;
     if (M == 0) return SA_OK;
@@ -423,11 +566,11 @@ int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, 
     a.y = static_cast<__nv_bfloat16 *>(y);
     a.residual = static_cast<const __nv_bfloat16 *>(residual);
     a.ldy = N;
-    return launch_gemm<EPI_PLAIN>(ta, tb, tb, a, stream) == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+    return launch_gemm<EPI_PLAIN>(ta, tb, tb, a, splitk_ws, splitk_bytes, stream, launches) == cudaSuccess ? SA_OK : SA_ERR_CUDA;
 }
 
 int32_t gemm_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
-                    cudaStream_t stream) {
+                    void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches) {
     if (M < 0 || F <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
     if (K % GBK != 0 || F % 8 != 0 || M > (int64_t(1) << 30)) return SA_ERR_UNSUPPORTED;
     if (M == 0) return SA_OK;
@@ -443,7 +586,7 @@ int32_t gemm_swiglu(const void *x, const void *w_gate, const void *w_up, void *a
     a.n_tiles = (F + 127) / 128;
     a.y = static_cast<__nv_bfloat16 *>(act);
     a.ldy = F;
-    return launch_gemm<EPI_SWIGLU>(ta, tg, tu, a, stream) == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+    return launch_gemm<EPI_SWIGLU>(ta, tg, tu, a, splitk_ws, splitk_bytes, stream, launches) == cudaSuccess ? SA_OK : SA_ERR_CUDA;
 }
 
 int32_t rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, cudaStream_t stream) {
@@ -457,14 +600,24 @@ int32_t rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int
     return cudaGetLastError() == cudaSuccess ? SA_OK : SA_ERR_CUDA;
 }
 
-size_t qkv_workspace_bytes(int64_t total) {
+static size_t qkv_tables_bytes(int64_t total) {
     const size_t T = size_t(std::max<int64_t>(total, 0));
     return (T * 64 * sizeof(float2) + 255) / 256 * 256 + (T * sizeof(int64_t) + 255) / 256 * 256 + 256;
+}
+// per-token tables + split-K scratch; the hidden size is not known here, so the scratch is sized for the most
+// slices any K can ask for (tiles x slices never exceeds the SM count)
+size_t qkv_workspace_bytes(const sa_kv_pool *pool, int64_t total) {
+    const int sms = device_sms();
+    const int64_t n_tiles = ((pool->cfg.num_q_heads + 2 * pool->cfg.num_kv_heads) * 128 + GBN - 1) / GBN;
+    const int64_t tiles = (std::max<int64_t>(total, 0) + GBM - 1) / GBM * n_tiles;
+    const size_t scratch = (sms > 0 && tiles > 0 && tiles * 2 <= sms) ? size_t(sms) * kPartialFloats * sizeof(float) + 512 : 0;
+    return qkv_tables_bytes(total) + scratch;
 }
 
 // the device half of sa_qkv_rope_append, after append_prepare has placed the tokens
 int32_t qkv_rope_append_device(sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req, int64_t total, const void *h,
-                               const void *w_qkv, int32_t hidden, void *q_out, void *workspace, cudaStream_t stream) {
+                               const void *w_qkv, int32_t hidden, void *q_out, void *workspace, size_t workspace_bytes,
+                               cudaStream_t stream) {
     const sa_kv_pool_config &c = pool->cfg;
     const int32_t N = (c.num_q_heads + 2 * c.num_kv_heads) * 128;
     uintptr_t w = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255);
@@ -491,8 +644,12 @@ int32_t qkv_rope_append_device(sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_
     a.stride_head = pool->stride_head;
     a.Hq = c.num_q_heads;
     a.Hkv = c.num_kv_heads;
-    if (launch_gemm<EPI_QKV>(ta, tb, tb, a, stream) != cudaSuccess) return SA_ERR_CUDA;
-    ++pool->last_launches;
+    const size_t tables = qkv_tables_bytes(total);
+    char *scratch = reinterpret_cast<char *>(w) + tables;
+    const size_t used = size_t(scratch - static_cast<char *>(workspace));
+    if (launch_gemm<EPI_QKV>(ta, tb, tb, a, scratch, workspace_bytes > used ? workspace_bytes - used : 0, stream,
+                             &pool->last_launches) != cudaSuccess)
+        return SA_ERR_CUDA;
     return SA_OK;
 }
 

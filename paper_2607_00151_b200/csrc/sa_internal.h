@@ -170,13 +170,16 @@ cudaError_t launch_flash_prefill_legacy(const sa_kv_pool *pool, const ReqMeta *r
 
 // dense operators of the layer (sa_gemm_tc5.cu); each returns an SA_* status
 int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
-                   cudaStream_t stream);
+                   void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches);
 int32_t gemm_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
-                    cudaStream_t stream);
+                    void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches);
+size_t gemm_plain_splitk_bytes(int64_t M, int32_t N, int32_t K);
+size_t gemm_swiglu_splitk_bytes(int64_t M, int32_t F, int32_t K);
 int32_t rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, cudaStream_t stream);
-size_t qkv_workspace_bytes(int64_t total);
+size_t qkv_workspace_bytes(const sa_kv_pool *pool, int64_t total);
 int32_t qkv_rope_append_device(sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req, int64_t total, const void *h,
-                               const void *w_qkv, int32_t hidden, void *q_out, void *workspace, cudaStream_t stream);
+                               const void *w_qkv, int32_t hidden, void *q_out, void *workspace, size_t workspace_bytes,
+                               cudaStream_t stream);
 // sa_mixed_attention's workspace need for a batch whose q_r tokens are still to be appended (sa_attention.cu)
 int32_t attention_workspace_after_append(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                          const int32_t *qo_indptr, size_t *out_bytes);

@@ -13,7 +13,7 @@ namespace {
 inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
 struct LayerWs {
-    size_t off_h, off_q, off_attn, off_x1, off_act, off_qkv, off_attn_ws, total;
+    size_t off_h, off_q, off_attn, off_x1, off_act, off_qkv, off_attn_ws, off_splitk, splitk_bytes, total;
 };
 
 LayerWs layer_ws(const sa_kv_pool *pool, const sa_layer_weights *L, int64_t T, size_t attn_ws) {
@@ -25,8 +25,12 @@ LayerWs layer_ws(const sa_kv_pool *pool, const sa_layer_weights *L, int64_t T, s
     w.off_x1 = w.off_attn + up256(t * QD * 2);
     w.off_act = w.off_x1 + up256(t * H * 2);
     w.off_qkv = w.off_act + up256(t * size_t(L->ffn) * 2);
-    w.off_attn_ws = w.off_qkv + up256(sa::qkv_workspace_bytes(T));
-    w.total = w.off_attn_ws + up256(attn_ws) + 512;
+    w.off_attn_ws = w.off_qkv + up256(sa::qkv_workspace_bytes(pool, T));
+    w.off_splitk = w.off_attn_ws + up256(attn_ws) + 256;
+    // split-K scratch of the output projection, the SwiGLU GEMM and the down projection (they run one after the other)
+    w.splitk_bytes = std::max(std::max(sa::gemm_plain_splitk_bytes(T, L->hidden, int32_t(QD)), sa::gemm_swiglu_splitk_bytes(T, L->ffn, L->hidden)),
+                              sa::gemm_plain_splitk_bytes(T, L->hidden, L->ffn));
+    w.total = w.off_splitk + up256(w.splitk_bytes) + 512;
     return w;
 }
 
@@ -51,12 +55,34 @@ __global__ void fill_small_kernel(__nv_bfloat16 *p, size_t n, uint32_t salt, flo
 
 extern "C" int32_t sa_linear(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N,
                              int32_t K, void *stream) {
-    return sa::gemm_plain(x, w, residual, y, M, N, K, static_cast<cudaStream_t>(stream));
+    return sa::gemm_plain(x, w, residual, y, M, N, K, nullptr, 0, static_cast<cudaStream_t>(stream), nullptr);
 }
 
 extern "C" int32_t sa_swiglu(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F,
                              int32_t K, void *stream) {
-    return sa::gemm_swiglu(x, w_gate, w_up, act, M, F, K, static_cast<cudaStream_t>(stream));
+    return sa::gemm_swiglu(x, w_gate, w_up, act, M, F, K, nullptr, 0, static_cast<cudaStream_t>(stream), nullptr);
+}
+
+extern "C" int32_t sa_linear_workspace_bytes(int64_t M, int32_t N, int32_t K, size_t *out_bytes) {
+    if (!out_bytes || M < 0 || N <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
+    *out_bytes = sa::gemm_plain_splitk_bytes(M, N, K);
+    return SA_OK;
+}
+
+extern "C" int32_t sa_linear_ws(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
+                                void *workspace, size_t workspace_bytes, void *stream) {
+    return sa::gemm_plain(x, w, residual, y, M, N, K, workspace, workspace_bytes, static_cast<cudaStream_t>(stream), nullptr);
+}
+
+extern "C" int32_t sa_swiglu_workspace_bytes(int64_t M, int32_t F, int32_t K, size_t *out_bytes) {
+    if (!out_bytes || M < 0 || F <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
+    *out_bytes = sa::gemm_swiglu_splitk_bytes(M, F, K);
+    return SA_OK;
+}
+
+extern "C" int32_t sa_swiglu_ws(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
+                                void *workspace, size_t workspace_bytes, void *stream) {
+    return sa::gemm_swiglu(x, w_gate, w_up, act, M, F, K, workspace, workspace_bytes, static_cast<cudaStream_t>(stream), nullptr);
 }
 
 extern "C" int32_t sa_rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, void *stream) {
@@ -65,7 +91,7 @@ extern "C" int32_t sa_rmsnorm(const void *x, const void *w, float eps, void *y, 
 
 extern "C" int32_t sa_qkv_rope_append_workspace_bytes(const sa_kv_pool *pool, int64_t total_tokens, size_t *out_bytes) {
     if (!pool || !out_bytes || total_tokens < 0) return SA_ERR_INVALID_ARG;
-    *out_bytes = sa::qkv_workspace_bytes(total_tokens);
+    *out_bytes = sa::qkv_workspace_bytes(pool, total_tokens);
     return SA_OK;
 }
 
@@ -77,8 +103,8 @@ extern "C" int32_t sa_qkv_rope_append(sa_kv_pool *pool, int32_t n_req, const int
     if (pool->cfg.head_dim != 128 || hidden % 64 != 0) return SA_ERR_UNSUPPORTED;
     if (n_req > 0 && qo_indptr && !pool->host_only) {
         const int64_t total = qo_indptr[n_req];
-        if (total > 0 && (!h || !w_qkv || !q_out || !workspace || workspace_bytes < qkv_workspace_bytes(total)))
-            return total > 0 && workspace && workspace_bytes < qkv_workspace_bytes(total) ? SA_ERR_WORKSPACE_TOO_SMALL
+        if (total > 0 && (!h || !w_qkv || !q_out || !workspace || workspace_bytes < qkv_workspace_bytes(pool, total)))
+            return total > 0 && workspace && workspace_bytes < qkv_workspace_bytes(pool, total) ? SA_ERR_WORKSPACE_TOO_SMALL
                                                                                          : SA_ERR_INVALID_ARG;
         if ((reinterpret_cast<uintptr_t>(h) | reinterpret_cast<uintptr_t>(w_qkv) | reinterpret_cast<uintptr_t>(q_out)) & 15)
             return SA_ERR_INVALID_ARG;
@@ -88,7 +114,7 @@ extern "C" int32_t sa_qkv_rope_append(sa_kv_pool *pool, int32_t n_req, const int
     int64_t total = 0;
     const int32_t st = append_prepare(pool, n_req, sids, qo_indptr, h && w_qkv, stream, &reqs_dev, &total);
     if (st != SA_OK || !reqs_dev || total == 0) return st;
-    return qkv_rope_append_device(pool, reqs_dev, n_req, total, h, w_qkv, hidden, q_out, workspace, stream);
+    return qkv_rope_append_device(pool, reqs_dev, n_req, total, h, w_qkv, hidden, q_out, workspace, workspace_bytes, stream);
 }
 
 extern "C" int32_t sa_layer_workspace_bytes(const sa_kv_pool *pool, const sa_layer_weights *layer, int32_t n_req,
@@ -131,7 +157,7 @@ extern "C" int32_t sa_layer_forward(sa_kv_pool *pool, const sa_layer_weights *L,
     if ((st = rmsnorm(x, L->norm1, L->rms_eps, h, T, H, stream)) != SA_OK) return st;
     ++launches;
     // q|k|v = h W_qkv^T, RoPE, K'/V into the pages, Q' to q   (all-or-nothing on page exhaustion)
-    st = sa_qkv_rope_append(pool, n_req, sids, qo_indptr, h, L->w_qkv, H, q, w + wl.off_qkv, sa::qkv_workspace_bytes(T), stream);
+    st = sa_qkv_rope_append(pool, n_req, sids, qo_indptr, h, L->w_qkv, H, q, w + wl.off_qkv, sa::qkv_workspace_bytes(pool, T), stream);
     if (st != SA_OK) return st;
     launches += pool->last_launches;
     // a = attention over the paged cache (prefill chunks and decode rows of the batch together)
@@ -139,14 +165,17 @@ extern "C" int32_t sa_layer_forward(sa_kv_pool *pool, const sa_layer_weights *L,
     if (st != SA_OK) return st;
     launches += pool->last_launches;
     // x1 = x + a W_o^T
-    if ((st = gemm_plain(attn, L->w_o, x, x1, T, H, QD, stream)) != SA_OK) return st;
+    void *sk = w + wl.off_splitk;
+    const size_t skb = up256(wl.splitk_bytes) + 256;
+    if ((st = gemm_plain(attn, L->w_o, x, x1, T, H, QD, sk, skb, stream, &launches)) != SA_OK) return st;
     // h2 = RMSNorm(x1; norm2)  (reuses h)
     if ((st = rmsnorm(x1, L->norm2, L->rms_eps, h, T, H, stream)) != SA_OK) return st;
+    ++launches;
     // act = SiLU(h2 W_gate^T) * (h2 W_up^T)
-    if ((st = gemm_swiglu(h, L->w_gate, L->w_up, act, T, L->ffn, H, stream)) != SA_OK) return st;
+    if ((st = gemm_swiglu(h, L->w_gate, L->w_up, act, T, L->ffn, H, sk, skb, stream, &launches)) != SA_OK) return st;
     // y = x1 + act W_down^T
-    if ((st = gemm_plain(act, L->w_down, x1, y, T, H, L->ffn, stream)) != SA_OK) return st;
-    pool->last_launches = launches + 4;
+    if ((st = gemm_plain(act, L->w_down, x1, y, T, H, L->ffn, sk, skb, stream, &launches)) != SA_OK) return st;
+    pool->last_launches = launches;
     return SA_OK;
 }
 
@@ -186,6 +215,9 @@ extern "C" int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_head
     void *w_d = b.alloc(H * F * 2), *n1 = b.alloc(H * 2), *n2 = b.alloc(H * 2);
     void *x = b.alloc(M * H * 2), *h = b.alloc(M * H * 2), *qkv = b.alloc(M * NQKV * 2), *x1 = b.alloc(M * H * 2);
     void *act = b.alloc(M * F * 2), *y = b.alloc(M * H * 2), *flush = b.alloc(flush_bytes);
+    const size_t skb = size_t(160) * 128 * 1024;  // split-K scratch: tiles x slices never exceeds the SM count
+    void *sk = b.alloc(skb);
+    if (!sk) return SA_ERR_CUDA;
     if (!w_qkv || !w_o || !w_g || !w_u || !w_d || !n1 || !n2 || !x || !h || !qkv || !x1 || !act || !y || !flush) return SA_ERR_CUDA;
     if (cudaEventCreate(&b.e0) != cudaSuccess || cudaEventCreate(&b.e1) != cudaSuccess) return SA_ERR_CUDA;
     struct { void *p; size_t n; float amp; } fills[] = {
@@ -204,11 +236,11 @@ extern "C" int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_head
             cudaEventRecord(b.e0, stream);
             int32_t st = rmsnorm(x, n1, 1e-5f, h, m, hidden, stream);
             // the attention output stands in for the o-projection's input: the first Hq*D columns of qkv's buffer
-            if (st == SA_OK) st = gemm_plain(h, w_qkv, nullptr, qkv, m, int32_t(NQKV), hidden, stream);
-            if (st == SA_OK) st = gemm_plain(qkv, w_o, x, x1, m, hidden, int32_t(QD), stream);
+            if (st == SA_OK) st = gemm_plain(h, w_qkv, nullptr, qkv, m, int32_t(NQKV), hidden, sk, skb, stream, nullptr);
+            if (st == SA_OK) st = gemm_plain(qkv, w_o, x, x1, m, hidden, int32_t(QD), sk, skb, stream, nullptr);
             if (st == SA_OK) st = rmsnorm(x1, n2, 1e-5f, h, m, hidden, stream);
-            if (st == SA_OK) st = gemm_swiglu(h, w_g, w_u, act, m, ffn, hidden, stream);
-            if (st == SA_OK) st = gemm_plain(act, w_d, x1, y, m, hidden, ffn, stream);
+            if (st == SA_OK) st = gemm_swiglu(h, w_g, w_u, act, m, ffn, hidden, sk, skb, stream, nullptr);
+            if (st == SA_OK) st = gemm_plain(act, w_d, x1, y, m, hidden, ffn, sk, skb, stream, nullptr);
             if (st != SA_OK) return st;
             cudaEventRecord(b.e1, stream);
             if (cudaEventSynchronize(b.e1) != cudaSuccess) return SA_ERR_CUDA;

@@ -95,6 +95,54 @@ def test_linear_untouched_outside():
     _check_op(y, lo.linear(x, w), "linear 130x264x64")
 
 
+# ------------------------------------------------------------------ split-K (small M: decode batches)
+@pytest.mark.parametrize("M,N,K,res", [
+    (1, 4096, 4096, True),        # one decode row through the output projection: 16 tiles x 9 k slices
+    (64, 4096, 14336, True),      # the down projection of a 64-row decode batch: 224 k-steps cut 9 ways
+    (200, 6144, 4096, False),     # two m-tiles x 24 n-tiles = 48 tiles x 3 slices
+    (130, 520, 448, True),        # ragged N, 7 k-steps in 3 uneven slices (2 + 2 + 3)
+])
+def test_linear_split_k(M, N, K, res):
+    nb = sa.sa_linear_workspace_bytes(M, N, K)
+    assert nb > 0, "this shape is expected to split"
+    x = _rand((M, K), 11)
+    w = _rand((N, K), 12, K ** -0.5)
+    r = _rand((M, N), 13) if res else None
+    ws = torch.full((nb,), 0xFF, dtype=torch.uint8, device=DEV)   # NaN bit patterns: a partial read before it is written shows
+    ref = lo.linear(x, w)
+    if res:
+        ref = ref + lo.widen(r)
+    ys = []
+    for _ in range(2):
+        y = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device=DEV)
+        sa.sa_linear_ws(x, w, y, ws, r)
+        torch.cuda.synchronize()
+        _check_op(y, ref, "split-K linear %dx%dx%d" % (M, N, K))
+        ys.append(y)
+    assert torch.equal(ys[0].view(torch.int16), ys[1].view(torch.int16)), "slices are summed in a fixed order"
+    # without scratch the same call runs unsplit and still meets the oracle
+    y0 = torch.full((M, N), float("nan"), dtype=torch.bfloat16, device=DEV)
+    sa.sa_linear_ws(x, w, y0, None, r)
+    torch.cuda.synchronize()
+    _check_op(y0, ref, "unsplit fallback")
+    # large M never asks for scratch
+    assert sa.sa_linear_workspace_bytes(4096, N, K) == 0
+
+
+def test_swiglu_split_k():
+    M, F, K = 16, 4096, 4096      # 32 tiles x 4 slices
+    nb = sa.sa_swiglu_workspace_bytes(M, F, K)
+    assert nb > 0
+    x = _rand((M, K), 14)
+    wg = _rand((F, K), 15, 2.0 * K ** -0.5)
+    wu = _rand((F, K), 16, K ** -0.5)
+    ws = torch.full((nb,), 0xFF, dtype=torch.uint8, device=DEV)
+    act = torch.full((M, F), float("nan"), dtype=torch.bfloat16, device=DEV)
+    sa.sa_swiglu_ws(x, wg, wu, act, ws)
+    torch.cuda.synchronize()
+    _check_op(act, lo.swiglu_act(x, wg, wu), "split-K swiglu")
+
+
 # ------------------------------------------------------------------ sa_swiglu / sa_rmsnorm
 @pytest.mark.parametrize("M,F,K", [(5, 128, 64), (200, 328, 256), (1030, 14336, 4096)])
 def test_swiglu(M, F, K):
