@@ -131,14 +131,13 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
     const float a3 = max3(l1[9], __uint_as_float(s[30]), __uint_as_float(s[31]));
     return fmaxf(max3(a0, a1, a2), a3);
 }
-// exp2 of one chunk, row sums, bf16 P into 16 TMEM columns.  SA_POLY_SHARE of every four column
+// exp2 of column pairs [I0, I1) of one chunk, row sums, bf16 P packed into pk.  SA_POLY_SHARE of every four column
 // pairs take the packed cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
-template <bool MASKED>
-__device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
-                                                uint32_t taddr) {
-    uint32_t pk[16];
+template <bool MASKED, int I0, int I1>
+__device__ __forceinline__ void chunk_exp(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
+                                          uint32_t (&pk)[16]) {
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
+    for (int i = I0; i < I1; ++i) {
         // x = s * scale_log2 - m * scale_log2 for two columns at once (FFMA2)
         float x0, x1;
         unpack_f32x2(ffma2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sl2_2, neg_2), x0, x1);
@@ -153,7 +152,20 @@ __device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_
         __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
         pk[i] = *reinterpret_cast<uint32_t *>(&pb);
     }
+}
+// a whole chunk into 16 TMEM columns
+template <bool MASKED>
+__device__ __forceinline__ void chunk_exp_store(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
+                                                uint32_t taddr) {
+    uint32_t pk[16];
+    chunk_exp<MASKED, 0, 16>(s, sl2_2, neg_2, lsum, pk);
     tmem_st16(taddr, pk);
+}
+// P of the chunks stored so far is in TMEM: tell the MMA warp
+__device__ __forceinline__ void publish_p(uint32_t bar_addr) {
+    tmem_wait_st();
+    tc_fence_before();
+    mbar_arrive(bar_addr);
 }
 
 template <int LOG2B>
@@ -431,26 +443,35 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 }
                 const float neg = (m_used == -INFINITY) ? 0.f : -m_used * sl2;
                 const uint64_t neg_2 = pack_f32x2(neg, neg);
+                // A piece of P is published half a chunk late: by then its tcgen05.st has long landed, so
+                // tcgen05.wait::st does not stall the exponentials, and its PV product still has the rest of the tile
+                // to run under.  Only the last piece waits for its own store.
                 if (masked) {
+                    uint32_t pk[16];
                     chunk_exp_store<true>(s0, sl2_2, neg_2, lsum, tS);
                     chunk_exp_store<true>(s1, sl2_2, neg_2, lsum, tS + 16);
+                    chunk_exp<true, 0, 8>(s2, sl2_2, neg_2, lsum, pk);
+                    publish_p(bar(BAR_P_A + t));
+                    chunk_exp<true, 8, 16>(s2, sl2_2, neg_2, lsum, pk);
+                    tmem_st16(tS + 32, pk);
+                    chunk_exp<true, 0, 8>(s3, sl2_2, neg_2, lsum, pk);
+                    publish_p(bar(BAR_P_B + t));
+                    chunk_exp<true, 8, 16>(s3, sl2_2, neg_2, lsum, pk);
+                    tmem_st16(tS + 48, pk);
                 } else {
+                    uint32_t pk[16];
                     chunk_exp_store<false>(s0, sl2_2, neg_2, lsum, tS);
                     chunk_exp_store<false>(s1, sl2_2, neg_2, lsum, tS + 16);
+                    chunk_exp<false, 0, 8>(s2, sl2_2, neg_2, lsum, pk);
+                    publish_p(bar(BAR_P_A + t));
+                    chunk_exp<false, 8, 16>(s2, sl2_2, neg_2, lsum, pk);
+                    tmem_st16(tS + 32, pk);
+                    chunk_exp<false, 0, 8>(s3, sl2_2, neg_2, lsum, pk);
+                    publish_p(bar(BAR_P_B + t));
+                    chunk_exp<false, 8, 16>(s3, sl2_2, neg_2, lsum, pk);
+                    tmem_st16(tS + 48, pk);
                 }
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(bar(BAR_P_A + t));
-                if (masked) chunk_exp_store<true>(s2, sl2_2, neg_2, lsum, tS + 32);
-                else chunk_exp_store<false>(s2, sl2_2, neg_2, lsum, tS + 32);
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(bar(BAR_P_B + t));
-                if (masked) chunk_exp_store<true>(s3, sl2_2, neg_2, lsum, tS + 48);
-                else chunk_exp_store<false>(s3, sl2_2, neg_2, lsum, tS + 48);
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(bar(BAR_P_C + t));
+                publish_p(bar(BAR_P_C + t));
             }
             float l;
             {
