@@ -39,7 +39,7 @@ constexpr int TILE_BYTES = BN * D * 2;   // 32 KiB: two 64-wide halves of 128 ro
 constexpr int HALF_BYTES = TILE_BYTES / 2;
 constexpr int KV_STAGES = 2;
 #ifndef SA_POLY_SHARE
-#define SA_POLY_SHARE 0  // n of every 4 column pairs take exp2 as a packed cubic on the FMA pipe, the rest the MUFU
+#define SA_POLY_SHARE 2  // n of every 8 column pairs take exp2 as a packed cubic on the FMA pipe, the rest the MUFU
 #endif
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the row max grows by > 2^8
 
@@ -131,7 +131,7 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
     const float a3 = max3(l1[9], __uint_as_float(s[30]), __uint_as_float(s[31]));
     return fmaxf(max3(a0, a1, a2), a3);
 }
-// exp2 of column pairs [I0, I1) of one chunk, row sums, bf16 P packed into pk.  SA_POLY_SHARE of every four column
+// exp2 of column pairs [I0, I1) of one chunk, row sums, bf16 P packed into pk.  SA_POLY_SHARE of every eight column
 // pairs take the packed cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
 template <bool MASKED, int I0, int I1>
 __device__ __forceinline__ void chunk_exp(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
@@ -142,7 +142,7 @@ __device__ __forceinline__ void chunk_exp(const uint32_t (&s)[32], uint64_t sl2_
         float x0, x1;
         unpack_f32x2(ffma2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sl2_2, neg_2), x0, x1);
         float p0, p1;
-        if (!MASKED && (i & 3) < SA_POLY_SHARE) {
+        if (!MASKED && (i & 7) < SA_POLY_SHARE) {
             ex2_poly3_x2(x0, x1, p0, p1);
         } else {
             p0 = ex2_approx(x0);
