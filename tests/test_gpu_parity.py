@@ -255,6 +255,49 @@ def test_mixed_batch_equals_separate_calls_bitwise():
         check_lse(mixed[i][1], ref["lse"], 1e-3, "mixed s%d" % i)
 
 
+def test_decode_row_bits_do_not_depend_on_the_batch_size():
+    """Splits depend on the request alone (R17), so a decode row's bits must be the same alone, in a
+    40-row batch and in a 140-row batch, whatever launch shape the planner picks, and must meet the oracle
+    (PAPER.md L305).  140 forks of one 8000-token session share its pages."""
+    L = Layer(32, 8, 128, 64, 500000.0)
+    ctx, n_rows = 8000, 140                      # 8 splits per (row, head), the last one ragged
+    pages = ctx // 64 + 2 + n_rows + 4           # the forks share the whole pages and own a copy of the partial one
+    cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, pages, n_rows + 2, ctx + 64, L.rope_base, 0)
+    storage = torch.empty(sa.sa_kv_pool_storage_bytes(cfg), dtype=torch.uint8, device="cuda")
+    pool = sa.sa_kv_pool_create(cfg, storage, np.random.default_rng(3).permutation(pages).astype(np.int32))
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(77)
+    rnd = lambda n, h: (torch.randn((n, h, 128), generator=gen, device="cuda") * 128 ** -0.5).to(torch.bfloat16)
+    k, v, q = rnd(ctx, 8), rnd(ctx, 8), rnd(n_rows, 32)
+    base = sa.sa_kv_session_open(pool)
+    sa.sa_rope_kv_append(pool, [base], [0, ctx], k, v, None)
+    sids = [base] + [sa.sa_kv_session_fork(pool, base, ctx) for _ in range(n_rows - 1)]
+
+    def run(rows):
+        ss = [sids[i] for i in rows]
+        ip = np.arange(len(rows) + 1, dtype=np.int32)
+        qq = q[rows].contiguous()
+        out = torch.empty_like(qq)
+        lse = torch.empty((len(rows), 32), dtype=torch.float32, device="cuda")
+        ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(pool, ss, ip), 256), dtype=torch.uint8, device="cuda")
+        sa.sa_mixed_attention(pool, ss, ip, qq, out, lse, 0.0, ws)
+        torch.cuda.synchronize()
+        return out, lse
+
+    o140, l140 = run(list(range(140)))           # 140 x 8 x 8 = 8960 decode CTAs
+    o40, l40 = run(list(range(100, 140)))        # 2560
+    assert torch.equal(_bits(o40), _bits(o140[100:])) and torch.equal(l40, l140[100:])
+    for i in (0, 57, 139):                       # 64
+        o1, l1 = run([i])
+        assert torch.equal(_bits(o1[0]), _bits(o140[i])) and torch.equal(l1[0], l140[i])
+    # the oracle: every session holds the same 8000 cached tokens; row i queries with q[i] (already rotated) at position 7999
+    k_rot = orc.rope(k.cpu(), np.arange(ctx), L.rope_base)
+    for i in (0, 139):
+        ref = orc.attend(orc.widen(q[i:i + 1].cpu()), k_rot, orc.widen(v.cpu()), ctx - 1)
+        check_out(o140[i:i + 1], ref["o"], "decode row %d" % i)
+    sa.sa_kv_pool_destroy(pool)
+
+
 @pytest.mark.parametrize("Hq,Hkv,D,B", [(8, 8, 128, 64), (16, 2, 128, 16), (64, 8, 128, 64), (4, 2, 64, 64), (16, 1, 64, 16)])
 def test_shapes_gqa_pages(Hq, Hkv, D, B):
     sessions = [SessionSpec(150, 77), SessionSpec(1100, 1), SessionSpec(0, 200), SessionSpec(40, 2)]
