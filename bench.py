@@ -321,6 +321,76 @@ def measure_parts(local: int, peaks, iters: int = 10):
 
 
 # --------------------------------------------------------------------------------- whole layer (N3)
+def measure_config(cfg_id: int, local: int, peaks, iters: int):
+    """One other BASELINE.json config through the same two C-ABI calls, inputs resident in HBM: the step
+    (append + attention per chunk round) and the attention calls alone.  Config 5 generates its sessions
+    one at a time (lazy runner: the raw prefixes of 11 M tokens are never resident together)."""
+    from paper_2607_00151_b200 import binding as sa
+    from paper_2607_00151_b200.harness import Runner, make_pool
+    w = get_workload(cfg_id)
+    L = w.layer
+    dev = torch.device("cuda:%d" % local)
+    if cfg_id == 5 and torch.cuda.mem_get_info(dev)[1] < 170e9:
+        return {"workload": w.name, "skipped": "needs a 180 GB device"}
+    stream = torch.cuda.current_stream()
+    pool = make_pool(w, local, "random")
+    r = Runner(w, pool, None, local, want_lse=False, lazy=(cfg_id == 5))
+    r.fill_prefixes()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    A = w.pair_count()
+    flops = 4.0 * L.head_dim * L.num_q_heads * A
+    kappa = 2 * L.num_kv_heads * L.head_dim * 2
+    tokens = sum(s.new for s in w.sessions)
+    step_ms, attn_ms = [], []
+    for it in range(iters + 2):
+        flush.fill_(1)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        pairs = []
+        ev[0].record(stream)
+        r.truncate_to_prefix()
+        for rd in r.rounds:
+            rd.q.copy_(rd.q_raw)
+            sa.sa_rope_kv_append(pool, rd.sids, rd.indptr, rd.k, rd.v, rd.q)
+            if rd.workspace is None:
+                nb = sa.sa_mixed_attention_workspace_bytes(pool, rd.sids, rd.indptr)
+                rd.workspace = torch.empty(max(nb, 256), dtype=torch.uint8, device=dev)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(stream)
+            sa.sa_mixed_attention(pool, rd.sids, rd.indptr, rd.q, rd.out, None, 0.0, rd.workspace)
+            a1.record(stream)
+            pairs.append((a0, a1))
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        if it >= 2:   # two warm-up passes
+            step_ms.append(ev[0].elapsed_time(ev[1]))
+            attn_ms.append(sum(a.elapsed_time(b) for a, b in pairs))
+    sm, am = float(np.median(step_ms)), float(np.median(attn_ms))
+    res = {"workload": w.name, "layer": "Hq=%d Hkv=%d D=%d page=%d" % (L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size),
+           "requests": len(w.sessions), "tokens_per_step": tokens, "causal_pairs": A,
+           "decode_bytes": kappa * w.decode_kv_tokens(), "step_ms": sm, "attention_ms": am, "attention_ms_min": float(min(attn_ms)),
+           "tokens_per_s": tokens / (sm * 1e-3), "bound": "tensor", "unit": "TFLOP/s",
+           "achieved": flops / (am * 1e-3) / 1e12, "peak": peaks["bf16_tflops"], "iters": iters,
+           "note": "attention time is the whole sa_mixed_attention call (the decode rows of the workload included); "
+                   "causal algorithmic flops only; L2 flushed between iterations"}
+    res["frac"] = res["achieved"] / res["peak"]
+    r.close()
+    sa.sa_kv_pool_destroy(pool)
+    return res
+
+
+def measure_other_configs(local: int, peaks):
+    """Configs 3 and 5 (config 2 is the headline line, config 4 the `mixed_config4` object, config 1 is a
+    parity case too small to time).  A failure here never takes the headline line down."""
+    out = {}
+    for cfg_id, iters in ((3, 10), (5, 3)):
+        try:
+            out["config%d" % cfg_id] = measure_config(cfg_id, local, peaks, iters)
+        except Exception as e:   # noqa: BLE001 - reported in the JSON line
+            out["config%d" % cfg_id] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
+        torch.cuda.empty_cache()
+    return out
+
+
 def measure_layer(local: int, peaks, iters: int = 10):
     """Re-prefill of config 2's segment through sa_layer_forward (RMSNorm, fused QKV+RoPE+append, paged
     attention, output projection, SwiGLU FFN: PAPER.md L299-303 plus the attention path), Llama-3-8B
@@ -551,6 +621,9 @@ def run_ours(args, world, rank, local):
         line["mixed_config4"] = mixed
         line["transfer_config4"] = xfer
         line["layer"] = measure_layer(local, peaks)
+        torch.cuda.empty_cache()
+        if not args.no_other_configs:
+            line["other_configs"] = measure_other_configs(local, peaks)
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_sample(w, 15.0)
@@ -570,6 +643,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parts", action="store_true", help="skip the decode / append bandwidth measurements on config 4")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the config 3 / config 5 measurements")
+    ap.add_argument("--other-configs-only", action="store_true", help="only the config 3 / config 5 measurements")
     ap.add_argument("--parts-only", action="store_true", help="only the decode / append measurements (for profiling them)")
     ap.add_argument("--layer-only", action="store_true", help="only the whole-layer measurement (for profiling the GEMMs)")
     args = ap.parse_args()
@@ -582,6 +657,11 @@ def main():
         world = int(os.environ.get("WORLD_SIZE", "1"))
         rank = int(os.environ.get("RANK", "0"))
         run_reference(args, world, rank)
+        return
+    if args.other_configs_only:
+        import __graft_entry__
+        __graft_entry__.build()
+        print(json.dumps({"other_configs": measure_other_configs(0, load_peaks())}))
         return
     if args.parts_only:
         import __graft_entry__
