@@ -378,10 +378,46 @@ def measure_config(cfg_id: int, local: int, peaks, iters: int):
     return res
 
 
+def measure_latency_table(local: int, peaks):
+    """BASELINE.json config 4's sweep: sa_latency_table over prefill tokens {0, 512, 1K, 2K, 4K} (as 2048-token
+    chunks on a 20K-token prefix) x decode batch {1, 16, 64, 256} (contexts uniform in [8K, 32K]), and the
+    least-squares fit of PAPER.md Eq. 1's attention terms (L305-319, L349-353) on it."""
+    from paper_2607_00151_b200 import binding as sa
+    L = get_workload(4).layer
+    p_tok, d_bat = [0, 512, 1024, 2048, 4096], [1, 16, 64, 256]
+    cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, 140000, 320, 36864, L.rope_base, local)
+    pool = sa.sa_kv_pool_create(cfg)
+    try:
+        ms, sums = sa.sa_latency_table(pool, p_tok, d_bat, 20480, 8192, 32768, seed=4, warmup=3, iters=10)
+        model, fit_err = sa.sa_latency_fit(ms.reshape(-1), sums.reshape(-1, 2), True)
+    finally:
+        sa.sa_kv_pool_destroy(pool)
+    pred = model.c0_ms + model.alpha_d_ms * sums[:, :, 0] + model.alpha_p_ms * sums[:, :, 1]
+    rel = np.abs(pred - ms) / ms
+    kappa = 2 * L.num_kv_heads * L.head_dim * 2
+    dec_gbs = [float(kappa * sums[0, b, 0] / (ms[0, b] * 1e-3) / 1e9) for b in range(len(d_bat))]
+    return {"prefill_tokens": p_tok, "decode_batch": d_bat, "prefill_prefix": 20480, "decode_ctx": [8192, 32768],
+            "ms": [[round(float(x), 4) for x in row] for row in ms],
+            "sum_L": [int(x) for x in sums[0, :, 0]], "sum_A": [int(x) for x in sums[:, 0, 1]],
+            "decode_only_gbs": dec_gbs,
+            "eq1_fit": {"c0_ms": model.c0_ms, "alpha_d_ms_per_kv_token": model.alpha_d_ms, "alpha_p_ms_per_pair": model.alpha_p_ms,
+                        "max_rel_err": float(fit_err),
+                        "max_rel_err_points_over_0.25ms": float(rel[ms >= 0.25].max()),
+                        "decode_gbs_implied": kappa / model.alpha_d_ms / 1e6 if model.alpha_d_ms > 0 else None,
+                        "prefill_tflops_implied": 4.0 * L.head_dim * L.num_q_heads / model.alpha_p_ms / 1e9 if model.alpha_p_ms > 0 else None},
+            "note": "median of 10 CUDA-event timings of one sa_mixed_attention call per grid point, L2 evicted before each; "
+                    "d = 1 and p = 512 are launch- / fill-bound (reported, not gated)"}
+
+
 def measure_other_configs(local: int, peaks):
-    """Configs 3 and 5 (config 2 is the headline line, config 4 the `mixed_config4` object, config 1 is a
+    """Config 4's latency sweep, then configs 3 and 5 (config 2 is the headline line, config 4 the `mixed_config4` object, config 1 is a
     parity case too small to time).  A failure here never takes the headline line down."""
     out = {}
+    try:
+        out["latency_table_config4"] = measure_latency_table(local, peaks)
+    except Exception as e:   # noqa: BLE001 - reported in the JSON line
+        out["latency_table_config4"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
+    torch.cuda.empty_cache()
     for cfg_id, iters in ((3, 10), (5, 3)):
         try:
             out["config%d" % cfg_id] = measure_config(cfg_id, local, peaks, iters)
