@@ -18,7 +18,10 @@ namespace {
 
 constexpr int kThreads = 128;
 constexpr int kBN = 64;      // keys per tile
-constexpr int kStages = 3;
+#ifndef SA_DEC_STAGES
+#define SA_DEC_STAGES 3
+#endif
+constexpr int kStages = SA_DEC_STAGES;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -63,28 +66,47 @@ struct KvView {
     int32_t log2_page;
 };
 
-// Gather one 64-key tile of K and V (logical keys kt .. kt+63) into swizzled smem; rows at or
-// beyond kv_len are zero-filled, so slots the session does not own never reach the math.
+// Gather one 64-key tile of K and V (logical keys kt .. kt+63, kt a multiple of 64 and < kv_len) into
+// swizzled smem; rows at or beyond kv_len are zero-filled (src-size 0: nothing is read), so slots the
+// session does not own never reach the math.  The block-table reads come first and are branch-free:
+// with pages of >= 64 slots a tile lies in one page (one read per thread); smaller pages read one entry
+// per row, all independent, so their latencies overlap instead of adding up row by row.
 template <int D>
 __device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_len, uint32_t sK, uint32_t sV, int tid) {
     constexpr int CPR = D / 8;               // 16-byte chunks per row
     constexpr int RPP = kThreads / CPR;      // rows per pass
+    constexpr int NP = kBN / RPP;            // passes
     const int chunk = tid % CPR;
     const int r0 = tid / CPR;
-    const int pmask = (1 << kv.log2_page) - 1;
+    const int last = kv_len - 1;
+    if (kv.log2_page >= 6) {
+        const int32_t page = __ldg(kv.bt_row + (kt >> kv.log2_page));
+        const int slot0 = (kt & ((1 << kv.log2_page) - 1)) + r0;
+        const int64_t base = int64_t(page) * kv.stride_page + kv.head_off + int64_t(slot0) * D + chunk * 8;
+        const __nv_bfloat16 *kp = kv.k_base + base, *vp = kv.v_base + base;
 #pragma unroll
-    for (int i = 0; i < kBN / RPP; ++i) {
+        for (int i = 0; i < NP; ++i) {
+            const int row = r0 + i * RPP;
+            const int nb = (kt + row <= last) ? 16 : 0;
+            const uint32_t so = tile_off<D>(row, chunk);
+            cp_async16(sK + so, kp + i * (RPP * D), nb);
+            cp_async16(sV + so, vp + i * (RPP * D), nb);
+        }
+        return;
+    }
+    const int pmask = (1 << kv.log2_page) - 1;
+    int32_t page[NP];
+#pragma unroll
+    for (int i = 0; i < NP; ++i) page[i] = __ldg(kv.bt_row + (min(kt + r0 + i * RPP, last) >> kv.log2_page));
+#pragma unroll
+    for (int i = 0; i < NP; ++i) {
         const int row = r0 + i * RPP;
         const int key = kt + row;
-        const bool valid = key < kv_len;
-        int64_t off = 0;
-        if (valid) {
-            const int32_t page = __ldg(kv.bt_row + (key >> kv.log2_page));
-            off = int64_t(page) * kv.stride_page + kv.head_off + int64_t(key & pmask) * D + chunk * 8;
-        }
+        const int64_t off = int64_t(page[i]) * kv.stride_page + kv.head_off + int64_t(min(key, last) & pmask) * D + chunk * 8;
         const uint32_t so = tile_off<D>(row, chunk);
-        cp_async16(sK + so, kv.k_base + off, valid ? 16 : 0);
-        cp_async16(sV + so, kv.v_base + off, valid ? 16 : 0);
+        const int nb = key <= last ? 16 : 0;
+        cp_async16(sK + so, kv.k_base + off, nb);
+        cp_async16(sV + so, kv.v_base + off, nb);
     }
 }
 
