@@ -170,7 +170,14 @@ def _check(status: int, where: str):
 
 
 def _i32(a: Sequence[int]):
-    arr = np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+    """-> (int32 array the caller keeps alive, something ctypes passes as const int32_t*).  On the per-call path:
+    a ctypes array over the ndarray's buffer costs a third of ndarray.ctypes.data_as (which builds a helper object)."""
+    if type(a) is np.ndarray and a.dtype == np.int32 and a.flags.c_contiguous:
+        arr = a
+    else:
+        arr = np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+    if arr.size and arr.flags.writeable:
+        return arr, (ctypes.c_int32 * arr.size).from_buffer(arr)
     return arr, arr.ctypes.data_as(_i32p)
 
 
