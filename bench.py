@@ -270,7 +270,10 @@ def measure_parts(local: int, peaks, iters: int = 10):
               "frac": dec_bytes / (ms_dec * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": load_traffic().get("flash_mma_decode_cfg4"),
               "kernel": "flash_mma_kernel<128,0> (split-KV decode) + merge_splits_kernel on config 4's %d decode rows, "
                         "%d cached tokens; 4 calls back to back per event pair (5.8 GB each: nothing is served from L2)" % (len(dec), kv_tok),
-              "bytes_per_launch": dec_bytes, "ms": ms_dec, "ms_min": ms_dec_min, "peak_source": peaks["source"]}
+              "bytes_per_launch": dec_bytes, "ms": ms_dec, "ms_min": ms_dec_min, "peak_source": peaks["source"],
+              "frac_of_nominal_7700": dec_bytes / (ms_dec * 1e-3) / 1e9 / 7700.0,
+              "note": "the measured peak is a COPY (half reads, half writes); this kernel only reads, pays no read/write bus "
+                      "turnaround and can exceed it: the fraction of the 7.7 TB/s HGX datasheet figure is given beside it"}
     # ---- the mixed call (4 chunks x 2048 + 64 decode rows) for context
     if rd.workspace is None:
         rd.workspace = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(pool, rd.sids, rd.indptr), 256), dtype=torch.uint8, device=dev)
