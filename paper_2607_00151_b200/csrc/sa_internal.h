@@ -12,7 +12,10 @@
 namespace sa {
 
 constexpr int kMetaRing = 8;            // per-call metadata slabs in flight
-constexpr int kDecodeSplitKeys = 1024;  // split-KV granularity of decode-like rows (logical keys)
+#ifndef SA_DEC_SPLIT
+#define SA_DEC_SPLIT 1024
+#endif
+constexpr int kDecodeSplitKeys = SA_DEC_SPLIT;  // split-KV granularity of decode-like rows (logical keys)
 constexpr int kLegacyTileM = 64;        // packed rows per CTA of the mma.sync prefill kernel
 constexpr int kTc5TileM = 256;          // packed rows per CTA of the tcgen05 prefill kernel
 constexpr int kMaxChunkLatency = 2048;  // sa_latency_table prefill chunk size
