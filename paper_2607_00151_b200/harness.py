@@ -52,9 +52,12 @@ def make_pool(w: Workload, device: int = 0, page_order="random", sentinel: Optio
 
 class Runner:
     def __init__(self, w: Workload, pool: sa.Pool, data: Optional[Dict[int, tuple]] = None, device: int = 0,
-                 scale: Optional[float] = None, want_lse: bool = True, lazy: bool = False):
+                 scale: Optional[float] = None, want_lse: bool = True, lazy: bool = False, transform=None):
         """lazy=True (config 5): raw inputs are generated session by session inside fill_prefixes and only
-        the new tokens' k, v, q are kept, so the 45 GB of raw prefix inputs are never resident at once."""
+        the new tokens' k, v, q are kept, so the 45 GB of raw prefix inputs are never resident at once.
+        transform (lazy only): callable (k, v, q) -> (k, v, q) applied to each generated session (the
+        closed-form tests zero Q and rescale V this way)."""
+        self.transform = transform
         self.w, self.pool, self.device = w, pool, device
         self.dev = torch.device("cuda:%d" % device)
         self.scale, self.lazy = scale, lazy
@@ -79,6 +82,8 @@ class Runner:
         if self.lazy:
             for i, s in enumerate(self.w.sessions):
                 k, v, q = gen_session(self.w, i, self.dev, self.scale)
+                if self.transform is not None:
+                    k, v, q = self.transform(k, v, q)
                 if s.prefix > 0:
                     sa.sa_rope_kv_append(self.pool, [self.sids[i]], [0, s.prefix], k[: s.prefix].contiguous(),
                                          v[: s.prefix].contiguous(), None)
