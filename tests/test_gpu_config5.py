@@ -42,7 +42,9 @@ def test_config5_long_horizon_sampled():
     rng = np.random.default_rng(55)
     pre = sorted(range(8), key=lambda i: -w.sessions[i].prefix)
     dec = sorted(range(8, 136), key=lambda i: -w.sessions[i].prefix)
-    sample = [pre[0], pre[-1], dec[0], dec[len(dec) // 2]]   # longest + shortest prefill, longest + median decode
+    # reading R16: all 8 prefill sessions (first + last row and 254 random (row, head) pairs each) and 16 decode rows
+    # (every head): the longest, the shortest and 14 seeded others
+    sample = pre + [dec[0], dec[-1]] + [dec[j] for j in rng.choice(np.arange(1, len(dec) - 1), size=14, replace=False)]
     for i in sample:
         s = w.sessions[i]
         data = {i: gen_session(w, i, "cuda")}
@@ -50,8 +52,8 @@ def test_config5_long_horizon_sampled():
             rows = np.zeros(64, dtype=np.int64)
             heads = np.arange(64, dtype=np.int32)
         else:
-            rows = np.concatenate([[0, s.new - 1], rng.integers(0, s.new, size=30)])
-            heads = rng.integers(0, 64, size=32).astype(np.int32)
+            rows = np.concatenate([[0, s.new - 1], rng.integers(0, s.new, size=254)])
+            heads = rng.integers(0, 64, size=256).astype(np.int32)
         ref = oracle_session(w, i, data, rows=rows, heads=heads)
         del data
         g = outs[i][0][torch.as_tensor(rows), torch.as_tensor(heads.astype(np.int64))]
