@@ -31,11 +31,11 @@ namespace {
 
 using namespace ptx;
 
-constexpr int D = 128;            // head_dim of this kernel
+constexpr int DMAX = 128;         // largest head_dim; the kernels are instantiated for DH = 1 or 2 halves of 64 dims
 constexpr int BM = 128;           // rows per Q tile
 constexpr int BN = 128;           // keys per KV tile
 constexpr int kThreadsTc5 = 384;
-constexpr int TILE_BYTES = BN * D * 2;   // 32 KiB: two 64-wide halves of 128 rows x 128 B
+constexpr int TILE_BYTES = BN * DMAX * 2;   // 32 KiB: two 64-wide halves of 128 rows x 128 B (head_dim 64 uses the first)
 constexpr int HALF_BYTES = TILE_BYTES / 2;
 constexpr int KV_STAGES = 2;
 #ifndef SA_POLY_SHARE
@@ -168,11 +168,12 @@ __device__ __forceinline__ void publish_p(uint32_t bar_addr) {
     mbar_arrive(bar_addr);
 }
 
-template <int LOG2B>
+template <int LOG2B, int DH>
 __global__ void __launch_bounds__(kThreadsTc5, 1)
 prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                    const __grid_constant__ CUtensorMap tmap_v, const Tc5Args a) {
     constexpr int B = 1 << LOG2B;
+    constexpr int D = DH * 64;                     // head_dim: DH halves of 64 dims (one SWIZZLE_128B atom each)
     constexpr int PAGES_PER_TILE = BN / B;
     constexpr uint32_t PAGE_HALF_BYTES = B * 128;  // one page, one 64-wide half: B rows x 128 B
 
@@ -238,12 +239,12 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 const PartGeom gm = load_part<LOG2B>(a, p);
                 // Q of this part may land once every QK product of the previous part has read its Q
                 if (p > pb) mbar_wait(bar(BAR_Q_EMPTY), (p - pb - 1) & 1);
-                mbar_expect_tx(bar(BAR_Q_FULL), 2 * TILE_BYTES);
+                mbar_expect_tx(bar(BAR_Q_FULL), 2 * DH * HALF_BYTES);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
                     const int tok0 = gm.r.q_start + ((gm.rho0 + t * BM) >> a.log2G);
 #pragma unroll
-                    for (int h = 0; h < 2; ++h)
+                    for (int h = 0; h < DH; ++h)
                         tma_load_3d(sQ + t * TILE_BYTES + h * HALF_BYTES, &tmap_q, bar(BAR_Q_FULL), h * 64, gm.g << a.log2G, tok0);
                 }
                 const int32_t *bt = a.block_table + int64_t(gm.r.sid) * a.mpps;
@@ -255,20 +256,20 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
 #pragma unroll
                     for (int u = 0; u < PAGES_PER_TILE; ++u) pg[u] = u < np ? __ldg(bt + p0 + u) : 0;
                     mbar_wait(bar(BAR_K_EMPTY + s), ph ^ 1);
-                    mbar_expect_tx(bar(BAR_K_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
+                    mbar_expect_tx(bar(BAR_K_FULL + s), uint32_t(np) * DH * PAGE_HALF_BYTES);
 #pragma unroll
                     for (int u = 0; u < PAGES_PER_TILE; ++u)
                         if (u < np) {
                             tma_load_4d(sK + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 0, 0, gm.g, pg[u]);
-                            tma_load_4d(sK + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 64, 0, gm.g, pg[u]);
+                            if (DH == 2) tma_load_4d(sK + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 64, 0, gm.g, pg[u]);
                         }
                     mbar_wait(bar(BAR_V_EMPTY + s), ph ^ 1);
-                    mbar_expect_tx(bar(BAR_V_FULL + s), uint32_t(np) * 2 * PAGE_HALF_BYTES);
+                    mbar_expect_tx(bar(BAR_V_FULL + s), uint32_t(np) * DH * PAGE_HALF_BYTES);
 #pragma unroll
                     for (int u = 0; u < PAGES_PER_TILE; ++u)
                         if (u < np) {
                             tma_load_4d(sV + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 0, 0, gm.g, pg[u]);
-                            tma_load_4d(sV + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 64, 0, gm.g, pg[u]);
+                            if (DH == 2) tma_load_4d(sV + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_v, bar(BAR_V_FULL + s), 64, 0, gm.g, pg[u]);
                         }
                 }
             }
@@ -294,7 +295,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             const uint64_t dv = umma_desc_adv(dv0, s * TILE_BYTES);
 #pragma unroll
             for (int ks = ks0; ks < ks0 + nks; ++ks)
-                umma_ts(tmem + 2 * BN + t * D, tmem + t * BN + ks * 8, umma_desc_adv(dv, ks * 2048), idesc_pv, acc || ks > ks0);
+                umma_ts(tmem + 2 * BN + t * DMAX, tmem + t * BN + ks * 8, umma_desc_adv(dv, ks * 2048), idesc_pv, acc || ks > ks0);
         };
         // S_t of the first KV tile of a part; `single`: that tile is also the part's last, so its
         // second QK product is the last reader of the part's Q
@@ -327,9 +328,9 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 mbar_wait(bar(BAR_V_FULL + s), ph);
                 if (last && gm.fix_last) {
                     // V rows that hold no session data must be exactly zero: P is 0 there, and 0 * NaN = NaN
-                    const int n_zero = BN - gm.valid_last;  // rows [valid_last, 128), 2 halves x 8 chunks of 16 B each
-                    for (int e = lane; e < n_zero * 16; e += 32) {
-                        const int row = gm.valid_last + (e >> 4), hc = e & 15;
+                    const int n_zero = BN - gm.valid_last;  // rows [valid_last, 128), DH halves x 8 chunks of 16 B each
+                    for (int e = lane; e < n_zero * (8 * DH); e += 32) {
+                        const int row = gm.valid_last + e / (8 * DH), hc = e % (8 * DH);
                         const uint32_t addr = sV + s * TILE_BYTES + (hc >> 3) * HALF_BYTES + row * 128 + (hc & 7) * 16;
                         asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(addr), "r"(0) : "memory");
                     }
@@ -387,7 +388,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
         const int t = (warp - 4) >> 2;                 // Q tile of this warpgroup
         const int row = ((warp & 3) << 5) + lane;      // TMEM lane == row of the tile
         const uint32_t lane_addr = tmem + (uint32_t((warp & 3) << 5) << 16);
-        const uint32_t tS = lane_addr + t * BN, tO = lane_addr + 2 * BN + t * D;
+        const uint32_t tS = lane_addr + t * BN, tO = lane_addr + 2 * BN + t * DMAX;
         const float sl2 = a.scale_log2;
         const uint64_t sl2_2 = pack_f32x2(sl2, sl2);
         const int G = 1 << a.log2G;
@@ -431,7 +432,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                     }
                     if (j > gm.u0) {  // PV(t, j-1) has completed (it precedes QK(t, j) in the pipe); PV(t, j) waits for P
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) {
+                        for (int c = 0; c < D / 32; ++c) {
                             uint32_t rr[32];
                             tmem_ld32(tO + c * 32, rr);
                             tmem_wait_ld();
@@ -488,11 +489,11 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 const int tok = rho >> a.log2G, hq = (gm.g << a.log2G) + (rho & (G - 1));
                 const int64_t orow = int64_t(gm.r.q_start + tok) * a.Hq + hq;
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
+                for (int c = 0; c < D / 32; ++c) {
                     uint32_t rr[32];
                     tmem_ld32(tO + c * 32, rr);
                     tmem_wait_ld();
-                    if (c == 3) {  // O_t is in registers: the next part's PV products may overwrite it
+                    if (c == D / 32 - 1) {  // O_t is in registers: the next part's PV products may overwrite it
                         tc_fence_before();
                         mbar_arrive(bar(BAR_O_EMPTY + t));
                     }
@@ -515,14 +516,14 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             } else {
                 // part of a split item: unnormalised O, running max (log2 domain) and row sum to the partial slot
                 char *slot = a.partials + size_t(gm.slot) * kTc5SlotBytes;
-                float *po = reinterpret_cast<float *>(slot) + size_t(t * BM + row) * D;
-                float2 *pml = reinterpret_cast<float2 *>(slot + size_t(2 * BM) * D * 4) + (t * BM + row);
+                float *po = reinterpret_cast<float *>(slot) + size_t(t * BM + row) * DMAX;   // slot layout is head_dim-independent
+                float2 *pml = reinterpret_cast<float2 *>(slot + size_t(2 * BM) * DMAX * 4) + (t * BM + row);
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
+                for (int c = 0; c < D / 32; ++c) {
                     uint32_t rr[32];
                     tmem_ld32(tO + c * 32, rr);
                     tmem_wait_ld();
-                    if (c == 3) {
+                    if (c == D / 32 - 1) {
                         tc_fence_before();
                         mbar_arrive(bar(BAR_O_EMPTY + t));
                     }
@@ -550,7 +551,9 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
 // Merge of the parts of split items, in KV order (fixed, so bit-reproducible).  grid = (split
 // items, 32): each CTA takes 8 of the item's 256 rows, one row per warp, lanes cover D with float4;
 // the loads of up to four parts are issued together (the kernel is latency-bound otherwise).
+template <int DH>
 __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
+    constexpr int D = DH * 64;
     const Tc5Merge mg = a.merges[blockIdx.x];
     const ReqMeta r = a.reqs[mg.req];
     const int G = 1 << a.log2G;
@@ -560,8 +563,8 @@ __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
     const int lrow = blockIdx.y * 8 + warp;
     const int rho = mg.tile * (2 * BM) + lrow;
     if (rho >= n_rows) return;
-    auto ml_of = [&](int s) { return reinterpret_cast<const float2 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(2 * BM) * D * 4)[lrow]; };
-    auto o_of = [&](int s) { return reinterpret_cast<const float4 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(lrow) * D * 4)[lane]; };
+    auto ml_of = [&](int s) { return reinterpret_cast<const float2 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(2 * BM) * DMAX * 4)[lrow]; };
+    auto o_of = [&](int s) { return reinterpret_cast<const float4 *>(slot0 + size_t(s) * kTc5SlotBytes + size_t(lrow) * DMAX * 4)[lane]; };
     float M = -INFINITY;
     for (int s = 0; s < mg.n_parts; ++s) M = fmaxf(M, ml_of(s).x);
     const float Mb = (M == -INFINITY) ? 0.f : M;
@@ -574,7 +577,7 @@ __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
         for (int u = 0; u < 4; ++u)
             if (s0 + u < mg.n_parts) {
                 ml[u] = ml_of(s0 + u);
-                ov[u] = o_of(s0 + u);
+                ov[u] = lane < D / 4 ? o_of(s0 + u) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
 #pragma unroll
         for (int u = 0; u < 4; ++u)  // KV order
@@ -594,7 +597,7 @@ __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
     uint2 pk;
     pk.x = *reinterpret_cast<uint32_t *>(&lo);
     pk.y = *reinterpret_cast<uint32_t *>(&hi);
-    *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
+    if (lane < D / 4) *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
     if (a.lse && lane == 0) a.lse[orow] = (M + log2f(L)) * 0.6931471805599453f;
 }
 
@@ -629,12 +632,20 @@ extern "C" __attribute__((visibility("default"))) int32_t sa_debug_tc5_probe(uns
 
 void *tensor_map_encode_fn() { return reinterpret_cast<void *>(get_encode()); }
 
+// the instantiation for a (page size, head_dim) pair; nullptr if there is none
+static const void *tc5_kernel_of(int page_size, int head_dim) {
+    if (page_size == 64) return head_dim == 128 ? (const void *)prefill_tc5_kernel<6, 2> : (const void *)prefill_tc5_kernel<6, 1>;
+    if (page_size == 16) return head_dim == 128 ? (const void *)prefill_tc5_kernel<4, 2> : (const void *)prefill_tc5_kernel<4, 1>;
+    return nullptr;
+}
+
 int32_t tc5_init(sa_kv_pool *pool) {
     pool->tc5_ready = false;
-    if (pool->cfg.head_dim != D) return SA_OK;  // head_dim 64 stays on the mma.sync kernel
+    if (pool->cfg.head_dim != 64 && pool->cfg.head_dim != 128) return SA_OK;
     EncodeTiledFn enc = get_encode();
     if (!enc) return SA_ERR_CUDA;
     const sa_kv_pool_config &c = pool->cfg;
+    const cuuint64_t D = cuuint64_t(c.head_dim);
     cuuint64_t dims[4] = {cuuint64_t(D), cuuint64_t(c.page_size), cuuint64_t(c.num_kv_heads), cuuint64_t(c.num_pages)};
     cuuint64_t strides[3] = {cuuint64_t(D) * 2, cuuint64_t(c.page_size) * D * 2,
                              cuuint64_t(c.num_kv_heads) * c.page_size * D * 2};
@@ -646,17 +657,17 @@ int32_t tc5_init(sa_kv_pool *pool) {
                           CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (rc != CUDA_SUCCESS) return SA_ERR_CUDA;
     }
-    cudaError_t e = pool->cfg.page_size == 64
-                        ? cudaFuncSetAttribute(prefill_tc5_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemTc5))
-                        : cudaFuncSetAttribute(prefill_tc5_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemTc5));
-    if (e != cudaSuccess) return SA_ERR_CUDA;
+    const void *fn = tc5_kernel_of(c.page_size, c.head_dim);
+    if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemTc5)) != cudaSuccess) return SA_ERR_CUDA;
     pool->tc5_ready = true;
     return SA_OK;
 }
 
 // Host-only pools (no device) report the same routing a device pool of this shape would use, so
 // the planner can be tested without a GPU.
-bool tc5_supported(const sa_kv_pool *pool) { return pool->host_only ? pool->cfg.head_dim == D : pool->tc5_ready; }
+bool tc5_supported(const sa_kv_pool *pool) {
+    return pool->host_only ? (pool->cfg.head_dim == 64 || pool->cfg.head_dim == 128) : pool->tc5_ready;
+}
 
 cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
                                const Tc5Schedule &sched, const char *sched_dev, char *partials,
@@ -668,6 +679,7 @@ cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
     const sa_kv_pool_config &c = pool->cfg;
     // Q as [T][Hq][D]; one box = 64 dims x G heads x 128/G tokens = a 128-row packed tile half
     alignas(64) CUtensorMap tq;
+    const cuuint64_t D = cuuint64_t(c.head_dim);
     cuuint64_t dims[3] = {cuuint64_t(D), cuuint64_t(c.num_q_heads), cuuint64_t(total_q)};
     cuuint64_t strides[2] = {cuuint64_t(D) * 2, cuuint64_t(c.num_q_heads) * D * 2};
     cuuint32_t box[3] = {64, cuuint32_t(pool->G), cuuint32_t(BM / pool->G)};
@@ -696,15 +708,20 @@ cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
     a.scale_log2 = sm_scale * 1.4426950408889634f;
     const CUtensorMap &tk = *reinterpret_cast<const CUtensorMap *>(pool->tmap_k);
     const CUtensorMap &tv = *reinterpret_cast<const CUtensorMap *>(pool->tmap_v);
-    if (c.page_size == 64)
-        prefill_tc5_kernel<6><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+    if (c.page_size == 64 && c.head_dim == 128)
+        prefill_tc5_kernel<6, 2><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+    else if (c.page_size == 64)
+        prefill_tc5_kernel<6, 1><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+    else if (c.head_dim == 128)
+        prefill_tc5_kernel<4, 2><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
     else
-        prefill_tc5_kernel<4><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        prefill_tc5_kernel<4, 1><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
     ++*launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (!sched.merges.empty()) {
-        tc5_merge_kernel<<<dim3(unsigned(sched.merges.size()), 32), 256, 0, stream>>>(a);
+        if (c.head_dim == 128) tc5_merge_kernel<2><<<dim3(unsigned(sched.merges.size()), 32), 256, 0, stream>>>(a);
+        else tc5_merge_kernel<1><<<dim3(unsigned(sched.merges.size()), 32), 256, 0, stream>>>(a);
         ++*launches;
         e = cudaGetLastError();
     }

@@ -102,6 +102,8 @@ def test_cfg1_attention_parity_and_decomposability():
     out, lse, _ = r.outputs()[0]
     check_out(out, ref["o"], "cfg1 cached")
     check_lse(lse, ref["lse"], 1e-2, "cfg1 cached")
+    # head_dim 64 / page 16 runs on the tcgen05 kernel too (one 64-dim half per tile), not on an mma.sync fallback
+    assert sa.sa_mixed_attention_plan(pool, r.rounds[0].sids, r.rounds[0].indptr)["tcgen05"] == 1
     # P3a on the GPU: one-shot prefill of the whole 384-token context gives the same rows
     w_full = copy.deepcopy(w)
     w_full.sessions = [SessionSpec(0, 384)]
