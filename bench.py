@@ -268,7 +268,7 @@ def measure_parts(local: int, peaks, iters: int = 10):
     dec_bytes = float(kappa) * kv_tok + 2.0 * q.numel() * 2
     decode = {"bound": "hbm", "achieved": dec_bytes / (ms_dec * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
               "frac": dec_bytes / (ms_dec * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": load_traffic().get("flash_mma_decode_cfg4"),
-              "kernel": "flash_mma_kernel<128,0> (split-KV decode) + merge_splits_kernel on config 4's %d decode rows, "
+              "kernel": "flash_mma_kernel<128> (split-KV decode) + merge_splits_kernel on config 4's %d decode rows, "
                         "%d cached tokens; 4 calls back to back per event pair (5.8 GB each: nothing is served from L2)" % (len(dec), kv_tok),
               "bytes_per_launch": dec_bytes, "ms": ms_dec, "ms_min": ms_dec_min, "peak_source": peaks["source"],
               "frac_of_nominal_7700": dec_bytes / (ms_dec * 1e-3) / 1e9 / 7700.0,

@@ -173,12 +173,12 @@ SA_API int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t
  * on host-only pools).  out_stats (host int64[8]) = { decode-like requests, prefill requests,
  * decode CTAs, prefill work items (parts of the schedule on the tcgen05 path), split partial rows, sum_j L_j over decode-like requests,
  * sum_j A_j over prefill requests (A_j = q_j*prefix_j + q_j(q_j+1)/2, L313), 1 if prefill chunks
- * run on the tcgen05 kernel else 0 }. */
+ * run on the tcgen05 kernel (always, for the supported shapes) }. */
 SA_API int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                 const int32_t *qo_indptr, int64_t *out_stats);
 
 /* The static schedule the tcgen05 prefill kernel would run for this batch (host only; works on
- * host-only pools; SA_ERR_UNSUPPORTED when prefill chunks do not take the tcgen05 path).  An item is
+ * host-only pools; every supported shape takes the tcgen05 path).  An item is
  * (request, kv head, tile of 256 packed rows: row rho = token*G + head-in-group); its cost is n_kv =
  * the number of 128-key tiles it attends to (the causal work A_j of L313 in tiles).  Items are
  * assigned to one persistent CTA per SM; an item that does not fit under the balanced makespan is

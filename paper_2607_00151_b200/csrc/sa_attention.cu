@@ -35,8 +35,9 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
     if (n_req == 0) return SA_OK;
     if (!sids || !qo_indptr || qo_indptr[0] != 0 || n_req > pool->cfg.max_sessions) return SA_ERR_INVALID_ARG;
     const int G = pool->G, Hq = pool->cfg.num_q_heads, Hkv = pool->cfg.num_kv_heads;
-    hp->use_tc5 = tc5_supported(pool);
-    const int tile_m = hp->use_tc5 ? kTc5TileM : kLegacyTileM;
+    hp->use_tc5 = tc5_supported(pool);  // every supported shape (head_dim 64 / 128, page 16 / 64) has a tcgen05 instantiation
+    if (!hp->use_tc5) return SA_ERR_UNSUPPORTED;
+    const int tile_m = kTc5TileM;
     std::vector<std::pair<ReqMeta, int32_t>> pre;
     for (int r = 0; r < n_req; ++r) {
         const int32_t sid = sids[r];
@@ -91,7 +92,7 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
     if (items > INT32_MAX) return SA_ERR_UNSUPPORTED;
     hp->plan.n_pre = int32_t(hp->pre.size());
     hp->plan.pre_items = int32_t(items);
-    if (hp->use_tc5 && !hp->pre.empty()) {
+    if (!hp->pre.empty()) {
         tc5_schedule(hp->pre, G, Hkv, pool->num_sms, &hp->sched);
         hp->plan.pre_items = int32_t(hp->sched.parts.size());
     }
@@ -250,11 +251,8 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
 
     // prefill first: it is the long pole; the decode kernel fills in behind it on the same stream
     cudaError_t e;
-    if (hp.use_tc5)
-        e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.sched, sched_dev, tc5_partials, hp.total_q, q, out, lse, sm_scale,
-                               stream, &pool->last_launches);
-    else
-        e = launch_flash_prefill_legacy(pool, pre_dev, hp.plan, q, out, lse, sm_scale, stream, &pool->last_launches);
+    e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.sched, sched_dev, tc5_partials, hp.total_q, q, out, lse, sm_scale,
+                           stream, &pool->last_launches);
     if (e != cudaSuccess) return SA_ERR_CUDA;
     e = launch_flash_decode(pool, dec_dev, hp.plan, q, out, lse, sm_scale, part_o, part_lse, stream, &pool->last_launches);
     if (e != cudaSuccess) return SA_ERR_CUDA;

@@ -1,11 +1,10 @@
-// sa_flash_mma.cu -- attention over paged KV on the warp-level tensor path (mma.sync m16n8k16):
-//   * decode-like rows (q_len * G <= 16): split-KV, HBM-bound.  One CTA per (request, kv head,
-//     1024-key split); the G query heads of the group are the M rows of the MMA so K/V are read
-//     once per group; 4 warps take 16 keys each of every 64-key tile; cp.async 3-stage ring of
-//     page-gathered tiles; deterministic merge of the splits ("a single query
-//     token that attends to its full KV cache of length L_j ... memory-bandwidth bound").
-//   * prefill chunks that the tcgen05 kernel does not take (head_dim 64, or no tcgen05 path):
-//     64 packed rows per CTA, flash-style online softmax.
+// sa_flash_mma.cu -- decode attention over paged KV on the warp-level tensor path (mma.sync m16n8k16):
+// decode-like rows (q_len * G <= 16), split-KV, HBM-bound.  One CTA per (request, kv head, 1024-key
+// split); the G query heads of the group are the M rows of the MMA so K/V are read once per group;
+// 4 warps take 16 keys each of every 64-key tile; cp.async 3-stage ring of page-gathered tiles;
+// deterministic merge of the splits ("a single query token that attends to its full
+// KV cache of length L_j ... memory-bandwidth bound").  Prefill chunks run on the tcgen05 kernel
+// (sa_prefill_tc5.cu) for every supported head_dim.
 // Packed rows: row rho of a (request, kv head g) pair is (token rho / G, q head g*G + rho % G).
 #include <cuda_bf16.h>
 #include <math.h>
@@ -233,11 +232,11 @@ __device__ __forceinline__ void load_q_tile(const AttnArgs &a, const ReqMeta &r,
 }
 
 // ------------------------------------------------------------------------------------------
-// MODE 0: decode-like, split-KV, partials out.   MODE 1: prefill, 64 packed rows, direct out.
-template <int D, int MODE>
+// Decode-like rows: split-KV, partials out.
+template <int D>
 __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
-    constexpr int BM = MODE == 0 ? 16 : kLegacyTileM;
+    constexpr int BM = 16;
     constexpr int TILE_BYTES = kBN * D * 2;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t s_base = smem_u32(smem);
@@ -249,21 +248,10 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
     const int local = item - r.item_begin;
     const int G = 1 << a.log2G;
     const int n_rows = r.q_len * G;
-    int g, rho0, k_begin, k_end, split = 0;
-    if (MODE == 0) {
-        g = local / r.n_splits;
-        split = local % r.n_splits;
-        rho0 = 0;
-        k_begin = split * kDecodeSplitKeys;
-        k_end = min(r.kv_len, k_begin + kDecodeSplitKeys);
-    } else {
-        const int tile = r.n_tiles - 1 - local / a.Hkv;  // heavy (late) tiles first
-        g = local % a.Hkv;
-        rho0 = tile * BM;
-        k_begin = 0;
-        const int tok_max = min(r.q_len - 1, (rho0 + BM - 1) >> a.log2G);
-        k_end = r.kv_len - r.q_len + tok_max + 1;
-    }
+    const int g = local / r.n_splits, split = local % r.n_splits;
+    constexpr int rho0 = 0;
+    const int k_begin = split * kDecodeSplitKeys;
+    const int k_end = min(r.kv_len, k_begin + kDecodeSplitKeys);
     KvView kv;
     kv.k_base = a.k_base;
     kv.v_base = a.v_base;
@@ -283,7 +271,7 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
     }
     load_q_tile<D, BM>(a, r, g, rho0, n_rows, sQ, tid);
     __syncthreads();
-    const int row_base = MODE == 0 ? 0 : warp * 16;
+    constexpr int row_base = 0;
     uint32_t qf[D / 16][4];
     {
         const int mi = lane >> 3, rr = lane & 7;
@@ -320,15 +308,10 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
         const int st = t % kStages;
         const uint32_t sK = s_base + st * 2 * TILE_BYTES, sV = sK + TILE_BYTES;
         const int kt = k_begin + t * kBN;
-        if (MODE == 0) {
-            const int key_off = warp * 16;
-            if (kt + key_off < k_end) {  // warp-uniform: this warp's 16 keys hold at least one live key
-                const bool need_mask = kt + key_off + 15 > lim_min;
-                warp_step<D, 1>(qf, sK, sV, key_off, kt, lim0, lim1, need_mask, a.scale_log2, o, m0, m1, l0, l1, lane);
-            }
-        } else {
-            const bool need_mask = kt + kBN - 1 > lim_min;
-            warp_step<D, 4>(qf, sK, sV, 0, kt, lim0, lim1, need_mask, a.scale_log2, o, m0, m1, l0, l1, lane);
+        const int key_off = warp * 16;
+        if (kt + key_off < k_end) {  // warp-uniform: this warp's 16 keys hold at least one live key
+            const bool need_mask = kt + key_off + 15 > lim_min;
+            warp_step<D, 1>(qf, sK, sV, key_off, kt, lim0, lim1, need_mask, a.scale_log2, o, m0, m1, l0, l1, lane);
         }
     }
     cp_async_wait<0>();
@@ -337,28 +320,7 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
     l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
     l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
 
-    if (MODE == 1) {
-        const float inv0 = l0 > 0.f ? 1.f / l0 : 0.f, inv1 = l1 > 0.f ? 1.f / l1 : 0.f;
-#pragma unroll
-        for (int half = 0; half < 2; ++half) {
-            const int rho = half ? rB : rA;
-            if (rho >= n_rows) continue;
-            const int tok = rho >> a.log2G, hq = (g << a.log2G) + (rho & (G - 1));
-            const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
-            __nv_bfloat16 *op = a.out + orow * D + 2 * (lane & 3);
-            const float inv = half ? inv1 : inv0;
-#pragma unroll
-            for (int nt = 0; nt < D / 8; ++nt)
-                *reinterpret_cast<uint32_t *>(op + nt * 8) = pack_bf16(o[nt][half * 2] * inv, o[nt][half * 2 + 1] * inv);
-            if (a.lse && (lane & 3) == 0) {
-                const float m = half ? m1 : m0, l = half ? l1 : l0;
-                a.lse[orow] = (m + log2f(l)) * 0.6931471805599453f;
-            }
-        }
-        return;
-    }
-
-    // ---- MODE 0: merge the four warps' states (each saw a disjoint quarter of every tile)
+    // ---- merge the four warps' states (each saw a disjoint quarter of every tile)
     __syncthreads();  // everyone is done with the stage buffers
     float *sO = reinterpret_cast<float *>(smem);             // [4][16][D]
     float *sM = sO + 4 * 16 * D;                             // [4][16]
@@ -474,18 +436,18 @@ AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const
     return a;
 }
 
-template <int D, int MODE>
+template <int D>
 cudaError_t launch_flash(const AttnArgs &a, int items, cudaStream_t stream) {
-    constexpr int BM = MODE == 0 ? 16 : kLegacyTileM;
+    constexpr int BM = 16;
     constexpr size_t smem = size_t(kStages) * 2 * kBN * D * 2 + size_t(BM) * D * 2;
     static_assert(smem >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(flash_mma_kernel<D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+        cudaError_t e = cudaFuncSetAttribute(flash_mma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    flash_mma_kernel<D, MODE><<<unsigned(items), kThreads, smem, stream>>>(a);
+    flash_mma_kernel<D><<<unsigned(items), kThreads, smem, stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -496,8 +458,8 @@ cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
                                 float *part_lse, cudaStream_t stream, int32_t *launches) {
     if (plan.dec_items == 0) return cudaSuccess;
     AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
-    cudaError_t e = pool->cfg.head_dim == 128 ? launch_flash<128, 0>(a, plan.dec_items, stream)
-                                              : launch_flash<64, 0>(a, plan.dec_items, stream);
+    cudaError_t e = pool->cfg.head_dim == 128 ? launch_flash<128>(a, plan.dec_items, stream)
+                                              : launch_flash<64>(a, plan.dec_items, stream);
     if (e != cudaSuccess) return e;
     ++*launches;
     dim3 grid(unsigned(plan.n_dec), unsigned(pool->cfg.num_kv_heads));
@@ -505,17 +467,6 @@ cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
     else merge_splits_kernel<64><<<grid, 128, 0, stream>>>(a);
     ++*launches;
     return cudaGetLastError();
-}
-
-cudaError_t launch_flash_prefill_legacy(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
-                                        const void *q, void *out, float *lse, float sm_scale, cudaStream_t stream,
-                                        int32_t *launches) {
-    if (plan.pre_items == 0) return cudaSuccess;
-    AttnArgs a = make_args(pool, reqs_dev, plan.n_pre, q, out, lse, sm_scale, nullptr, nullptr);
-    cudaError_t e = pool->cfg.head_dim == 128 ? launch_flash<128, 1>(a, plan.pre_items, stream)
-                                              : launch_flash<64, 1>(a, plan.pre_items, stream);
-    if (e == cudaSuccess) ++*launches;
-    return e;
 }
 
 }  // namespace sa

@@ -16,7 +16,6 @@ constexpr int kMetaRing = 8;            // per-call metadata slabs in flight
 #define SA_DEC_SPLIT 1024
 #endif
 constexpr int kDecodeSplitKeys = SA_DEC_SPLIT;  // split-KV granularity of decode-like rows (logical keys)
-constexpr int kLegacyTileM = 64;        // packed rows per CTA of the mma.sync prefill kernel
 constexpr int kTc5TileM = 256;          // packed rows per CTA of the tcgen05 prefill kernel
 constexpr int kMaxChunkLatency = 2048;  // sa_latency_table prefill chunk size
 constexpr int kTc5KeysPerUnit = 128;    // one schedule unit of the tcgen05 kernel = one 128-key KV tile of an item
@@ -167,10 +166,6 @@ struct AttnPlan {
 cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
                                 const void *q, void *out, float *lse, float sm_scale, float *part_o,
                                 float *part_lse, cudaStream_t stream, int32_t *launches);
-cudaError_t launch_flash_prefill_legacy(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
-                                        const AttnPlan &plan, const void *q, void *out, float *lse,
-                                        float sm_scale, cudaStream_t stream, int32_t *launches);
-
 // dense operators of the layer (sa_gemm_tc5.cu); each returns an SA_* status
 int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
                    void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches);

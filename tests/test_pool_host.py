@@ -100,11 +100,9 @@ def test_planner_classes_and_sums():
     assert st["partial_rows"] == 20 * 1 * 32 + 3 * 3 * 32    # [split][token][head]
     assert st["sum_decode_kv"] == 20480 * 1 + 3000 * 3
     assert st["sum_prefill_A"] == 2048 * 8192 + 2048 * 2049 // 2
-    if st["tcgen05"]:
-        parts, sm = sa.sa_mixed_attention_schedule(p, sids, [0, 1, 4, 4 + 2048, 4 + 2048])
-        assert st["prefill_ctas"] == sm["parts"] == len(parts) >= 8 * (2048 * 4 // 256)
-    else:
-        assert st["prefill_ctas"] == 8 * (2048 * 4 // 64)
+    assert st["tcgen05"] == 1   # every supported shape has a tcgen05 instantiation
+    parts, sm = sa.sa_mixed_attention_schedule(p, sids, [0, 1, 4, 4 + 2048, 4 + 2048])
+    assert st["prefill_ctas"] == sm["parts"] == len(parts) >= 8 * (2048 * 4 // 256)
     # a request cannot have more query rows than cached tokens (append first, then attend)
     with pytest.raises(sa.SAError):
         sa.sa_mixed_attention_plan(p, [sids[3]], [0, 6])
