@@ -13,7 +13,6 @@
 // of prefill requests of the call (through the cut points), never on decode rows or on physical
 // pages; the same call always gives the same bits.
 #include <algorithm>
-#include <queue>
 
 #include "sa_internal.h"
 
@@ -31,6 +30,11 @@ void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc
         int32_t req, g, tile, n_kv;
     };
     std::vector<Item> items;
+    {
+        size_t n_items = 0;
+        for (const ReqMeta &r : pre) n_items += size_t(Hkv) * size_t((int64_t(r.q_len) * G + kTc5TileM - 1) / kTc5TileM);
+        items.reserve(n_items);
+    }
     for (size_t ri = 0; ri < pre.size(); ++ri) {
         const ReqMeta &r = pre[ri];
         const int64_t n_rows = int64_t(r.q_len) * G;
@@ -54,18 +58,37 @@ void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc
     int64_t T = (out->total_units + F * (int64_t(items.size()) + n_cta) + n_cta - 1) / n_cta;
     T = std::max<int64_t>(T, kTc5MinPart + F);
 
-    typedef std::pair<int64_t, int32_t> Load;  // (load, cta): least loaded first, ties by CTA index
-    std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-    for (int c = 0; c < n_cta; ++c) heap.push(Load(0, c));
-    std::vector<std::vector<Tc5Part>> per_cta;
-    per_cta.resize(size_t(n_cta));
+    // Min-heap of (load, cta): least loaded first, ties by CTA index (a total order: the top is unique, so the
+    // schedule does not depend on the heap's internal layout).  The only update is "give the top more load".
+    typedef std::pair<int64_t, int32_t> Load;
+    std::vector<Load> heap(static_cast<size_t>(n_cta));
+    for (int c = 0; c < n_cta; ++c) heap[size_t(c)] = Load(0, c);  // ascending: already a heap
+    auto raise_top = [&heap, n_cta](int64_t new_load) {
+        Load x(new_load, heap[0].second);
+        int i = 0;
+        for (;;) {
+            int ch = 2 * i + 1;
+            if (ch >= n_cta) break;
+            if (ch + 1 < n_cta && heap[size_t(ch + 1)] < heap[size_t(ch)]) ++ch;
+            if (!(heap[size_t(ch)] < x)) break;
+            heap[size_t(i)] = heap[size_t(ch)];
+            i = ch;
+        }
+        heap[size_t(i)] = x;
+    };
+    // parts in creation order; grouped by CTA afterwards with a stable counting sort (this runs on the host inside
+    // every sa_mixed_attention call: no per-CTA vectors, no reallocation)
+    std::vector<Tc5Part> flat;
+    flat.reserve(items.size() + size_t(n_cta) + 8);
+    std::vector<int32_t> per_cta_count(size_t(n_cta), 0);
+    out->merges.reserve(size_t(n_cta) + 8);
 
     for (const Item &it : items) {
         int u = 0;
         int first_slot = out->n_slots, n_parts = 0;
         bool split = false;
         while (u < it.n_kv) {
-            Load top = heap.top();
+            const Load top = heap[0];
             const int64_t cap = T - top.first - F;
             const int remaining = it.n_kv - u;
             int take;
@@ -79,7 +102,6 @@ void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc
                 T += kTc5MinPart;  // every CTA is (nearly) full: raise the makespan a little and retry
                 continue;
             }
-            heap.pop();
             Tc5Part p;
             p.req = it.req;
             p.g = it.g;
@@ -90,8 +112,9 @@ void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc
             p.cta = top.second;
             split = split || take < it.n_kv;
             p.slot = split ? out->n_slots++ : -1;
-            per_cta[size_t(top.second)].push_back(p);
-            heap.push(Load(top.first + take + F, top.second));
+            flat.push_back(p);
+            ++per_cta_count[size_t(top.second)];
+            raise_top(top.first + take + F);
             u += take;
             ++n_parts;
         }
@@ -105,16 +128,20 @@ void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc
             out->merges.push_back(m);
         }
     }
+    int32_t run = 0;
     for (int c = 0; c < n_cta; ++c) {
-        out->cta_begin[size_t(c)] = int32_t(out->parts.size());
-        int64_t load = 0;
-        for (const Tc5Part &p : per_cta[size_t(c)]) {
-            out->parts.push_back(p);
-            load += p.u1 - p.u0 + F;
-        }
-        out->makespan = std::max(out->makespan, load);
+        out->cta_begin[size_t(c)] = run;
+        run += per_cta_count[size_t(c)];
     }
-    out->cta_begin[size_t(n_cta)] = int32_t(out->parts.size());
+    out->cta_begin[size_t(n_cta)] = run;
+    out->parts.resize(flat.size());
+    std::vector<int32_t> cursor(out->cta_begin.begin(), out->cta_begin.end() - 1);
+    std::vector<int64_t> load(size_t(n_cta), 0);
+    for (const Tc5Part &p : flat) {  // creation order within a CTA = execution order
+        out->parts[size_t(cursor[size_t(p.cta)]++)] = p;
+        load[size_t(p.cta)] += p.u1 - p.u0 + F;
+    }
+    for (int c = 0; c < n_cta; ++c) out->makespan = std::max(out->makespan, load[size_t(c)]);
 }
 
 }  // namespace sa
