@@ -323,3 +323,28 @@ def test_truncate_then_reprefill_reuses_pages_and_matches():
     for i in range(2):
         assert torch.equal(_bits(a[i]), _bits(r.outputs()[i][0]))
     assert sorted(sum(pages_a, [])) == sorted(sum([sa.sa_kv_session_query(pool, s)[1] for s in r.sids], []))
+
+
+@pytest.mark.parametrize("B,G", [(16, 4), (64, 2)])
+def test_head_dim_64_long_context_stream_k_parts_and_merge(B, G):
+    # head_dim 64 on the tcgen05 kernel (DH = 1) at a size where items are cut along KV and merged: a 1500-row chunk on a
+    # 9000-token prefix, a second ragged session and a decode row, NaN in every unused slot; sampled rows against the oracle
+    sessions = [SessionSpec(9000, 1500), SessionSpec(3001, 700), SessionSpec(5000, 1)]
+    w = _small_l8b(sessions, seed=64, scale=64 ** -0.25, B=B, D=64, Hq=4 * G, Hkv=4)
+    pool, r, data = run_workload(w, sentinel=0x7FC1)
+    st = sa.sa_mixed_attention_plan(pool, r.rounds[0].sids, r.rounds[0].indptr)
+    assert st["tcgen05"] == 1 and st["prefill_requests"] == 2 and st["decode_requests"] == 1
+    parts, sm = sa.sa_mixed_attention_schedule(pool, r.rounds[0].sids, r.rounds[0].indptr)
+    assert sm["split_items"] > 0   # some items are split, so tc5_merge_kernel<1> runs
+    rng = np.random.default_rng(640)
+    for i, s in enumerate(sessions):
+        if s.new == 1:
+            rows, heads = np.zeros(4 * G, dtype=np.int64), np.arange(4 * G, dtype=np.int32)
+        else:
+            rows = np.concatenate([[0, s.new - 1], rng.integers(0, s.new, size=62)])
+            heads = rng.integers(0, 4 * G, size=64).astype(np.int32)
+        ref = oracle_session(w, i, data, rows=rows, heads=heads)
+        out, lse, _ = r.outputs()[i]
+        idx = (torch.as_tensor(rows), torch.as_tensor(heads.astype(np.int64)))
+        check_out(out[idx], ref["o"], "D64 B%d s%d" % (B, i), max_abs=3e-2, mean_abs=3e-3)
+        check_lse(lse[idx], ref["lse"], 1e-2, "D64 B%d s%d" % (B, i))
