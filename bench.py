@@ -312,7 +312,7 @@ def measure_parts(local: int, peaks, iters: int = 10):
                 "export_ms": ms_ex, "export_gbs": xbytes / (ms_ex * 1e-3) / 1e9, "import_ms": ms_im,
                 "import_gbs": xbytes / (ms_im * 1e-3) / 1e9, "bytes_per_pass": xbytes,
                 "note": "config 4's 68 sessions, one sa_kv_session_export / sa_kv_session_import call per session "
-                        "(read kappa + write kappa per token; import includes page allocation and block-table update)"}
+                        "(read kappa + write kappa per token; import includes page allocation and block-table update; a call carries ~29 us of GPU work, so the loop is close to host-bound through the Python binding)"}
     transfer["frac"] = min(transfer["export_gbs"], transfer["import_gbs"]) / peaks["hbm_gbs"]
     for sid in sids2:
         sa.sa_kv_session_close(pool2, sid)

@@ -34,16 +34,31 @@ kv_export_kernel(const __nv_bfloat16 *__restrict__ k_base, const __nv_bfloat16 *
         s_src[threadIdx.x] = int64_t(page) * stride_page + int64_t(pos & ((1 << log2_page) - 1)) * D;
     }
     __syncthreads();
-    const int cpr = D / 8;                      // 16-byte chunks per row
-    const int per_tok = 2 * Hkv * cpr;
-    for (int e = threadIdx.x; e < nt * per_tok; e += kXferThreads) {
-        const int tl = e / per_tok, u = e % per_tok;
-        const int hk = u / cpr, c = u % cpr;    // hk in [0, 2 Hkv): K heads then V heads
-        const bool is_v = hk >= Hkv;
-        const int h = is_v ? hk - Hkv : hk;
-        const __nv_bfloat16 *src = (is_v ? v_base : k_base) + s_src[tl] + int64_t(h) * stride_head + c * 8;
-        __nv_bfloat16 *dst = image + ((int64_t(is_v) * Hkv + h) * n_tok + (t0 + tl)) * D + c * 8;
-        *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+    // 16-byte chunks; D is 64 or 128, so chunk-in-row is a shift.  Four chunks in flight per thread: all loads, then
+    // all stores (one dependent load -> store pair at a time left the kernel latency-bound at 80 % of the copy peak).
+    const int lc = D == 128 ? 4 : 3;            // log2(chunks per row)
+    const int rows = nt * 2 * Hkv;              // (token, K|V head) rows of this CTA
+    const int total = rows << lc;
+    constexpr int U = 4;
+    for (int base = threadIdx.x; base < total; base += kXferThreads * U) {
+        uint4 val[U];
+        __nv_bfloat16 *dst[U];
+#pragma unroll
+        for (int i = 0; i < U; ++i) {
+            const int e = base + i * kXferThreads;
+            dst[i] = nullptr;
+            if (e >= total) continue;
+            const int row = e >> lc, c = e & ((1 << lc) - 1);
+            const int tl = row / (2 * Hkv), hk = row % (2 * Hkv);   // hk in [0, 2 Hkv): K heads then V heads
+            const bool is_v = hk >= Hkv;
+            const int h = is_v ? hk - Hkv : hk;
+            const __nv_bfloat16 *src = (is_v ? v_base : k_base) + s_src[tl] + int64_t(h) * stride_head + c * 8;
+            dst[i] = image + ((int64_t(is_v) * Hkv + h) * n_tok + (t0 + tl)) * D + c * 8;
+            val[i] = *reinterpret_cast<const uint4 *>(src);
+        }
+#pragma unroll
+        for (int i = 0; i < U; ++i)
+            if (dst[i]) *reinterpret_cast<uint4 *>(dst[i]) = val[i];
     }
 }
 
@@ -63,16 +78,29 @@ kv_import_kernel(const ReqMeta *__restrict__ req, __nv_bfloat16 *__restrict__ k_
         s_dst[threadIdx.x] = int64_t(page) * stride_page + int64_t(pos & ((1 << log2_page) - 1)) * D;
     }
     __syncthreads();
-    const int cpr = D / 8;
-    const int per_tok = 2 * Hkv * cpr;
-    for (int e = threadIdx.x; e < nt * per_tok; e += kXferThreads) {
-        const int tl = e / per_tok, u = e % per_tok;
-        const int hk = u / cpr, c = u % cpr;
-        const bool is_v = hk >= Hkv;
-        const int h = is_v ? hk - Hkv : hk;
-        const __nv_bfloat16 *src = image + ((int64_t(is_v) * src_heads + head_begin + h) * n_tok + (t0 + tl)) * D + c * 8;
-        __nv_bfloat16 *dst = (is_v ? v_base : k_base) + s_dst[tl] + int64_t(h) * stride_head + c * 8;
-        *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+    const int lc = D == 128 ? 4 : 3;
+    const int rows = nt * 2 * Hkv;
+    const int total = rows << lc;
+    constexpr int U = 4;   // chunks in flight per thread, as in the export kernel
+    for (int base = threadIdx.x; base < total; base += kXferThreads * U) {
+        uint4 val[U];
+        __nv_bfloat16 *dst[U];
+#pragma unroll
+        for (int i = 0; i < U; ++i) {
+            const int e = base + i * kXferThreads;
+            dst[i] = nullptr;
+            if (e >= total) continue;
+            const int row = e >> lc, c = e & ((1 << lc) - 1);
+            const int tl = row / (2 * Hkv), hk = row % (2 * Hkv);
+            const bool is_v = hk >= Hkv;
+            const int h = is_v ? hk - Hkv : hk;
+            const __nv_bfloat16 *src = image + ((int64_t(is_v) * src_heads + head_begin + h) * n_tok + (t0 + tl)) * D + c * 8;
+            dst[i] = (is_v ? v_base : k_base) + s_dst[tl] + int64_t(h) * stride_head + c * 8;
+            val[i] = *reinterpret_cast<const uint4 *>(src);
+        }
+#pragma unroll
+        for (int i = 0; i < U; ++i)
+            if (dst[i]) *reinterpret_cast<uint4 *>(dst[i]) = val[i];
     }
 }
 
