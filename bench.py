@@ -504,7 +504,7 @@ def run_ours(args, world, rank, local):
     w = get_workload(args.config)
     L = w.layer
     pool = make_pool(w, local, "random")
-    r = Runner(w, pool, None, local, want_lse=True)
+    r = Runner(w, pool, None, local, want_lse=True, lazy=(args.config == 5))  # config 5: raw prefixes are never resident together
     prefix_tokens = r.fill_prefixes()
     torch.cuda.synchronize()
 
