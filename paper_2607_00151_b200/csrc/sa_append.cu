@@ -43,14 +43,19 @@ __global__ void block_table_update_kernel(const ReqMeta *__restrict__ reqs, cons
 
 // Per token: (2*Hkv + Hq) heads, each D/16 "units" of two 16-byte vectors (dims [8j, 8j+8) and
 // [D/2+8j, D/2+8j+8)): K and Q units are rotated, V units are copied bit for bit.
-template <int D>
+// INLINE: the call's metadata (requests, new page ids) rides in the kernel parameters instead of the slab: no upload
+// launch, no block-table launch -- the thread that places a token in a page this call allocated also writes that
+// page's block-table entry (every new page receives at least one new token; equal values from several threads).
+template <int D, bool INLINE>
 __global__ void __launch_bounds__(kAppendThreads)
-rope_append_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t total_rows,
+rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *__restrict__ reqs_slab, int32_t n_req_slab, int64_t total_rows,
                    const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
                    __nv_bfloat16 *__restrict__ q, __nv_bfloat16 *__restrict__ k_base,
                    __nv_bfloat16 *__restrict__ v_base, const int32_t *__restrict__ block_table, int64_t mpps,
                    int32_t log2_page, int64_t stride_page, int64_t stride_head,
-                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
+                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv, int32_t *__restrict__ block_table_w) {
+    const ReqMeta *reqs = INLINE ? im.reqs : reqs_slab;
+    const int32_t n_req = INLINE ? im.n_req : n_req_slab;
     constexpr int HALF = D / 2;
     constexpr int UPH = D / 16;  // units per head
     __shared__ int64_t s_dst[kAppendTok];
@@ -70,7 +75,14 @@ rope_append_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t tota
         }
         const ReqMeta r = reqs[lo];
         const int32_t pos = r.kv_len + int32_t(t - r.q_start);
-        const int32_t page = block_table[int64_t(r.sid) * mpps + (pos >> log2_page)];
+        const int32_t pi = pos >> log2_page;
+        int32_t page;
+        if (INLINE && pi >= r.part_begin && pi - r.part_begin < r.n_splits) {
+            page = im.pages[r.item_begin + pi - r.part_begin];       // allocated (or copied on write) by this call
+            block_table_w[int64_t(r.sid) * mpps + pi] = page;
+        } else {
+            page = block_table[int64_t(r.sid) * mpps + pi];
+        }
         const int32_t slot = pos & ((1 << log2_page) - 1);
         s_pos[tid] = pos;
         s_dst[tid] = int64_t(page) * stride_page + int64_t(slot) * D;
@@ -141,27 +153,35 @@ rope_append_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t tota
     }
 }
 
-cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
-                               int64_t total_rows, const void *k, const void *v, void *q,
-                               cudaStream_t stream, int32_t *launches) {
+template <bool INLINE>
+static cudaError_t launch_rope_append_t(const sa_kv_pool *pool, const InlineAppendMeta &im, const ReqMeta *reqs_dev,
+                                        int32_t n_req, int64_t total_rows, const void *k, const void *v, void *q,
+                                        cudaStream_t stream, int32_t *launches) {
     if (total_rows == 0) return cudaSuccess;
     const unsigned grid = unsigned((total_rows + kAppendTok - 1) / kAppendTok);
     auto kb = static_cast<__nv_bfloat16 *>(pool->k_base);
     auto vb = static_cast<__nv_bfloat16 *>(pool->v_base);
     if (pool->cfg.head_dim == 128)
-        rope_append_kernel<128><<<grid, kAppendThreads, 0, stream>>>(
-            reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
+        rope_append_kernel<128, INLINE><<<grid, kAppendThreads, 0, stream>>>(
+            im, reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
             static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
             pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
-            pool->cfg.num_kv_heads);
+            pool->cfg.num_kv_heads, pool->block_table);
     else
-        rope_append_kernel<64><<<grid, kAppendThreads, 0, stream>>>(
-            reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
+        rope_append_kernel<64, INLINE><<<grid, kAppendThreads, 0, stream>>>(
+            im, reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
             static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
             pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
-            pool->cfg.num_kv_heads);
+            pool->cfg.num_kv_heads, pool->block_table);
     ++*launches;
     return cudaGetLastError();
+}
+
+cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
+                               int64_t total_rows, const void *k, const void *v, void *q,
+                               cudaStream_t stream, int32_t *launches) {
+    static const InlineAppendMeta none{};  // the slab variant never reads it
+    return launch_rope_append_t<false>(pool, none, reqs_dev, n_req, total_rows, k, v, q, stream, launches);
 }
 
 }  // namespace sa
@@ -173,9 +193,11 @@ namespace sa {
 // the device and enqueues the block-table update.  *reqs_dev: the ReqMeta array of the call on the
 // device (kv_len = position of the request's first new token).  Nothing is changed on failure.
 int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
-                       bool have_data, cudaStream_t stream, const ReqMeta **reqs_dev_out, int64_t *total_out) {
+                       bool have_data, cudaStream_t stream, const ReqMeta **reqs_dev_out, int64_t *total_out,
+                       InlineAppendMeta *im) {
     *reqs_dev_out = nullptr;
     *total_out = 0;
+    if (im) im->used = 0;
     if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
     if (n_req == 0) {
         pool->last_launches = 0;
@@ -203,8 +225,10 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
     if (need_pages > int64_t(pool->free_pages.size())) return SA_ERR_OUT_OF_PAGES;
     if (!pool->host_only && total > 0 && !have_data) return SA_ERR_INVALID_ARG;
 
+    // small calls carry their metadata in the kernel parameters (sa_rope_kv_append only: im != nullptr)
+    const bool inline_meta = im && !pool->host_only && n_req <= kInlineReqs && need_pages <= kInlinePages;
     char *mh = nullptr, *md = nullptr;
-    if (!pool->host_only) {
+    if (!pool->host_only && !inline_meta) {
         int32_t st = acquire_meta(pool, &mh, &md);
         if (st != SA_OK) return st;
     }
@@ -217,6 +241,9 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
         host_pages.resize(size_t(need_pages) + 1);
         meta = host_meta.data();
         page_list = host_pages.data();
+    } else if (inline_meta) {
+        meta = im->reqs;
+        page_list = im->pages;
     } else {
         meta = reinterpret_cast<ReqMeta *>(mh);
         page_list = reinterpret_cast<int32_t *>(mh + sizeof(ReqMeta) * size_t(n_req));
@@ -264,6 +291,13 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
 
     for (const auto &c : cow)
         if (copy_page_async(pool, c.first, c.second, stream) != cudaSuccess) return SA_ERR_CUDA;
+    if (inline_meta) {
+        im->n_req = n_req;
+        im->n_list = n_list;
+        im->used = 1;
+        *total_out = total;
+        return SA_OK;
+    }
     // slab layout: [ReqMeta x n_req][new page ids x n_list][ReqMeta x n_gain]
     size_t off_gain = sizeof(ReqMeta) * size_t(n_req) + sizeof(int32_t) * size_t(n_list);
     off_gain = (off_gain + 15) / 16 * 16;
@@ -293,8 +327,15 @@ extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int3
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const ReqMeta *reqs_dev = nullptr;
     int64_t total = 0;
-    const int32_t st = append_prepare(pool, n_req, sids, qo_indptr, k && v, stream, &reqs_dev, &total);
-    if (st != SA_OK || !reqs_dev) return st;
+    InlineAppendMeta im;
+    const int32_t st = append_prepare(pool, n_req, sids, qo_indptr, k && v, stream, &reqs_dev, &total, &im);
+    if (st != SA_OK) return st;
+    if (im.used) {
+        if (launch_rope_append_t<true>(pool, im, nullptr, 0, total, k, v, q_inout, stream, &pool->last_launches) != cudaSuccess)
+            return SA_ERR_CUDA;
+        return SA_OK;
+    }
+    if (!reqs_dev) return st;
     if (launch_rope_append(pool, reqs_dev, n_req, total, k, v, q_inout, stream, &pool->last_launches) != cudaSuccess)
         return SA_ERR_CUDA;
     return SA_OK;

@@ -36,6 +36,15 @@ struct ReqMeta {
     int32_t n_tiles;     // prefill class: packed-row tiles per kv head
 };
 
+// Metadata of a small append carried in the kernel parameters (no upload launch, no block-table launch).
+constexpr int kInlineReqs = 64;
+constexpr int kInlinePages = 384;
+struct InlineAppendMeta {
+    ReqMeta reqs[kInlineReqs];     // as in the slab: kv_len = position of the first new token, item_begin / n_splits /
+    int32_t pages[kInlinePages];   // part_begin = the request's slice of `pages` and the block-table index it starts at
+    int32_t n_req, n_list, used, pad;
+};
+
 // tcgen05 prefill kernel: one persistent CTA per SM walks a list of parts.  An item is (request, kv
 // head, 256 packed rows); a part is the KV-tile range [u0, u1) of an item.  slot < 0: the part is the
 // whole item and writes the output directly; otherwise it writes partial slot `slot` and the merge
@@ -148,8 +157,11 @@ __device__ __forceinline__ float2 rope_cos_sin(int32_t pos, float2 u) {
 #endif
 
 // Host half of an append: validation, page allocation, metadata upload, block-table update (sa_append.cu).
+// im (nullable): if the call is small enough its metadata is returned there (im->used = 1) instead of going to the
+// device, and the caller's kernel updates the block table itself.
 int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
-                       bool have_data, cudaStream_t stream, const ReqMeta **reqs_dev_out, int64_t *total_out);
+                       bool have_data, cudaStream_t stream, const ReqMeta **reqs_dev_out, int64_t *total_out,
+                       InlineAppendMeta *im = nullptr);
 
 // --- kernel launchers (each returns a cudaError_t from the launch) ---
 cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
