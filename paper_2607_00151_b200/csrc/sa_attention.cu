@@ -214,8 +214,16 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     uintptr_t w = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255);
 
-    // per-call metadata: [decode ReqMeta][prefill ReqMeta][tcgen05 schedule] through the pinned slab ring; a
-    // schedule too long for the slab goes through the pool's growable pinned buffer into the workspace
+    float *part_o = reinterpret_cast<float *>(w);
+    float *part_lse = reinterpret_cast<float *>(w + wl.off_part_lse);
+    // a small decode-only call (the latency-critical one) carries its requests in the kernel parameters: no upload launch
+    if (hp.pre.empty() && hp.dec.size() <= size_t(kInlineReqs)) {
+        const cudaError_t e0 = launch_flash_decode(pool, nullptr, hp.dec.data(), hp.plan, q, out, lse, sm_scale, part_o, part_lse,
+                                                   stream, &pool->last_launches);
+        return e0 == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+    }
+    // otherwise the per-call metadata [decode ReqMeta][prefill ReqMeta][tcgen05 schedule] goes through the pinned slab
+    // ring; a schedule too long for the slab goes through the pool's growable pinned buffer into the workspace
     char *mh = nullptr, *md = nullptr;
     st = acquire_meta(pool, &mh, &md);
     if (st != SA_OK) return st;
@@ -245,8 +253,6 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     const ReqMeta *dec_dev = reinterpret_cast<const ReqMeta *>(md);
     const ReqMeta *pre_dev = reinterpret_cast<const ReqMeta *>(md + dec_bytes);
 
-    float *part_o = reinterpret_cast<float *>(w);
-    float *part_lse = reinterpret_cast<float *>(w + wl.off_part_lse);
     char *tc5_partials = reinterpret_cast<char *>(w + wl.off_slots);
 
     // prefill first: it is the long pole; the decode kernel fills in behind it on the same stream
@@ -254,7 +260,7 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.sched, sched_dev, tc5_partials, hp.total_q, q, out, lse, sm_scale,
                            stream, &pool->last_launches);
     if (e != cudaSuccess) return SA_ERR_CUDA;
-    e = launch_flash_decode(pool, dec_dev, hp.plan, q, out, lse, sm_scale, part_o, part_lse, stream, &pool->last_launches);
+    e = launch_flash_decode(pool, dec_dev, nullptr, hp.plan, q, out, lse, sm_scale, part_o, part_lse, stream, &pool->last_launches);
     if (e != cudaSuccess) return SA_ERR_CUDA;
     return SA_OK;
 }

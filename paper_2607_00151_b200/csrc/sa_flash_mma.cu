@@ -8,6 +8,7 @@
 // Packed rows: row rho of a (request, kv head g) pair is (token rho / G, q head g*G + rho % G).
 #include <cuda_bf16.h>
 #include <math.h>
+#include <string.h>
 
 #include "sa_internal.h"
 
@@ -233,8 +234,9 @@ __device__ __forceinline__ void load_q_tile(const AttnArgs &a, const ReqMeta &r,
 
 // ------------------------------------------------------------------------------------------
 // Decode-like rows: split-KV, partials out.
-template <int D>
-__global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
+// INLINE: the requests of a small decode-only call ride in the kernel parameters (no metadata upload launch).
+template <int D, bool INLINE>
+__global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int BM = 16;
     constexpr int TILE_BYTES = kBN * D * 2;
@@ -243,8 +245,9 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
     const uint32_t sQ = s_base + kStages * 2 * TILE_BYTES;
 
     const int item = blockIdx.x;
-    const int ri = find_req(a.reqs, a.n_reqs, item);
-    const ReqMeta r = a.reqs[ri];
+    const ReqMeta *reqs = INLINE ? ir.reqs : a.reqs;
+    const int ri = find_req(reqs, a.n_reqs, item);
+    const ReqMeta r = reqs[ri];
     const int local = item - r.item_begin;
     const int G = 1 << a.log2G;
     const int n_rows = r.q_len * G;
@@ -370,9 +373,9 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const AttnArgs a) {
 
 // Merge of the split partials, fixed split order.  grid = (decode-like requests, Hkv); each warp
 // takes packed rows of the group; lanes cover D with float4.
-template <int D>
-__global__ void __launch_bounds__(128) merge_splits_kernel(const AttnArgs a) {
-    const ReqMeta r = a.reqs[blockIdx.x];
+template <int D, bool INLINE>
+__global__ void __launch_bounds__(128) merge_splits_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
+    const ReqMeta r = INLINE ? ir.reqs[blockIdx.x] : a.reqs[blockIdx.x];
     const int g = blockIdx.y;
     const int G = 1 << a.log2G;
     const int n_rows = r.q_len * G;
@@ -436,37 +439,46 @@ AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const
     return a;
 }
 
-template <int D>
-cudaError_t launch_flash(const AttnArgs &a, int items, cudaStream_t stream) {
+template <int D, bool INLINE>
+cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, dim3 merge_grid, cudaStream_t stream,
+                         int32_t *launches) {
     constexpr int BM = 16;
     constexpr size_t smem = size_t(kStages) * 2 * kBN * D * 2 + size_t(BM) * D * 2;
     static_assert(smem >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(flash_mma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+        cudaError_t e = cudaFuncSetAttribute(flash_mma_kernel<D, INLINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    flash_mma_kernel<D><<<unsigned(items), kThreads, smem, stream>>>(a);
+    flash_mma_kernel<D, INLINE><<<unsigned(items), kThreads, smem, stream>>>(ir, a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    ++*launches;
+    merge_splits_kernel<D, INLINE><<<merge_grid, 128, 0, stream>>>(ir, a);
+    ++*launches;
     return cudaGetLastError();
 }
 
 }  // namespace
 
-cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
-                                const void *q, void *out, float *lse, float sm_scale, float *part_o,
-                                float *part_lse, cudaStream_t stream, int32_t *launches) {
+// reqs_host != nullptr (and plan.n_dec <= kInlineReqs): the requests go in the kernel parameters, reqs_dev is unused
+cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
+                                const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
+                                float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches) {
     if (plan.dec_items == 0) return cudaSuccess;
     AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
-    cudaError_t e = pool->cfg.head_dim == 128 ? launch_flash<128>(a, plan.dec_items, stream)
-                                              : launch_flash<64>(a, plan.dec_items, stream);
-    if (e != cudaSuccess) return e;
-    ++*launches;
-    dim3 grid(unsigned(plan.n_dec), unsigned(pool->cfg.num_kv_heads));
-    if (pool->cfg.head_dim == 128) merge_splits_kernel<128><<<grid, 128, 0, stream>>>(a);
-    else merge_splits_kernel<64><<<grid, 128, 0, stream>>>(a);
-    ++*launches;
-    return cudaGetLastError();
+    const dim3 grid(unsigned(plan.n_dec), unsigned(pool->cfg.num_kv_heads));
+    const bool d128 = pool->cfg.head_dim == 128;
+    if (reqs_host) {
+        InlineReqs ir;
+        memcpy(ir.reqs, reqs_host, sizeof(ReqMeta) * size_t(plan.n_dec));
+        return d128 ? launch_flash<128, true>(ir, a, plan.dec_items, grid, stream, launches)
+                    : launch_flash<64, true>(ir, a, plan.dec_items, grid, stream, launches);
+    }
+    static const InlineReqs none{};  // never read by the slab variants
+    return d128 ? launch_flash<128, false>(none, a, plan.dec_items, grid, stream, launches)
+                : launch_flash<64, false>(none, a, plan.dec_items, grid, stream, launches);
 }
 
 }  // namespace sa

@@ -45,6 +45,11 @@ struct InlineAppendMeta {
     int32_t n_req, n_list, used, pad;
 };
 
+// The requests of a small decode-only attention call, carried in the kernel parameters.
+struct InlineReqs {
+    ReqMeta reqs[kInlineReqs];
+};
+
 // tcgen05 prefill kernel: one persistent CTA per SM walks a list of parts.  An item is (request, kv
 // head, 256 packed rows); a part is the KV-tile range [u0, u1) of an item.  slot < 0: the part is the
 // whole item and writes the output directly; otherwise it writes partial slot `slot` and the merge
@@ -175,9 +180,9 @@ struct AttnPlan {
     int64_t dec_rows = 0;                // decode-like (token, head) rows to merge
 };
 
-cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const AttnPlan &plan,
-                                const void *q, void *out, float *lse, float sm_scale, float *part_o,
-                                float *part_lse, cudaStream_t stream, int32_t *launches);
+cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
+                                const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
+                                float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches);
 // dense operators of the layer (sa_gemm_tc5.cu); each returns an SA_* status
 int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
                    void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches);
