@@ -62,19 +62,29 @@ kv_export_kernel(const __nv_bfloat16 *__restrict__ k_base, const __nv_bfloat16 *
     }
 }
 
-// IMPORT: image -> pages of the tokens an append_prepare has just made room for.
+// IMPORT: image -> pages of the tokens an append_prepare has just made room for.  INLINE: the request and its new page
+// ids ride in the kernel parameters (no upload launch, no block-table launch; the placing thread writes the entry), as
+// in rope_append_kernel.
+template <bool INLINE>
 __global__ void __launch_bounds__(kXferThreads)
-kv_import_kernel(const ReqMeta *__restrict__ req, __nv_bfloat16 *__restrict__ k_base, __nv_bfloat16 *__restrict__ v_base,
-                 const int32_t *__restrict__ block_table, int64_t mpps, int32_t log2_page, int64_t stride_page,
+kv_import_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *__restrict__ req, __nv_bfloat16 *__restrict__ k_base, __nv_bfloat16 *__restrict__ v_base,
+                 int32_t *block_table, int64_t mpps, int32_t log2_page, int64_t stride_page,
                  int64_t stride_head, int32_t Hkv, int32_t D, int32_t src_heads, int32_t head_begin, int32_t n_tok,
                  const __nv_bfloat16 *__restrict__ image) {
     __shared__ int64_t s_dst[kXferTok];
-    const ReqMeta r = req[0];
+    const ReqMeta r = INLINE ? im.reqs[0] : req[0];
     const int t0 = blockIdx.x * kXferTok;
     const int nt = min(kXferTok, n_tok - t0);
     if (threadIdx.x < nt) {
         const int pos = r.kv_len + t0 + threadIdx.x;
-        const int32_t page = block_table[int64_t(r.sid) * mpps + (pos >> log2_page)];
+        const int32_t pi = pos >> log2_page;
+        int32_t page;
+        if (INLINE && pi >= r.part_begin && pi - r.part_begin < r.n_splits) {
+            page = im.pages[r.item_begin + pi - r.part_begin];
+            block_table[int64_t(r.sid) * mpps + pi] = page;
+        } else {
+            page = block_table[int64_t(r.sid) * mpps + pi];
+        }
         s_dst[threadIdx.x] = int64_t(page) * stride_page + int64_t(pos & ((1 << log2_page) - 1)) * D;
     }
     __syncthreads();
@@ -147,14 +157,21 @@ extern "C" int32_t sa_kv_session_import(sa_kv_pool *pool, int32_t sid, int64_t n
     const int32_t indptr[2] = {0, int32_t(n_tokens)};
     const sa::ReqMeta *req_dev = nullptr;
     int64_t total = 0;
+    sa::InlineAppendMeta im;
     // page allocation, copy-on-write of a shared partial page, block-table update and failure behaviour are the append's
-    const int32_t st = sa::append_prepare(pool, 1, &sid, indptr, image != nullptr, stream, &req_dev, &total);
-    if (st != SA_OK || !req_dev || total == 0) return st;
+    const int32_t st = sa::append_prepare(pool, 1, &sid, indptr, image != nullptr, stream, &req_dev, &total, &im);
+    if (st != SA_OK || (!req_dev && !im.used) || total == 0) return st;
     const unsigned grid = unsigned((n_tokens + sa::kXferTok - 1) / sa::kXferTok);
-    sa::kv_import_kernel<<<grid, sa::kXferThreads, 0, stream>>>(
-        req_dev, static_cast<__nv_bfloat16 *>(pool->k_base), static_cast<__nv_bfloat16 *>(pool->v_base), pool->block_table,
-        pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head, pool->cfg.num_kv_heads,
-        pool->cfg.head_dim, src_heads, head_begin, int32_t(n_tokens), static_cast<const __nv_bfloat16 *>(image));
+    if (im.used)
+        sa::kv_import_kernel<true><<<grid, sa::kXferThreads, 0, stream>>>(
+            im, nullptr, static_cast<__nv_bfloat16 *>(pool->k_base), static_cast<__nv_bfloat16 *>(pool->v_base), pool->block_table,
+            pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head, pool->cfg.num_kv_heads,
+            pool->cfg.head_dim, src_heads, head_begin, int32_t(n_tokens), static_cast<const __nv_bfloat16 *>(image));
+    else
+        sa::kv_import_kernel<false><<<grid, sa::kXferThreads, 0, stream>>>(
+            im, req_dev, static_cast<__nv_bfloat16 *>(pool->k_base), static_cast<__nv_bfloat16 *>(pool->v_base), pool->block_table,
+            pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head, pool->cfg.num_kv_heads,
+            pool->cfg.head_dim, src_heads, head_begin, int32_t(n_tokens), static_cast<const __nv_bfloat16 *>(image));
     ++pool->last_launches;
     return cudaGetLastError() == cudaSuccess ? SA_OK : SA_ERR_CUDA;
 }
