@@ -23,6 +23,8 @@
  *     (cudaStream_t; NULL = the legacy default stream), only enqueue work, never allocate
  *     device memory and never synchronise the device.  All hot calls on one pool must be
  *     issued on one stream (or on streams the caller orders).  A pool is not thread-safe.
+ *     They may wait on the host for a metadata slot of an earlier call and change host-side
+ *     session state when called, so they must not be issued under CUDA stream capture.
  *   - A call that fails leaves the pool, its block tables and session lengths unchanged.
  *   - All tensors are bf16 (raw 16-bit patterns), packed ragged: the tokens of request r are
  *     rows [qo_indptr[r], qo_indptr[r+1]) of a [T, heads, head_dim] row-major array.
