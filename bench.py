@@ -45,18 +45,62 @@ def load_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    """SM clock and throttle reasons sampled DURING the timed region: NVML polled from a thread every ~2 ms (a short
+    timed region is over before nvidia-smi has even started; `nvidia-smi -lms` is the fallback when NVML is not
+    importable).  The sampler runs from before the warm-up; every sample carries the host time it was taken at and
+    summary() keeps those inside [mark_begin(), mark_end()] (all of them -- warm-up steps of the same workload -- if
+    none fell inside)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    BITS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4))
 
     def __init__(self, index: int):
-        self.samples, self.proc, self.index = [], None, index
+        self.samples, self.proc, self.index = [], None, index   # samples: (host time, sm MHz, max MHz, [reasons])
+        self.t_begin, self.t_end = None, None
+        self.stop = threading.Event()
+        self.how = None
+
+    def mark_begin(self):
+        self.t_begin = time.time()
+
+    def mark_end(self):
+        self.t_end = time.time()
+
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        ids = [v.strip() for v in vis.split(",") if v.strip()]
+        if ids and self.index < len(ids) and ids[self.index].isdigit():
+            return int(ids[self.index])
+        return self.index
 
     def __enter__(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self._physical_index())
+            mx = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            reasons_fn = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+
+            def poll():
+                while not self.stop.is_set():
+                    try:
+                        mhz = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                        mask = int(reasons_fn(h))
+                        self.samples.append((time.time(), mhz, mx, [n for n, b in self.BITS if mask & b]))
+                    except Exception:
+                        pass
+                    time.sleep(0.002)
+            self.how = "nvml"
+            self.t = threading.Thread(target=poll, daemon=True)
+            self.t.start()
+            return self
+        except Exception:
+            pass
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self._physical_index()), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.how = "nvidia-smi"
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -64,12 +108,20 @@ class ClockSampler:
         return self
 
     def _read(self):
+        names = [n for n, _ in self.BITS]
+        order = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]   # the query's column order
         for line in self.proc.stdout:
-            self.samples.append(line.strip())
+            f = [x.strip() for x in line.split(",")]
+            try:
+                rs = [n for n, v in zip(order, f[2:6]) if v.lower().startswith("active") and n in names]
+                self.samples.append((time.time(), float(f[0]), float(f[1]), rs))
+            except Exception:
+                continue
 
     def __exit__(self, *a):
+        self.stop.set()
         if self.proc:
-            time.sleep(0.15)
+            time.sleep(0.05)
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=2)
@@ -77,21 +129,15 @@ class ClockSampler:
                 self.proc.kill()
 
     def summary(self):
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for s in self.samples:
-            f = [x.strip() for x in s.split(",")]
-            try:
-                sm.append(float(f[0]))
-                mx.append(float(f[1]))
-            except Exception:
-                continue
-            for n, v in zip(names, f[2:6]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
-        if not sm:
+        inside = [x for x in self.samples
+                  if self.t_begin is not None and self.t_end is not None and self.t_begin <= x[0] <= self.t_end]
+        use = inside or list(self.samples)
+        if not use:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+        reasons = sorted({r for x in use for r in x[3]})
+        return {"sm_mhz": float(np.median([x[1] for x in use])), "sm_max_mhz": float(max(x[2] for x in use)),
+                "reasons": reasons, "samples": len(use), "window": "timed region" if inside else "warm-up + timed region",
+                "source": self.how}
 
 
 def load_traffic():
@@ -542,18 +588,20 @@ def run_ours(args, world, rank, local):
         return e0, e1, launches
 
     r.step()  # allocates workspaces
-    for _ in range(max(args.warmup, 3)):
-        timed_step()
-    torch.cuda.synchronize()
-    dist_barrier(world)
-    torch.cuda.synchronize()
     ev, attn_ev, launches = [], [], 0
-    with ClockSampler(local) as cs:
+    with ClockSampler(local) as cs:   # started before the warm-up: see ClockSampler
+        for _ in range(max(args.warmup, 3)):
+            timed_step()
+        torch.cuda.synchronize()
+        dist_barrier(world)
+        torch.cuda.synchronize()
+        cs.mark_begin()
         for _ in range(args.steps):
             e0, e1, n = timed_step(attn_ev)
             ev.append((e0, e1))
             launches += n
         torch.cuda.synchronize()
+        cs.mark_end()
     dist_barrier(world)
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = dist_max(float(sum(step_ms)), world, dev)
