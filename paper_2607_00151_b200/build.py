@@ -59,7 +59,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if failed:
         raise RuntimeError("nvcc failed")
     tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.check_call([nvcc, "-shared", "-o", tmp, *objs, "-cudart", "static", "-Xlinker", "--exclude-libs,ALL"])
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs, "-cudart", "static",
+                           "-Xlinker", "--exclude-libs,ALL"])
     os.replace(tmp, LIB)
     return LIB
 
