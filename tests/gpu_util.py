@@ -10,6 +10,44 @@ from paper_2607_00151_b200.workloads import gen_session
 
 # BASELINE.json north_star gates + the binding relative gates of SURVEY 8(c) T-A
 MAX_ABS, MEAN_ABS, REL_L2 = 2e-2, 2e-3, 1e-2
+U_BF16 = 2.0 ** -9   # unit roundoff of bf16 (8 significand bits, round to nearest even)
+
+
+def derived_gates(sigma_logit, o_absmax, v_rms, stored_rounded=False):
+    """Gates for inputs that BASELINE.json's distributions do not cover (DESIGN.md section 3a derives every term).
+
+    sigma_logit: standard deviation of the scaled scores the test's inputs produce (sm_scale * sigma_q * sigma_k *
+    sqrt(D)); o_absmax: largest |o_ref|; v_rms: standard deviation of V.  Against the UNROUNDED fp64 oracle the
+    path's own contract -- K' and Q' are STORED in bf16 -- perturbs every logit by
+        sigma_delta = 1.5 * sqrt(2/3) * u * sigma_logit          (u = 2^-9; two operands, rel. error uniform in +-u each;
+                                                                  the 1.5 covers keys whose |q.k| is above average)
+    and a correct kernel then shows
+        |d lse|      <= 4.5 sigma_delta                          (4.5 sigma: the largest of <= 1e5 rows)
+        |d o| elem   <= half_ulp_bf16(|o|max) + 4.5 * sqrt(sigma_delta^2 + u^2/3) * v_rms   (output rounding + logit
+                                                                  perturbation and bf16 P, with sum_j p_j^2 <= 1)
+        mean |d o|   <= 0.8 * sqrt(sigma_delta^2 + 2 u^2/3) * v_rms
+        rel-L2       <= 2.5 * sqrt(sigma_delta^2 + 2 u^2/3)
+    stored_rounded=True: the reference is the oracle evaluated on q', k' rounded to bf16 (the diagnostic mode of SURVEY
+    8(c)); what is left of sigma_delta is the <= 1 % of stored elements that sit one ulp from the correctly rounded
+    value: a factor sqrt(0.01 * 4 / (1/3)) = 0.35.  No gate is ever tighter than BASELINE.json's 2e-2 / 2e-3 (and the
+    1e-2 normalised / 1e-3 lse gates of reading T-A); on BASELINE.json's distributions (sigma_logit ~ 0.008) every
+    derived term is far below them, so they apply unchanged.
+    Returns (max_abs, mean_abs, rel_l2, lse_tol)."""
+    sd = 1.5 * np.sqrt(2.0 / 3.0) * U_BF16 * sigma_logit * (0.35 if stored_rounded else 1.0)
+    half_ulp = 2.0 ** (np.floor(np.log2(max(o_absmax, 1e-30))) - 8)
+    max_abs = max(MAX_ABS, half_ulp + 4.5 * np.sqrt(sd ** 2 + U_BF16 ** 2 / 3) * v_rms)
+    mean_abs = max(MEAN_ABS, 0.8 * np.sqrt(sd ** 2 + 2 * U_BF16 ** 2 / 3) * v_rms)
+    rel_l2 = max(REL_L2, 2.5 * np.sqrt(sd ** 2 + 2 * U_BF16 ** 2 / 3))
+    lse_tol = max(1e-3, 4.5 * sd)
+    return float(max_abs), float(mean_abs), float(rel_l2), float(lse_tol)
+
+
+def check_derived(o_gpu, l_gpu, ref, sigma_logit, v_rms, what="", stored_rounded=False):
+    """check_out + check_lse with the gates derived_gates gives for these inputs."""
+    mx, mn, rl, lt = derived_gates(sigma_logit, float(np.abs(ref["o"]).max()), v_rms, stored_rounded)
+    e = check_out(o_gpu, ref["o"], what, max_abs=mx, mean_abs=mn, rel_l2=rl)
+    le = check_lse(l_gpu, ref["lse"], lt, what) if l_gpu is not None else 0.0
+    return e + (le,)
 
 
 def oracle_session(w, i, data, rows=None, heads=None):
@@ -20,6 +58,19 @@ def oracle_session(w, i, data, rows=None, heads=None):
     k_rot_prefix = orc.rope(k[:P], np.arange(P), w.layer.rope_base)
     return orc.oracle_cached(k_rot_prefix, orc.widen(v[:P]), q, k[P:], v[P:], P, w.layer.rope_base,
                              rows=rows, heads=heads)
+
+
+def oracle_session_stored(w, i, data, rows=None, heads=None):
+    """The diagnostic mode of SURVEY 8(c): the same oracle, but q' and k' are rounded to bf16 (nearest even, by torch on
+    the CPU, from the ORACLE's own fp64 RoPE -- nothing comes from the CUDA path) before the scores, as the cache stores
+    them.  Separates storage quantisation from kernel error."""
+    s = w.sessions[i]
+    k, v, q = (t.cpu() for t in data[i])
+    P = s.prefix
+    base = w.layer.rope_base
+    k_rot = bf16_rne(orc.rope(k, np.arange(s.total), base))
+    q_rot = bf16_rne(orc.rope(q, np.arange(P, s.total), base))
+    return orc.attend(q_rot, k_rot, orc.widen(v), P, rows=rows, heads=heads)
 
 
 def check_out(o_gpu, o_ref, what="", max_abs=MAX_ABS, mean_abs=MEAN_ABS, rel_l2=REL_L2):

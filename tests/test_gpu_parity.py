@@ -12,7 +12,8 @@ from paper_2607_00151_b200 import workloads as wl
 from paper_2607_00151_b200.harness import Runner, gather_kv, make_pool, pool_views
 from paper_2607_00151_b200.workloads import Layer, SessionSpec, Workload, gen_session
 
-from gpu_util import (bf16_rne, check_lse, check_out, check_rope_k, oracle_session, run_workload)
+from gpu_util import (bf16_rne, check_derived, check_lse, check_out, check_rope_k, oracle_session, oracle_session_stored,
+                      run_workload)
 
 pytestmark = pytest.mark.gpu
 
@@ -125,14 +126,19 @@ def test_cfg1_attention_parity_and_decomposability():
     assert torch.equal(_bits(r_c.gather_kv(0)[0]), _bits(r.gather_kv(0)[0]))
 
 
-def test_cfg1_sharp_values():
-    # logits with std ~ 8 (q, k x4 in the sharp variant of T-A): running max and rescale paths
+@pytest.mark.parametrize("sigma_logit", [2.0, 4.0])
+def test_cfg1_sharp_values(sigma_logit):
+    """Config 1 itself is reading T-A's "sharp" case (N(0,1) values: scores of std 1); here Q, K ~ N(0, sigma^2) with
+    sigma^2 = 2 and 4 ("peaked": a handful of keys carry each row): running max and O rescale paths.  Against the unrounded oracle the gates are derived_gates' (the bf16
+    storage of K', Q' moves every score by ~2.4e-3 sigma_logit: DESIGN.md 3a); against the oracle evaluated on q', k'
+    rounded to bf16 -- what the cache holds -- the same kernel output meets the tighter stored-operand gates."""
     w = wl.config1()
-    pool, r, data = run_workload(w, scale=2.0)
-    ref = oracle_session(w, 0, data)
+    pool, r, data = run_workload(w, scale=sigma_logit ** 0.5)
     out, lse, _ = r.outputs()[0]
-    check_out(out, ref["o"], "cfg1 sharp", max_abs=4e-2, mean_abs=4e-3, rel_l2=2e-2)
-    check_lse(lse, ref["lse"], 5e-2, "cfg1 sharp")
+    e = check_derived(out, lse, oracle_session(w, 0, data), sigma_logit, 1.0, "cfg1 sigma %g" % sigma_logit)
+    e2 = check_derived(out, lse, oracle_session_stored(w, 0, data), sigma_logit, 1.0, "cfg1 sigma %g, stored operands" % sigma_logit,
+                       stored_rounded=True)
+    print("cfg1 sigma_logit %g: vs oracle %s; vs oracle on bf16 q', k' %s" % (sigma_logit, e, e2))
 
 
 def test_cfg1_page_permutation_and_nan_slots_bit_exact():
@@ -214,8 +220,8 @@ def test_degenerate_sizes():
     for i, s in enumerate(w.sessions):
         if s.new == 0:
             continue
-        ref = oracle_session(w, i, data)
-        check_out(r.outputs()[i][0], ref["o"], "deg s%d" % i, max_abs=4e-2, mean_abs=6e-3, rel_l2=2e-2)
+        ref = oracle_session(w, i, data)   # N(0,1) values: scores of std 1, |o| up to |v|max ~ 4.5 (one-key rows)
+        check_derived(r.outputs()[i][0], r.outputs()[i][1], ref, 1.0, 1.0, "deg s%d" % i)
     # kv = 1: the row attends only itself, o = v_0 exactly (probability 1)
     assert torch.equal(_bits(r.outputs()[0][0][0]), _bits(data[0][1][0].repeat_interleave(4, dim=0)))
     # n_req = 0 and an all-empty batch are no-ops
@@ -306,9 +312,8 @@ def test_shapes_gqa_pages(Hq, Hkv, D, B):
     w = _small_l8b(sessions, seed=31, scale=D ** -0.25, B=B, D=D, Hq=Hq, Hkv=Hkv)
     pool, r, data = run_workload(w, sentinel=SENT)
     for i in range(len(sessions)):
-        ref = oracle_session(w, i, data)
-        check_out(r.outputs()[i][0], ref["o"], "shape s%d" % i, max_abs=3e-2, mean_abs=3e-3)
-        check_lse(r.outputs()[i][1], ref["lse"], 5e-3, "shape s%d" % i)
+        ref = oracle_session(w, i, data)   # q, k, v ~ N(0, D^-1/2): scores of std D^-1/2
+        check_derived(r.outputs()[i][0], r.outputs()[i][1], ref, D ** -0.5, D ** -0.25, "shape s%d" % i)
 
 
 def test_truncate_then_reprefill_reuses_pages_and_matches():
@@ -346,5 +351,4 @@ def test_head_dim_64_long_context_stream_k_parts_and_merge(B, G):
         ref = oracle_session(w, i, data, rows=rows, heads=heads)
         out, lse, _ = r.outputs()[i]
         idx = (torch.as_tensor(rows), torch.as_tensor(heads.astype(np.int64)))
-        check_out(out[idx], ref["o"], "D64 B%d s%d" % (B, i), max_abs=3e-2, mean_abs=3e-3)
-        check_lse(lse[idx], ref["lse"], 1e-2, "D64 B%d s%d" % (B, i))
+        check_derived(out[idx], lse[idx], ref, 64 ** -0.5, 64 ** -0.25, "D64 B%d s%d" % (B, i))
