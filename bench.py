@@ -142,7 +142,7 @@ class ClockSampler:
 
 def load_traffic():
     """dram bytes per launch of the three kernels, from the committed ncu --set full summaries (profiles/)."""
-    p = os.path.join(ROOT, "profiles", "r1c_traffic.json")
+    p = os.path.join(ROOT, "profiles", "traffic.json")
     return json.load(open(p)) if os.path.exists(p) else {}
 
 
