@@ -212,7 +212,13 @@ struct AttnArgs {
     int64_t mpps, stride_page, stride_head;
     int32_t log2_page, Hq, Hkv, log2G;
     float scale_log2;
+    // Captured launches (sa_decode_step): the grid is sized for the step's capacity and the actual counts are read on the
+    // device, dyn = {requests, decode CTAs, ...} in the step's metadata slab; nullptr: counts are the launch's own.
+    const int32_t *dyn;
 };
+
+// barrier over one 128-thread group of the CTA (id 0 with 128 threads is __syncthreads of a 128-thread CTA)
+__device__ __forceinline__ void group_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 
 // Load BM packed rows of Q (row base rho0) into swizzled smem; rows beyond n_rows are zero.
 template <int D, int BM>
@@ -234,19 +240,19 @@ __device__ __forceinline__ void load_q_tile(const AttnArgs &a, const ReqMeta &r,
 
 // ------------------------------------------------------------------------------------------
 // Decode-like rows: split-KV, partials out.
-// INLINE: the requests of a small decode-only call ride in the kernel parameters (no metadata upload launch).
-template <int D, bool INLINE>
-__global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
-    extern __shared__ __align__(128) unsigned char smem[];
+// One work item = one (request, kv head, 1024-key split), computed by a group of 128 threads over its own ring in
+// shared memory.  The arithmetic (and so every bit of the result) depends on the item alone: which kernel, CTA or
+// group runs it does not matter.
+template <int D>
+__device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *reqs, int n_reqs, int item, unsigned char *smem,
+                                            int tid, int bar_id) {
     constexpr int BM = 16;
     constexpr int TILE_BYTES = kBN * D * 2;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lane = tid & 31, warp = tid >> 5;
     const uint32_t s_base = smem_u32(smem);
     const uint32_t sQ = s_base + kStages * 2 * TILE_BYTES;
 
-    const int item = blockIdx.x;
-    const ReqMeta *reqs = INLINE ? ir.reqs : a.reqs;
-    const int ri = find_req(reqs, a.n_reqs, item);
+    const int ri = find_req(reqs, n_reqs, item);
     const ReqMeta r = reqs[ri];
     const int local = item - r.item_begin;
     const int G = 1 << a.log2G;
@@ -273,7 +279,7 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_consta
         cp_async_commit();
     }
     load_q_tile<D, BM>(a, r, g, rho0, n_rows, sQ, tid);
-    __syncthreads();
+    group_sync(bar_id);
     constexpr int row_base = 0;
     uint32_t qf[D / 16][4];
     {
@@ -298,7 +304,7 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_consta
 
     for (int t = 0; t < n_tiles; ++t) {
         cp_async_wait<kStages - 2>();
-        __syncthreads();
+        group_sync(bar_id);
         {
             const int tn = t + kStages - 1;
             if (tn < n_tiles) {
@@ -324,7 +330,7 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_consta
     l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
 
     // ---- merge the four warps' states (each saw a disjoint quarter of every tile)
-    __syncthreads();  // everyone is done with the stage buffers
+    group_sync(bar_id);  // everyone is done with the stage buffers
     float *sO = reinterpret_cast<float *>(smem);             // [4][16][D]
     float *sM = sO + 4 * 16 * D;                             // [4][16]
     float *sL = sM + 4 * 16;                                 // [4][16]
@@ -344,7 +350,7 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_consta
             sL[warp * 16 + r1] = l1;
         }
     }
-    __syncthreads();
+    group_sync(bar_id);
     for (int e = tid; e < n_rows * (D / 4); e += kThreads) {
         const int row = e / (D / 4), c4 = e % (D / 4);
         float M = -INFINITY;
@@ -371,10 +377,42 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_consta
     }
 }
 
+// grid = decode CTAs of the call (one item each).  INLINE: the requests of a small decode-only call ride in the kernel
+// parameters (no metadata upload launch).
+template <int D, bool INLINE>
+__global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    int n_reqs = a.n_reqs;
+    if (!INLINE && a.dyn) {
+        n_reqs = a.dyn[0];
+        if (int(blockIdx.x) >= a.dyn[1]) return;
+    }
+    decode_item<D>(a, INLINE ? ir.reqs : a.reqs, n_reqs, blockIdx.x, smem, threadIdx.x, 0);
+}
+
+// The same items on a FIXED number of CTAs, each with two 128-thread groups that walk the item list with their own
+// rings (2 x 100 KiB of shared memory: nothing else fits on the SM).  Used by the overlapped mixed call, where the
+// decode rows must stay on a subset of the SMs while the tensor-core prefill kernel owns the others.
+template <int D>
+__global__ void __launch_bounds__(2 * kThreads) flash_mma_persist_kernel(const AttnArgs a, int n_items) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr size_t GROUP_BYTES = size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2;
+    const int grp = threadIdx.x >> 7, tid = threadIdx.x & 127;
+    unsigned char *my = smem + size_t(grp) * GROUP_BYTES;
+    for (int item = blockIdx.x * 2 + grp; item < n_items; item += gridDim.x * 2) {
+        decode_item<D>(a, a.reqs, a.n_reqs, item, my, tid, 1 + grp);
+        group_sync(1 + grp);  // the merge scratch of this item lives in the ring the next item fills
+    }
+}
+
 // Merge of the split partials, fixed split order.  grid = (decode-like requests, Hkv); each warp
 // takes packed rows of the group; lanes cover D with float4.
 template <int D, bool INLINE>
 __global__ void __launch_bounds__(128) merge_splits_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
+    // launched with programmatic stream serialization: the grid is staged while the split kernel drains and waits
+    // here until that kernel has completed and its partials are visible (a no-op for an ordinary launch)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (!INLINE && a.dyn && int(blockIdx.x) >= a.dyn[0]) return;
     const ReqMeta r = INLINE ? ir.reqs[blockIdx.x] : a.reqs[blockIdx.x];
     const int g = blockIdx.y;
     const int G = 1 << a.log2G;
@@ -436,38 +474,88 @@ AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const
     while ((1 << lg) < pool->G) ++lg;
     a.log2G = lg;
     a.scale_log2 = sm_scale * 1.4426950408889634f;
+    a.dyn = nullptr;
     return a;
+}
+
+// The > 48 KiB dynamic shared memory opt-in is a per-device, per-function attribute: set it once per (function, device).
+template <auto kernel>
+cudaError_t opt_in_smem(size_t smem) {
+    static unsigned long long done = 0;  // bit per device ordinal; one static per kernel (the kernel is the template argument)
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 64 && (done >> dev) & 1ull) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (e == cudaSuccess && dev < 64) done |= 1ull << dev;
+    return e;
+}
+
+template <int D>
+constexpr size_t group_smem() {
+    return size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2;
+}
+
+// The merge of the splits is launched with programmatic stream serialization: its grid is set up while the split
+// kernel still runs and starts (griddepcontrol.wait at its top) the moment that kernel has completed.
+template <int D, bool INLINE>
+cudaError_t launch_merge(const InlineReqs &ir, const AttnArgs &a, dim3 grid, cudaStream_t stream) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(128);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, merge_splits_kernel<D, INLINE>, ir, a);
 }
 
 template <int D, bool INLINE>
 cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, dim3 merge_grid, cudaStream_t stream,
                          int32_t *launches) {
-    constexpr int BM = 16;
-    constexpr size_t smem = size_t(kStages) * 2 * kBN * D * 2 + size_t(BM) * D * 2;
+    constexpr size_t smem = group_smem<D>();
     static_assert(smem >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(flash_mma_kernel<D, INLINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    cudaError_t e = opt_in_smem<&flash_mma_kernel<D, INLINE>>(smem);
+    if (e != cudaSuccess) return e;
     flash_mma_kernel<D, INLINE><<<unsigned(items), kThreads, smem, stream>>>(ir, a);
-    cudaError_t e = cudaGetLastError();
+    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     ++*launches;
-    merge_splits_kernel<D, INLINE><<<merge_grid, 128, 0, stream>>>(ir, a);
+    e = launch_merge<D, INLINE>(ir, a, merge_grid, stream);
     ++*launches;
-    return cudaGetLastError();
+    return e;
+}
+
+template <int D>
+cudaError_t launch_flash_persist(const AttnArgs &a, int items, int n_cta, dim3 merge_grid, cudaStream_t stream, int32_t *launches) {
+    constexpr size_t smem = 2 * group_smem<D>();
+    cudaError_t e = opt_in_smem<&flash_mma_persist_kernel<D>>(smem);
+    if (e != cudaSuccess) return e;
+    flash_mma_persist_kernel<D><<<unsigned(n_cta), 2 * kThreads, smem, stream>>>(a, items);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    ++*launches;
+    static const InlineReqs none{};
+    e = launch_merge<D, false>(none, a, merge_grid, stream);
+    ++*launches;
+    return e;
 }
 
 }  // namespace
 
-// reqs_host != nullptr (and plan.n_dec <= kInlineReqs): the requests go in the kernel parameters, reqs_dev is unused
+// reqs_host != nullptr (and plan.n_dec <= kInlineReqs): the requests go in the kernel parameters, reqs_dev is unused.
+// persist_ctas > 0: the items run on that many two-group CTAs (one per SM) instead of one CTA each.
+// dyn != nullptr (captured step): grid sizes come from `plan` (the step's capacity), the actual counts from dyn.
 cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
                                 const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
-                                float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches) {
+                                float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches,
+                                int persist_ctas, const int32_t *dyn) {
     if (plan.dec_items == 0) return cudaSuccess;
     AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
+    a.dyn = dyn;
     const dim3 grid(unsigned(plan.n_dec), unsigned(pool->cfg.num_kv_heads));
     const bool d128 = pool->cfg.head_dim == 128;
     if (reqs_host) {
@@ -476,6 +564,9 @@ cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
         return d128 ? launch_flash<128, true>(ir, a, plan.dec_items, grid, stream, launches)
                     : launch_flash<64, true>(ir, a, plan.dec_items, grid, stream, launches);
     }
+    if (persist_ctas > 0)
+        return d128 ? launch_flash_persist<128>(a, plan.dec_items, persist_ctas, grid, stream, launches)
+                    : launch_flash_persist<64>(a, plan.dec_items, persist_ctas, grid, stream, launches);
     static const InlineReqs none{};  // never read by the slab variants
     return d128 ? launch_flash<128, false>(none, a, plan.dec_items, grid, stream, launches)
                 : launch_flash<64, false>(none, a, plan.dec_items, grid, stream, launches);

@@ -182,7 +182,8 @@ struct AttnPlan {
 
 cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
                                 const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
-                                float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches);
+                                float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches,
+                                int persist_ctas = 0, const int32_t *dyn = nullptr);
 // dense operators of the layer (sa_gemm_tc5.cu); each returns an SA_* status
 int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
                    void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches);
