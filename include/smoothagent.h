@@ -25,7 +25,15 @@
  *     issued on one stream (or on streams the caller orders).  A pool is not thread-safe.
  *     They may wait on the host for a metadata slot of an earlier call and change host-side
  *     session state when called, so they must not be issued under CUDA stream capture.
- *   - A call that fails leaves the pool, its block tables and session lengths unchanged.
+ *   - A call that fails with SA_ERR_INVALID_ARG, SA_ERR_OUT_OF_PAGES, SA_ERR_OUT_OF_SESSIONS, SA_ERR_UNSUPPORTED or
+ *     SA_ERR_WORKSPACE_TOO_SMALL leaves the pool, its block tables and session lengths unchanged: everything is
+ *     validated and sized before any state is touched.  SA_ERR_CUDA means the CUDA runtime refused a launch, copy or
+ *     event (in practice a sticky device error from earlier work): host bookkeeping may by then have moved on (pages
+ *     taken, sessions grown or committed, part of a layer enqueued), so the pool's state is undefined and the only
+ *     valid call on it is sa_kv_pool_destroy.
+ *   - Every call that touches the device runs on the pool's device (cfg.device) whatever device is current in the
+ *     calling thread, and restores the caller's current device before returning.  The pool-less dense operators
+ *     (sa_linear, sa_swiglu, sa_rmsnorm, sa_gemm_table) run on the current device.
  *   - All tensors are bf16 (raw 16-bit patterns), packed ragged: the tokens of request r are
  *     rows [qo_indptr[r], qo_indptr[r+1]) of a [T, heads, head_dim] row-major array.
  *   - There is no CPU fallback: without a CUDA device the hot calls return SA_ERR_CUDA.

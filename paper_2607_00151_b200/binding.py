@@ -191,10 +191,12 @@ def _ptr(t) -> Optional[int]:
     return t.data_ptr()
 
 
-def _stream_ptr(stream) -> Optional[int]:
+def _stream_ptr(stream, pool=None) -> Optional[int]:
+    """None = torch's current stream ON THE POOL'S DEVICE (the library runs every call on that device, whatever device is
+    current in the calling thread)."""
     if stream is None:
         import torch
-        return torch.cuda.current_stream().cuda_stream
+        return torch.cuda.current_stream(pool.cfg.device if pool is not None else None).cuda_stream
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
@@ -302,13 +304,13 @@ def sa_kv_session_truncate(pool: Pool, sid: int, new_len: int) -> None:
 
 def sa_kv_session_fork(pool: Pool, src_sid: int, prefix_len: int, stream=None) -> int:
     out = ctypes.c_int32(-1)
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_kv_session_fork(pool.handle, src_sid, prefix_len, ctypes.byref(out), sp), "sa_kv_session_fork")
     return int(out.value)
 
 
 def sa_kv_session_commit(pool: Pool, main_sid: int, lookahead_sid: int, stream=None) -> None:
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_kv_session_commit(pool.handle, main_sid, lookahead_sid, sp), "sa_kv_session_commit")
 
 
@@ -334,7 +336,7 @@ def sa_rope_kv_append(pool: Pool, sids, qo_indptr, k, v, q_inout=None, stream=No
     s_keep, s_ptr = _i32(sids)
     i_keep, i_ptr = _i32(qo_indptr)
     assert i_keep.shape[0] == s_keep.shape[0] + 1
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_rope_kv_append(pool.handle, s_keep.shape[0], s_ptr, i_ptr, _ptr(k), _ptr(v), _ptr(q_inout), sp),
            "sa_rope_kv_append")
 
@@ -353,7 +355,7 @@ def sa_mixed_attention(pool: Pool, sids, qo_indptr, q, out, lse=None, sm_scale: 
     i_keep, i_ptr = _i32(qo_indptr)
     assert i_keep.shape[0] == s_keep.shape[0] + 1
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_mixed_attention(pool.handle, s_keep.shape[0], s_ptr, i_ptr, _ptr(q), _ptr(out), _ptr(lse),
                                              float(sm_scale), _ptr(workspace), ws_bytes, sp), "sa_mixed_attention")
 
@@ -399,7 +401,7 @@ def sa_latency_table(pool: Pool, prefill_tokens, decode_batch, prefill_prefix_le
     sums = np.zeros((p_keep.shape[0], d_keep.shape[0], 2), dtype=np.int64)
     _check(load_library().sa_latency_table(pool.handle, p_ptr, p_keep.shape[0], d_ptr, d_keep.shape[0], prefill_prefix_len,
                                            decode_ctx_lo, decode_ctx_hi, seed, warmup, iters, ms.ctypes.data_as(_f32p),
-                                           sums.ctypes.data_as(_i64p), _stream_ptr(stream)), "sa_latency_table")
+                                           sums.ctypes.data_as(_i64p), _stream_ptr(stream, pool)), "sa_latency_table")
     return ms, sums
 
 
@@ -500,13 +502,13 @@ def sa_kv_wire_bytes(pool: Pool, n_tokens: int) -> int:
 
 def sa_kv_session_export(pool: Pool, sid: int, tok_begin: int, n_tokens: int, image, stream=None) -> None:
     """image: device bf16 tensor with >= 2*Hkv*n_tokens*D elements (local or peer-mapped)."""
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_kv_session_export(pool.handle, sid, tok_begin, n_tokens, _ptr(image), _nbytes(image), sp),
            "sa_kv_session_export")
 
 
 def sa_kv_session_import(pool: Pool, sid: int, n_tokens: int, image, src_heads: int, head_begin: int = 0, stream=None) -> None:
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_kv_session_import(pool.handle, sid, n_tokens, _ptr(image), src_heads, head_begin, sp),
            "sa_kv_session_import")
 
@@ -578,7 +580,7 @@ def sa_qkv_rope_append(pool: Pool, sids, qo_indptr, h, w_qkv, q_out, workspace, 
     i_keep, i_ptr = _i32(qo_indptr)
     assert i_keep.shape[0] == s_keep.shape[0] + 1
     hidden = w_qkv.shape[1]
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_qkv_rope_append(pool.handle, s_keep.shape[0], s_ptr, i_ptr, _ptr(h), _ptr(w_qkv), hidden,
                                              _ptr(q_out), _ptr(workspace), _nbytes(workspace), sp), "sa_qkv_rope_append")
 
@@ -615,7 +617,7 @@ def sa_layer_forward(pool: Pool, layer: LayerWeights, sids, qo_indptr, x, y, wor
     i_keep, i_ptr = _i32(qo_indptr)
     assert i_keep.shape[0] == s_keep.shape[0] + 1
     c = layer.to_c()
-    sp = None if pool.storage is None else _stream_ptr(stream)
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_layer_forward(pool.handle, ctypes.byref(c), s_keep.shape[0], s_ptr, i_ptr, _ptr(x), _ptr(y),
                                            float(sm_scale), _ptr(workspace), _nbytes(workspace), sp), "sa_layer_forward")
 

@@ -51,9 +51,9 @@ __global__ void __launch_bounds__(kAppendThreads)
 rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *__restrict__ reqs_slab, int32_t n_req_slab, int64_t total_rows,
                    const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
                    __nv_bfloat16 *__restrict__ q, __nv_bfloat16 *__restrict__ k_base,
-                   __nv_bfloat16 *__restrict__ v_base, const int32_t *__restrict__ block_table, int64_t mpps,
+                   __nv_bfloat16 *__restrict__ v_base, int32_t *block_table, int64_t mpps,
                    int32_t log2_page, int64_t stride_page, int64_t stride_head,
-                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv, int32_t *__restrict__ block_table_w) {
+                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
     const ReqMeta *reqs = INLINE ? im.reqs : reqs_slab;
     const int32_t n_req = INLINE ? im.n_req : n_req_slab;
     constexpr int HALF = D / 2;
@@ -79,7 +79,7 @@ rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *_
         int32_t page;
         if (INLINE && pi >= r.part_begin && pi - r.part_begin < r.n_splits) {
             page = im.pages[r.item_begin + pi - r.part_begin];       // allocated (or copied on write) by this call
-            block_table_w[int64_t(r.sid) * mpps + pi] = page;
+            block_table[int64_t(r.sid) * mpps + pi] = page;
         } else {
             page = block_table[int64_t(r.sid) * mpps + pi];
         }
@@ -166,13 +166,13 @@ static cudaError_t launch_rope_append_t(const sa_kv_pool *pool, const InlineAppe
             im, reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
             static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
             pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
-            pool->cfg.num_kv_heads, pool->block_table);
+            pool->cfg.num_kv_heads);
     else
         rope_append_kernel<64, INLINE><<<grid, kAppendThreads, 0, stream>>>(
             im, reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
             static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
             pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
-            pool->cfg.num_kv_heads, pool->block_table);
+            pool->cfg.num_kv_heads);
     ++*launches;
     return cudaGetLastError();
 }
@@ -207,6 +207,7 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
     const int B = pool->cfg.page_size;
     // ---- validate everything and size the page demand before touching any state
     std::vector<char> seen(pool->sessions.size(), 0);
+    std::vector<std::pair<int32_t, int32_t>> shared_tail;  // (shared partial last page, appenders of it in this call)
     int64_t need_pages = 0;
     for (int r = 0; r < n_req; ++r) {
         const int32_t sid = sids[r];
@@ -219,8 +220,19 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
         if (s.len + n > pool->cfg.max_session_tokens) return SA_ERR_INVALID_ARG;
         need_pages += (s.len + n + B - 1) / B - int64_t(s.pages.size());
         // copy-on-write: appending into a partly filled last page that another session also holds
-        if (n > 0 && s.len % B != 0 && pool->page_ref[size_t(s.pages.back())] > 1) ++need_pages;
+        if (n > 0 && s.len % B != 0 && pool->page_ref[size_t(s.pages.back())] > 1) {
+            bool found = false;
+            for (auto &sp : shared_tail)
+                if (sp.first == s.pages.back()) {
+                    ++sp.second;
+                    found = true;
+                }
+            if (!found) shared_tail.push_back(std::make_pair(s.pages.back(), 1));
+        }
     }
+    // a page held by c sessions of which k append into it in this call is copied min(k, c - 1) times: every copy drops a
+    // holder, and the last holder keeps the page itself
+    for (const auto &sp : shared_tail) need_pages += std::min<int64_t>(sp.second, pool->page_ref[size_t(sp.first)] - 1);
     const int64_t total = qo_indptr[n_req];
     if (need_pages > int64_t(pool->free_pages.size())) return SA_ERR_OUT_OF_PAGES;
     if (!pool->host_only && total > 0 && !have_data) return SA_ERR_INVALID_ARG;
@@ -323,6 +335,8 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
 extern "C" int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                      const int32_t *qo_indptr, const void *k, const void *v, void *q_inout,
                                      void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     using namespace sa;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const ReqMeta *reqs_dev = nullptr;

@@ -199,6 +199,8 @@ extern "C" int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n
 extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
                                       const void *q, void *out, float *lse, float sm_scale, void *workspace,
                                       size_t workspace_bytes, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     using namespace sa;
     HostPlan hp;
     int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hp);

@@ -18,10 +18,7 @@ namespace {
 
 constexpr int kThreads = 128;
 constexpr int kBN = 64;      // keys per tile
-#ifndef SA_DEC_STAGES
-#define SA_DEC_STAGES 3
-#endif
-constexpr int kStages = SA_DEC_STAGES;
+constexpr int kStages = 3;   // cp.async ring depth (64 KiB of K/V in flight per CTA)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));

@@ -12,10 +12,7 @@
 namespace sa {
 
 constexpr int kMetaRing = 8;            // per-call metadata slabs in flight
-#ifndef SA_DEC_SPLIT
-#define SA_DEC_SPLIT 1024
-#endif
-constexpr int kDecodeSplitKeys = SA_DEC_SPLIT;  // split-KV granularity of decode-like rows (logical keys)
+constexpr int kDecodeSplitKeys = 1024;  // split-KV granularity of decode-like rows (logical keys)
 constexpr int kTc5TileM = 256;          // packed rows per CTA of the tcgen05 prefill kernel
 constexpr int kMaxChunkLatency = 2048;  // sa_latency_table prefill chunk size
 constexpr int kTc5KeysPerUnit = 128;    // one schedule unit of the tcgen05 kernel = one 128-key KV tile of an item
@@ -128,6 +125,34 @@ struct sa_kv_pool {
 };
 
 namespace sa {
+
+// Every entry point that touches the device runs on the POOL's device (cfg.device), whatever device is current in the
+// calling thread, and leaves the caller's current device as it found it.  Host-only pools and null pools: a no-op.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false, ok = true;
+    explicit DeviceGuard(const sa_kv_pool *pool) {
+        if (pool && !pool->host_only) enter(pool->cfg.device);
+    }
+    explicit DeviceGuard(int device) { enter(device); }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+
+  private:
+    void enter(int device) {
+        if (cudaGetDevice(&prev) != cudaSuccess) {
+            ok = false;
+            return;
+        }
+        if (prev != device) {
+            ok = cudaSetDevice(device) == cudaSuccess;
+            switched = ok;
+        }
+    }
+};
 
 // Reserve the next metadata slab (host pinned + device twin); waits for the slab's previous
 // copy if it is still in flight.  commit_meta enqueues the H2D copy of `bytes` bytes.

@@ -71,6 +71,8 @@ extern "C" int32_t sa_latency_table(sa_kv_pool *pool, const int32_t *prefill_tok
                                     const int32_t *decode_batch, int32_t n_d, int64_t prefill_prefix_len,
                                     int64_t decode_ctx_lo, int64_t decode_ctx_hi, uint64_t seed, int32_t warmup,
                                     int32_t iters, float *out_ms, int64_t *out_sum_kv, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     if (!pool || !prefill_tokens || !decode_batch || !out_ms || n_p <= 0 || n_d <= 0 || iters <= 0 || warmup < 0 ||
         prefill_prefix_len < 0 || decode_ctx_lo < 1 || decode_ctx_hi < decode_ctx_lo)
         return SA_ERR_INVALID_ARG;

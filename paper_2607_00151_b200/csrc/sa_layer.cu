@@ -98,6 +98,8 @@ extern "C" int32_t sa_qkv_rope_append_workspace_bytes(const sa_kv_pool *pool, in
 extern "C" int32_t sa_qkv_rope_append(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
                                       const void *h, const void *w_qkv, int32_t hidden, void *q_out, void *workspace,
                                       size_t workspace_bytes, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     using namespace sa;
     if (!pool || n_req < 0 || hidden <= 0) return SA_ERR_INVALID_ARG;
     if (pool->cfg.head_dim != 128 || hidden % 64 != 0) return SA_ERR_UNSUPPORTED;
@@ -133,6 +135,8 @@ extern "C" int32_t sa_layer_workspace_bytes(const sa_kv_pool *pool, const sa_lay
 extern "C" int32_t sa_layer_forward(sa_kv_pool *pool, const sa_layer_weights *L, int32_t n_req, const int32_t *sids,
                                     const int32_t *qo_indptr, const void *x, void *y, float sm_scale, void *workspace,
                                     size_t workspace_bytes, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     using namespace sa;
     int32_t st = check_layer(pool, L);
     if (st != SA_OK) return st;

@@ -119,7 +119,8 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
         pool->block_table = reinterpret_cast<int32_t *>(base + cv.bt_off);
         pool->rope_tab = reinterpret_cast<float2 *>(base + cv.rope_off);
         pool->meta_dev = base + cv.meta_off;
-        bool ok = cudaSetDevice(cfg->device) == cudaSuccess;
+        sa::DeviceGuard device_guard(cfg->device);  // the caller's current device is restored on return
+        bool ok = device_guard.ok;
         ok = ok && cudaMallocHost(reinterpret_cast<void **>(&pool->meta_host), cv.slab * sa::kMetaRing) == cudaSuccess;
         for (int i = 0; ok && i < sa::kMetaRing; ++i)
             ok = cudaEventCreateWithFlags(&pool->meta_event[i], cudaEventDisableTiming) == cudaSuccess;
@@ -152,6 +153,8 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
 }
 
 extern "C" int32_t sa_kv_pool_destroy(sa_kv_pool *pool) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     if (!pool) return SA_ERR_INVALID_ARG;
     if (!pool->host_only) {
         for (int i = 0; i < sa::kMetaRing; ++i) {
@@ -232,6 +235,8 @@ static int32_t upload_row(sa_kv_pool *pool, int32_t sid, cudaStream_t stream) {
 }
 
 extern "C" int32_t sa_kv_session_fork(sa_kv_pool *pool, int32_t src_sid, int64_t prefix_len, int32_t *out_sid, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     sa::Session *src = get_session(pool, src_sid);
     if (!src || !out_sid || prefix_len < 0 || prefix_len > src->len) return SA_ERR_INVALID_ARG;
     const int B = pool->cfg.page_size;
@@ -267,6 +272,8 @@ extern "C" int32_t sa_kv_session_fork(sa_kv_pool *pool, int32_t src_sid, int64_t
 }
 
 extern "C" int32_t sa_kv_session_commit(sa_kv_pool *pool, int32_t main_sid, int32_t lookahead_sid, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     sa::Session *m = get_session(pool, main_sid);
     sa::Session *la = get_session(pool, lookahead_sid);
     if (!m || !la || main_sid == lookahead_sid) return SA_ERR_INVALID_ARG;

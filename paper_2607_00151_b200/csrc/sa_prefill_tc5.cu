@@ -38,20 +38,9 @@ constexpr int kThreadsTc5 = 384;
 constexpr int TILE_BYTES = BN * DMAX * 2;   // 32 KiB: two 64-wide halves of 128 rows x 128 B (head_dim 64 uses the first)
 constexpr int HALF_BYTES = TILE_BYTES / 2;
 constexpr int KV_STAGES = 2;
-#ifndef SA_POLY_SHARE
-#define SA_POLY_SHARE 2  // n of every 8 column pairs take exp2 as a packed cubic on the FMA pipe, the rest the MUFU
-#endif
+constexpr int kPolyShare = 2;  // of every 8 column pairs, this many take exp2 as a packed cubic on the FMA pipe, the rest the MUFU
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only when the row max grows by > 2^8
 
-#ifdef SA_TC5_PROBE
-// debug build only (-DSA_TC5_PROBE): per-CTA (clock64, globaltimer) at start and end, read back by sa_debug_tc5_probe
-__device__ unsigned long long g_tc5_probe[256][4];
-__device__ __forceinline__ unsigned long long gtimer() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-    return t;
-}
-#endif
 
 struct Tc5Args {
     const ReqMeta *reqs;
@@ -131,7 +120,7 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&s)[32]) {
     const float a3 = max3(l1[9], __uint_as_float(s[30]), __uint_as_float(s[31]));
     return fmaxf(max3(a0, a1, a2), a3);
 }
-// exp2 of column pairs [I0, I1) of one chunk, row sums, bf16 P packed into pk.  SA_POLY_SHARE of every eight column
+// exp2 of column pairs [I0, I1) of one chunk, row sums, bf16 P packed into pk.  kPolyShare of every eight column
 // pairs take the packed cubic on the FMA pipe (never on masked tiles: -inf must give exactly 0).
 template <bool MASKED, int I0, int I1>
 __device__ __forceinline__ void chunk_exp(const uint32_t (&s)[32], uint64_t sl2_2, uint64_t neg_2, uint64_t (&lsum)[4],
@@ -142,7 +131,7 @@ __device__ __forceinline__ void chunk_exp(const uint32_t (&s)[32], uint64_t sl2_
         float x0, x1;
         unpack_f32x2(ffma2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sl2_2, neg_2), x0, x1);
         float p0, p1;
-        if (!MASKED && (i & 7) < SA_POLY_SHARE) {
+        if (!MASKED && (i & 7) < kPolyShare) {
             ex2_poly3_x2(x0, x1, p0, p1);
         } else {
             p0 = ex2_approx(x0);
@@ -180,12 +169,6 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     // ---- the parts of this persistent CTA (uniform over the CTA: an idle CTA leaves at once)
     const int pb = a.cta_begin[blockIdx.x], pe = a.cta_begin[blockIdx.x + 1];
     if (pb == pe) return;
-#ifdef SA_TC5_PROBE
-    if (threadIdx.x == 0) {
-        g_tc5_probe[blockIdx.x][0] = clock64();
-        g_tc5_probe[blockIdx.x][1] = gtimer();
-    }
-#endif
 
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -540,12 +523,6 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     tc_fence_before();
     __syncthreads();
     if (warp == 2) tmem_dealloc<512>(tmem);
-#ifdef SA_TC5_PROBE
-    if (threadIdx.x == 0) {
-        g_tc5_probe[blockIdx.x][2] = clock64();
-        g_tc5_probe[blockIdx.x][3] = gtimer();
-    }
-#endif
 }
 
 // Merge of the parts of split items, in KV order (fixed, so bit-reproducible).  grid = (split
@@ -624,11 +601,6 @@ constexpr size_t kSmemTc5 = size_t(2 + 2 * KV_STAGES) * TILE_BYTES + 1024;
 
 }  // namespace
 
-#ifdef SA_TC5_PROBE
-extern "C" __attribute__((visibility("default"))) int32_t sa_debug_tc5_probe(unsigned long long *out) {
-    return cudaMemcpyFromSymbol(out, g_tc5_probe, sizeof(unsigned long long) * 256 * 4) == cudaSuccess ? 0 : -4;
-}
-#endif
 
 void *tensor_map_encode_fn() { return reinterpret_cast<void *>(get_encode()); }
 

@@ -10,6 +10,8 @@
 // of the pseudo-code's EstBatchLatency(B + {c}); the value is the same bit for bit).
 #include <math.h>
 
+#include <cmath>
+
 #include "sa_internal.h"
 
 namespace {
@@ -176,7 +178,10 @@ extern "C" int32_t sa_dynamic_chunk(const sa_latency_model *model, const int64_t
         remaining < 0 || max_chunk <= 0 || granularity <= 0)
         return SA_ERR_INVALID_ARG;
     Sums s;
-    for (int32_t i = 0; i < n_dec; ++i) s = with_decode(s, decode_L[i]);
+    for (int32_t i = 0; i < n_dec; ++i) {
+        if (decode_L[i] < 0) return SA_ERR_INVALID_ARG;
+        s = with_decode(s, decode_L[i]);
+    }
     for (int32_t i = 0; i < n_pre; ++i) s = with_chunk(s, chunks[i]);
     const int64_t top = remaining < max_chunk ? remaining : max_chunk;
     auto fits = [&](int64_t q) { return est(model, with_chunk(s, sa_chunk{q, prefix})) <= budget_ms; };
@@ -186,8 +191,21 @@ extern "C" int32_t sa_dynamic_chunk(const sa_latency_model *model, const int64_t
         *out_q = top;
         return SA_OK;
     }
-    // Eq. 1 grows with q: bisect over the multiples of the granularity below `top`
     int64_t lo = 0, hi = (top - 1) / granularity;  // candidates k * granularity, k in [1, hi]
+    // Eq. 1 grows with q when alpha_p >= 0 and T_GEMM does not decrease: then bisect over the candidates.  A profiled table
+    // (medians of measurements) or an unconstrained fit need not be monotone; then "the largest that fits" is found the way
+    // it is defined, by scanning down from the top.
+    bool monotone = model->alpha_p_ms >= 0.0 && std::isfinite(model->alpha_p_ms);
+    for (int i = 0; monotone && i < model->n_gemm; ++i)
+        monotone = std::isfinite(model->gemm_ms[i]) && (i == 0 || model->gemm_ms[i] >= model->gemm_ms[i - 1]);
+    if (!monotone) {
+        for (int64_t k = hi; k >= 1; --k)
+            if (fits(k * granularity)) {
+                *out_q = k * granularity;
+                return SA_OK;
+            }
+        return SA_OK;
+    }
     while (lo < hi) {
         const int64_t mid = (lo + hi + 1) / 2;
         if (fits(mid * granularity)) lo = mid; else hi = mid - 1;

@@ -126,6 +126,8 @@ extern "C" int32_t sa_kv_wire_bytes(const sa_kv_pool *pool, int64_t n_tokens, si
 
 extern "C" int32_t sa_kv_session_export(sa_kv_pool *pool, int32_t sid, int64_t tok_begin, int64_t n_tokens, void *image,
                                         size_t image_bytes, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     if (!pool || sid < 0 || size_t(sid) >= pool->sessions.size() || !pool->sessions[size_t(sid)].open)
         return SA_ERR_INVALID_ARG;
     const sa::Session &s = pool->sessions[size_t(sid)];
@@ -150,6 +152,8 @@ extern "C" int32_t sa_kv_session_export(sa_kv_pool *pool, int32_t sid, int64_t t
 
 extern "C" int32_t sa_kv_session_import(sa_kv_pool *pool, int32_t sid, int64_t n_tokens, const void *image,
                                         int32_t src_heads, int32_t head_begin, void *stream_) {
+    sa::DeviceGuard device_guard(pool);
+    if (!device_guard.ok) return SA_ERR_CUDA;
     if (!pool || n_tokens < 0 || n_tokens > INT32_MAX) return SA_ERR_INVALID_ARG;
     if (src_heads <= 0 || head_begin < 0 || head_begin + pool->cfg.num_kv_heads > src_heads) return SA_ERR_INVALID_ARG;
     if (!pool->host_only && n_tokens > 0 && (!image || (reinterpret_cast<uintptr_t>(image) & 15))) return SA_ERR_INVALID_ARG;

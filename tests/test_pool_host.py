@@ -288,3 +288,37 @@ def test_import_books_pages_like_an_append_and_validates_the_head_slice():
     with pytest.raises(sa.SAError) as ei:
         sa.sa_kv_session_export(p, s, 40, 10, None)
     assert ei.value.status == sa.SA_ERR_INVALID_ARG
+
+
+def test_two_appenders_of_one_shared_partial_page_need_one_copy():
+    """Two sessions that share a partly filled last page (forked at a page boundary, then both truncated into the shared
+    page) append in ONE call: the page is copied for the first appender only -- the second is then its last holder -- so the
+    call needs one free page, not two (the demand is min(appenders, holders - 1) per shared page)."""
+    p = _pool(num_pages=4, max_sessions=4)
+    a = sa.sa_kv_session_open(p)
+    sa.sa_rope_kv_append(p, [a], [0, 40], None, None)          # 3 pages
+    b = sa.sa_kv_session_fork(p, a, 32)                        # shares pages 0 and 1, nothing copied
+    sa.sa_kv_session_truncate(p, a, 20)                        # page 2 back to the pool; page 1 now partial in both
+    sa.sa_kv_session_truncate(p, b, 20)
+    c = sa.sa_kv_session_open(p)
+    sa.sa_rope_kv_append(p, [c], [0, 1], None, None)           # takes one of the two free pages
+    assert sa.sa_kv_pool_free_pages(p) == 1
+    shared = sa.sa_kv_session_query(p, a)[1][1]
+    assert sa.sa_kv_session_query(p, b)[1][1] == shared and sa.sa_kv_page_refcount(p, shared) == 2
+    sa.sa_rope_kv_append(p, [a, b], [0, 4, 8], None, None)     # both fit in their partial page: one copy-on-write in all
+    pa, pb = sa.sa_kv_session_query(p, a)[1], sa.sa_kv_session_query(p, b)[1]
+    assert sa.sa_kv_session_query(p, a)[0] == 24 and sa.sa_kv_session_query(p, b)[0] == 24
+    assert pa[0] == pb[0] and pa[1] != pb[1] and pb[1] == shared
+    assert sa.sa_kv_page_refcount(p, pa[1]) == 1 and sa.sa_kv_page_refcount(p, pb[1]) == 1
+    assert sa.sa_kv_pool_free_pages(p) == 0
+    # and with no free page left the same situation is refused without touching anything
+    sa.sa_kv_session_truncate(p, a, 16)                        # a's private copy back to the pool (1 free page)
+    d = sa.sa_kv_session_fork(p, b, 16)                        # shares page 0 only
+    sa.sa_rope_kv_append(p, [d], [0, 1], None, None)           # takes the free page
+    assert sa.sa_kv_pool_free_pages(p) == 0
+    sa.sa_kv_session_truncate(p, a, 8)
+    sa.sa_kv_session_truncate(p, d, 8)                         # d's page freed; a, b, d all hold page 0; a and d partial in it
+    assert sa.sa_kv_pool_free_pages(p) == 1
+    with pytest.raises(sa.SAError):
+        sa.sa_rope_kv_append(p, [a, d], [0, 1, 2], None, None)  # holders 3 (b keeps it), appenders 2: two copies, one page
+    assert sa.sa_kv_session_query(p, a)[0] == 8 and sa.sa_kv_session_query(p, d)[0] == 8 and sa.sa_kv_pool_free_pages(p) == 1

@@ -83,6 +83,39 @@ def test_dynamic_chunk_equals_the_oracle_scan():
             assert got == so.dynamic_chunk(m, dec, lc, prefix, remaining, 2048, gran, budget)
 
 
+def test_dynamic_chunk_with_a_non_monotone_model_equals_the_oracle_scan():
+    """A measured T_GEMM table (medians) or an unconstrained fit need not be monotone in q; "the largest chunk that fits"
+    is then not found by bisection.  The C++ side must fall back to the definition (scan from the top), like the oracle."""
+    rng = np.random.default_rng(15)
+    models = [
+        {"c0": 0.0, "alpha_d": 2.5e-7, "alpha_p": 1.9e-8,   # a dip at M = 256 (a faster kernel variant kicks in)
+         "gemm": [(1, 0.35), (64, 0.50), (256, 0.30), (1024, 1.61), (2048, 1.2), (4096, 6.2)]},
+        {"c0": 0.5, "alpha_d": 1e-7, "alpha_p": -2e-9, "gemm": [(1, 0.2), (2048, 3.0)]},   # a negative fitted coefficient
+    ]
+    differs_from_bisection = 0
+    for m in models:
+        for _ in range(150):
+            dec, lc, _ = _rand_batch(rng)
+            prefix, remaining = int(rng.integers(0, 60000)), int(rng.integers(1, 9000))
+            gran = int(rng.choice([16, 64, 128]))
+            top_est = so.est_batch_latency(m, dec, lc + [(min(remaining, 2048), prefix)])
+            budget = float(rng.uniform(0.3, 1.1) * top_est)
+            ref = so.dynamic_chunk(m, dec, lc, prefix, remaining, 2048, gran, budget)
+            assert sa.sa_dynamic_chunk(_to(m), dec, lc, prefix, remaining, 2048, gran, budget) == ref
+            # what a bisection that assumes monotonicity would have returned
+            top = min(remaining, 2048)
+            fits = lambda q: so.est_batch_latency(m, dec, lc + [(q, prefix)]) <= budget
+            if not fits(top):
+                lo, hi = 0, (top - 1) // gran
+                while lo < hi:
+                    mid = (lo + hi + 1) // 2
+                    lo, hi = (mid, hi) if fits(mid * gran) else (lo, mid - 1)
+                differs_from_bisection += int(lo * gran != ref)
+    assert differs_from_bisection > 0   # the instances do exercise the difference
+    with pytest.raises(sa.SAError):
+        sa.sa_dynamic_chunk(_to(models[0]), [100, -1], [], 0, 100, 2048, 16, 1.0)
+
+
 def test_fit_equals_numpy_least_squares():
     rng = np.random.default_rng(14)
     for with_c0 in (True, False):
