@@ -167,6 +167,8 @@ SA_API int32_t sa_rope_kv_append(sa_kv_pool *pool, int32_t n_req, const int32_t 
  * prefill requests of the call (their work is balanced over the SMs by cutting items along KV,
  * see sa_mixed_attention_schedule) and not on the decode rows co-batched with them; neither depends
  * on which physical pages hold the cache.  Contents of page slots >= kv_r never influence a result, NaN included.
+ * The call only reads the cache, so a session may be named by several requests of one call; each request is then what
+ * it would be alone (its rows are the last q_r tokens of that session).  sa_rope_kv_append, which writes, refuses that.
  *   q    : device bf16 [T, Hq, D], already rotated (sa_rope_kv_append's q_inout)
  *   out  : device bf16 [T, Hq, D]
  *   lse  : device f32 [T, Hq], nullable; natural-log sum-exp of the scaled scores of the row
@@ -212,17 +214,23 @@ SA_API int32_t sa_last_launch_count(const sa_kv_pool *pool, int32_t *out_launche
  * profiled", L303).  Prefill tokens p are issued as ceil(p/2048) chunks of <= 2048 tokens, each
  * over its own prefix of prefill_prefix_len tokens; decode rows have contexts drawn uniformly
  * from [decode_ctx_lo, decode_ctx_hi] with a counter-based generator seeded by seed.
- * NOT a hot call: it opens scratch sessions in the pool's free pages, allocates its own
- * temporary device buffers (cudaMalloc), synchronises the stream, and closes the sessions
- * before returning.  Between timed iterations it evicts L2 by writing a 256 MiB buffer.
+ * NOT a hot call: it opens scratch sessions in the pool's free pages (at most max(decode_batch) + ceil(max(prefill_tokens)
+ * / 2048) of them: SA_ERR_OUT_OF_SESSIONS / SA_ERR_OUT_OF_PAGES before anything is opened), synchronises the stream, and
+ * closes the sessions before returning.  It allocates no device memory: its source K/V, queries, outputs, the 256 MiB buffer
+ * it writes between timed iterations to evict L2 and the attention workspace all come from `workspace`
+ * (>= sa_latency_table_workspace_bytes for the same arguments; that call replays the run's sessions on a host-only twin of
+ * the pool, so the figure is the planner's own).
  *   out_ms : host float [n_p][n_d], median over iters of CUDA-event times on `stream`
  *   out_sum_kv (nullable): host int64 [n_p][n_d][2] = {sum_j L_j of the decode rows,
  *                          sum_j A_j of the prefill chunks} for fitting alpha_d, alpha_p */
+SA_API int32_t sa_latency_table_workspace_bytes(const sa_kv_pool *pool, const int32_t *prefill_tokens, int32_t n_p,
+                                         const int32_t *decode_batch, int32_t n_d, int64_t prefill_prefix_len,
+                                         int64_t decode_ctx_lo, int64_t decode_ctx_hi, uint64_t seed, size_t *out_bytes);
 SA_API int32_t sa_latency_table(sa_kv_pool *pool, const int32_t *prefill_tokens, int32_t n_p,
                          const int32_t *decode_batch, int32_t n_d, int64_t prefill_prefix_len,
                          int64_t decode_ctx_lo, int64_t decode_ctx_hi, uint64_t seed,
                          int32_t warmup, int32_t iters, float *out_ms, int64_t *out_sum_kv,
-                         void *stream);
+                         void *workspace, size_t workspace_bytes, void *stream);
 
 /* ---- lookahead-aware scheduler core (section 4) --------------
  * Host-only calls (no device work, no pool): the consumer of sa_latency_table.
@@ -383,12 +391,15 @@ SA_API int32_t sa_layer_forward(sa_kv_pool *pool, const sa_layer_weights *layer,
 /* T_GEMM(M), the "offline-profiled lookup table" of L303: for every M in m_list the time of the layer's
  * dense operators on M tokens (QKV projection, output projection + residual, SwiGLU GEMM, down
  * projection + residual, the two RMSNorms), median over iters of CUDA-event times on `stream`, L2
- * evicted between iterations.  NOT a hot call: allocates its own activations and weights of the given
- * shape (cudaMalloc, values irrelevant to the timing), synchronises, frees.  The result goes into
- * sa_latency_model.gemm_m / gemm_ms. */
+ * evicted between iterations.  NOT a hot call (it synchronises), but it allocates nothing: weights and activations of the
+ * given shape (values irrelevant to the timing), the L2-eviction buffer and the split-K scratch are carved from `workspace`
+ * (device, >= sa_gemm_table_workspace_bytes for the same arguments; about 0.8 GB for the Llama-3-8B layer at M = 8192).
+ * The result goes into sa_latency_model.gemm_m / gemm_ms. */
+SA_API int32_t sa_gemm_table_workspace_bytes(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads,
+                                      int32_t head_dim, const int32_t *m_list, int32_t n_m, size_t *out_bytes);
 SA_API int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
                       const int32_t *m_list, int32_t n_m, int32_t warmup, int32_t iters, float *out_ms,
-                      void *stream);
+                      void *workspace, size_t workspace_bytes, void *stream);
 
 /* ---- KV hand-over between pools ----------------------------------------------------
  * in PD-disaggregated serving "KV transfer" moves a request's cache from the prefill
@@ -412,6 +423,17 @@ SA_API int32_t sa_kv_session_export(sa_kv_pool *pool, int32_t sid, int64_t tok_b
  * failure behaviour are sa_rope_kv_append's (SA_ERR_OUT_OF_PAGES changes nothing); nothing is rotated. */
 SA_API int32_t sa_kv_session_import(sa_kv_pool *pool, int32_t sid, int64_t n_tokens, const void *image, int32_t src_heads,
                              int32_t head_begin, void *stream);
+
+/* The same two operations for MANY sessions in one call and one kernel launch each (a PD hand-over moves every request of a
+ * batch; one launch per session leaves the copy host- and launch-bound).  Range i is tokens [tok_begin[i], tok_begin[i] +
+ * n_tokens[i]) of session sids[i] and has its own image (images[i], image_bytes[i]; any mix of local and peer addresses);
+ * a session may appear in several ranges of an export.  Import: session sids[i] (each at most once) grows by n_tokens[i]
+ * tokens from images[i]; page allocation is all-or-nothing over the whole call.  sids, tok_begin, n_tokens, images,
+ * image_bytes are HOST arrays of n entries, copied before the call returns; at most 4 x max_sessions ranges per export. */
+SA_API int32_t sa_kv_sessions_export(sa_kv_pool *pool, int32_t n_ranges, const int32_t *sids, const int64_t *tok_begin,
+                              const int64_t *n_tokens, void *const *images, const size_t *image_bytes, void *stream);
+SA_API int32_t sa_kv_sessions_import(sa_kv_pool *pool, int32_t n_sessions, const int32_t *sids, const int64_t *n_tokens,
+                              const void *const *images, int32_t src_heads, int32_t head_begin, void *stream);
 
 #ifdef __cplusplus
 }

@@ -113,8 +113,11 @@ PROTOTYPES = {
     "sa_mixed_attention_plan": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _i64p]),
     "sa_mixed_attention_schedule": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i32p, _i32p, ctypes.c_int32, _i64p]),
     "sa_last_launch_count": (ctypes.c_int32, [_vp, _i32p]),
+    "sa_latency_table_workspace_bytes": (ctypes.c_int32, [_vp, _i32p, ctypes.c_int32, _i32p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
+                                                          ctypes.c_int64, ctypes.c_uint64, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_latency_table": (ctypes.c_int32, [_vp, _i32p, ctypes.c_int32, _i32p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
-                                          ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32, ctypes.c_int32, _f32p, _i64p, _vp]),
+                                          ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32, ctypes.c_int32, _f32p, _i64p, _vp,
+                                          ctypes.c_size_t, _vp]),
     "sa_latency_fit": (ctypes.c_int32, [_f32p, _i64p, ctypes.c_int32, ctypes.c_int32, _modelp, _f64p]),
     "sa_est_batch_latency": (ctypes.c_int32, [_modelp, _i64p, ctypes.c_int32, _chunkp, ctypes.c_int32, _f64p]),
     "sa_schedule_hybrid": (ctypes.c_int32, [_modelp, _i64p, ctypes.c_int32, _chunkp, ctypes.c_int32, _chunkp, ctypes.c_int32,
@@ -133,8 +136,10 @@ PROTOTYPES = {
                                                   ctypes.POINTER(ctypes.c_size_t)]),
     "sa_layer_forward": (ctypes.c_int32, [_vp, ctypes.POINTER(sa_layer_weights), ctypes.c_int32, _i32p, _i32p, _vp, _vp,
                                           ctypes.c_float, _vp, ctypes.c_size_t, _vp]),
+    "sa_gemm_table_workspace_bytes": (ctypes.c_int32, [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p,
+                                                       ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_gemm_table": (ctypes.c_int32, [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p,
-                                       ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _f32p, _vp]),
+                                       ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _f32p, _vp, ctypes.c_size_t, _vp]),
     "sa_linear_workspace_bytes": (ctypes.c_int32, [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_linear_ws": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp, ctypes.c_size_t, _vp]),
     "sa_swiglu_workspace_bytes": (ctypes.c_int32, [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
@@ -142,6 +147,10 @@ PROTOTYPES = {
     "sa_kv_wire_bytes": (ctypes.c_int32, [_vp, ctypes.c_int64, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_kv_session_export": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, _vp, ctypes.c_size_t, _vp]),
     "sa_kv_session_import": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, _vp, ctypes.c_int32, ctypes.c_int32, _vp]),
+    "sa_kv_sessions_export": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i64p, _i64p, ctypes.POINTER(ctypes.c_void_p),
+                                               ctypes.POINTER(ctypes.c_size_t), _vp]),
+    "sa_kv_sessions_import": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i64p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int32,
+                                               ctypes.c_int32, _vp]),
 }
 
 _lib = None
@@ -392,16 +401,35 @@ def sa_last_launch_count(pool: Pool) -> int:
     return int(out.value)
 
 
+def sa_latency_table_workspace_bytes(pool: Pool, prefill_tokens, decode_batch, prefill_prefix_len: int, decode_ctx_lo: int,
+                                     decode_ctx_hi: int, seed: int = 0) -> int:
+    p_keep, p_ptr = _i32(prefill_tokens)
+    d_keep, d_ptr = _i32(decode_batch)
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_latency_table_workspace_bytes(pool.handle, p_ptr, p_keep.shape[0], d_ptr, d_keep.shape[0],
+                                                           prefill_prefix_len, decode_ctx_lo, decode_ctx_hi, seed, ctypes.byref(out)),
+           "sa_latency_table_workspace_bytes")
+    return int(out.value)
+
+
 def sa_latency_table(pool: Pool, prefill_tokens, decode_batch, prefill_prefix_len: int, decode_ctx_lo: int,
-                     decode_ctx_hi: int, seed: int = 0, warmup: int = 3, iters: int = 10, stream=None):
-    """-> (ms [n_p, n_d] float32, sums [n_p, n_d, 2] int64 = (sum L_j, sum A_j))"""
+                     decode_ctx_hi: int, seed: int = 0, warmup: int = 3, iters: int = 10, stream=None, workspace=None):
+    """-> (ms [n_p, n_d] float32, sums [n_p, n_d, 2] int64 = (sum L_j, sum A_j)).
+    workspace: device uint8 tensor of >= sa_latency_table_workspace_bytes(...) bytes; None = one is taken from torch here."""
     p_keep, p_ptr = _i32(prefill_tokens)
     d_keep, d_ptr = _i32(decode_batch)
     ms = np.zeros((p_keep.shape[0], d_keep.shape[0]), dtype=np.float32)
     sums = np.zeros((p_keep.shape[0], d_keep.shape[0], 2), dtype=np.int64)
+    if workspace is None and pool.storage is not None:
+        import torch
+        workspace = torch.empty(sa_latency_table_workspace_bytes(pool, prefill_tokens, decode_batch, prefill_prefix_len,
+                                                                 decode_ctx_lo, decode_ctx_hi, seed), dtype=torch.uint8,
+                                device=pool.storage.device)
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     _check(load_library().sa_latency_table(pool.handle, p_ptr, p_keep.shape[0], d_ptr, d_keep.shape[0], prefill_prefix_len,
                                            decode_ctx_lo, decode_ctx_hi, seed, warmup, iters, ms.ctypes.data_as(_f32p),
-                                           sums.ctypes.data_as(_i64p), _stream_ptr(stream, pool)), "sa_latency_table")
+                                           sums.ctypes.data_as(_i64p), _ptr(workspace), ws_bytes,
+                                           None if pool.storage is None else _stream_ptr(stream, pool)), "sa_latency_table")
     return ms, sums
 
 
@@ -513,6 +541,31 @@ def sa_kv_session_import(pool: Pool, sid: int, n_tokens: int, image, src_heads: 
            "sa_kv_session_import")
 
 
+
+
+def sa_kv_sessions_export(pool: Pool, sids, tok_begin, n_tokens, images, stream=None) -> None:
+    """Many session ranges -> their wire images in one call (one kernel launch).  images: one device tensor per range."""
+    s_keep, s_ptr = _i32(sids)
+    b_keep, b_ptr = _i64(tok_begin)
+    n_keep, n_ptr = _i64(n_tokens)
+    n = s_keep.shape[0]
+    assert b_keep.shape[0] == n and n_keep.shape[0] == n and len(images) == n
+    ptrs = (ctypes.c_void_p * max(n, 1))(*[_ptr(im) for im in images])
+    sizes = (ctypes.c_size_t * max(n, 1))(*[0 if im is None else im.numel() * im.element_size() for im in images])
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
+    _check(load_library().sa_kv_sessions_export(pool.handle, n, s_ptr, b_ptr, n_ptr, ptrs, sizes, sp), "sa_kv_sessions_export")
+
+
+def sa_kv_sessions_import(pool: Pool, sids, n_tokens, images, src_heads: int, head_begin: int = 0, stream=None) -> None:
+    """Many sessions grow from their wire images in one call (one kernel launch; page allocation all-or-nothing)."""
+    s_keep, s_ptr = _i32(sids)
+    n_keep, n_ptr = _i64(n_tokens)
+    n = s_keep.shape[0]
+    assert n_keep.shape[0] == n and len(images) == n
+    ptrs = (ctypes.c_void_p * max(n, 1))(*[_ptr(im) for im in images])
+    sp = None if pool.storage is None else _stream_ptr(stream, pool)
+    _check(load_library().sa_kv_sessions_import(pool.handle, n, s_ptr, n_ptr, ptrs, src_heads, head_begin, sp), "sa_kv_sessions_import")
+
 # ---------------------------------------------------------------- dense operators of the layer (N3)
 def _nbytes(t) -> int:
     return 0 if t is None else t.numel() * t.element_size()
@@ -622,11 +675,25 @@ def sa_layer_forward(pool: Pool, layer: LayerWeights, sids, qo_indptr, x, y, wor
                                            float(sm_scale), _ptr(workspace), _nbytes(workspace), sp), "sa_layer_forward")
 
 
+def sa_gemm_table_workspace_bytes(hidden: int, ffn: int, num_q_heads: int, num_kv_heads: int, head_dim: int, m_list) -> int:
+    m_keep, m_ptr = _i32(m_list)
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_gemm_table_workspace_bytes(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_ptr, m_keep.shape[0],
+                                                        ctypes.byref(out)), "sa_gemm_table_workspace_bytes")
+    return int(out.value)
+
+
 def sa_gemm_table(hidden: int, ffn: int, num_q_heads: int, num_kv_heads: int, head_dim: int, m_list, warmup: int = 3,
-                  iters: int = 10, stream=None):
-    """-> ms float32 [len(m_list)]: T_GEMM(M) of PAPER.md L299-303 measured on this library's kernels."""
+                  iters: int = 10, stream=None, workspace=None):
+    """-> ms float32 [len(m_list)]: T_GEMM(M) of PAPER.md L299-303 measured on this library's kernels.
+    workspace: device uint8 tensor of >= sa_gemm_table_workspace_bytes(...) bytes; None = one is taken from torch here."""
     m_keep, m_ptr = _i32(m_list)
     ms = np.zeros(m_keep.shape[0], dtype=np.float32)
+    if workspace is None:
+        import torch
+        workspace = torch.empty(sa_gemm_table_workspace_bytes(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_list),
+                                dtype=torch.uint8, device="cuda")
     _check(load_library().sa_gemm_table(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_ptr, m_keep.shape[0], warmup, iters,
-                                        ms.ctypes.data_as(_f32p), _stream_ptr(stream)), "sa_gemm_table")
+                                        ms.ctypes.data_as(_f32p), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                        _stream_ptr(stream)), "sa_gemm_table")
     return ms

@@ -183,46 +183,76 @@ extern "C" int32_t sa_layer_forward(sa_kv_pool *pool, const sa_layer_weights *L,
     return SA_OK;
 }
 
-extern "C" int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
-                                 const int32_t *m_list, int32_t n_m, int32_t warmup, int32_t iters, float *out_ms,
-                                 void *stream_) {
-    using namespace sa;
-    if (!m_list || !out_ms || n_m <= 0 || iters <= 0 || warmup < 0 || hidden <= 0 || ffn <= 0 || num_q_heads <= 0 ||
-        num_kv_heads <= 0 || head_dim <= 0)
+namespace {
+constexpr size_t kGemmTableFlush = size_t(256) << 20;          // larger than the 126 MB L2
+constexpr size_t kGemmTableSplitK = size_t(160) * 128 * 1024;  // split-K scratch: tiles x slices never exceeds the SM count
+inline size_t gt_up(size_t b) { return (std::max<size_t>(b, 256) + 255) / 256 * 256; }
+int32_t gemm_table_check(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
+                         const int32_t *m_list, int32_t n_m, int32_t *m_max) {
+    if (!m_list || n_m <= 0 || hidden <= 0 || ffn <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || head_dim <= 0)
         return SA_ERR_INVALID_ARG;
     if (hidden % 64 != 0 || ffn % 64 != 0 || (num_q_heads * head_dim) % 64 != 0) return SA_ERR_UNSUPPORTED;
-    int32_t m_max = 0;
+    *m_max = 0;
     for (int i = 0; i < n_m; ++i) {
         if (m_list[i] <= 0) return SA_ERR_INVALID_ARG;
-        m_max = std::max(m_max, m_list[i]);
+        *m_max = std::max(*m_max, m_list[i]);
     }
+    return SA_OK;
+}
+}  // namespace
+
+extern "C" int32_t sa_gemm_table_workspace_bytes(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads,
+                                                 int32_t head_dim, const int32_t *m_list, int32_t n_m, size_t *out_bytes) {
+    int32_t m_max = 0;
+    const int32_t st = gemm_table_check(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_list, n_m, &m_max);
+    if (st != SA_OK) return st;
+    if (!out_bytes) return SA_ERR_INVALID_ARG;
+    const size_t H = size_t(hidden), F = size_t(ffn), QD = size_t(num_q_heads) * head_dim;
+    const size_t NQKV = size_t(num_q_heads + 2 * num_kv_heads) * head_dim, M = size_t(m_max);
+    *out_bytes = gt_up(NQKV * H * 2) + gt_up(H * QD * 2) + 3 * gt_up(F * H * 2) + 2 * gt_up(H * 2) + 4 * gt_up(M * H * 2) +
+                 gt_up(M * NQKV * 2) + gt_up(M * F * 2) + gt_up(kGemmTableFlush) + gt_up(kGemmTableSplitK) + 256;
+    return SA_OK;
+}
+
+extern "C" int32_t sa_gemm_table(int32_t hidden, int32_t ffn, int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
+                                 const int32_t *m_list, int32_t n_m, int32_t warmup, int32_t iters, float *out_ms,
+                                 void *workspace, size_t workspace_bytes, void *stream_) {
+    using namespace sa;
+    int32_t m_max = 0;
+    {
+        const int32_t st = gemm_table_check(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_list, n_m, &m_max);
+        if (st != SA_OK) return st;
+    }
+    if (!out_ms || iters <= 0 || warmup < 0) return SA_ERR_INVALID_ARG;
+    size_t need = 0;
+    sa_gemm_table_workspace_bytes(hidden, ffn, num_q_heads, num_kv_heads, head_dim, m_list, n_m, &need);
+    if (!workspace || workspace_bytes < need) return SA_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const size_t H = size_t(hidden), F = size_t(ffn), QD = size_t(num_q_heads) * head_dim;
     const size_t NQKV = size_t(num_q_heads + 2 * num_kv_heads) * head_dim, M = size_t(m_max);
+    // weights and activations of the given shape are carved from the CALLER's workspace (values irrelevant to the timing)
     struct Buf {
-        std::vector<void *> p;
+        char *base = nullptr;
+        size_t used = 0;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         ~Buf() {
-            for (void *q : p) cudaFree(q);
             if (e0) cudaEventDestroy(e0);
             if (e1) cudaEventDestroy(e1);
         }
         void *alloc(size_t bytes) {
-            void *q = nullptr;
-            if (cudaMalloc(&q, std::max<size_t>(bytes, 256)) != cudaSuccess) return nullptr;
-            p.push_back(q);
+            void *q = base + used;
+            used += gt_up(bytes);
             return q;
         }
     } b;
-    const size_t flush_bytes = size_t(256) << 20;
+    b.base = reinterpret_cast<char *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
+    const size_t flush_bytes = kGemmTableFlush;
     void *w_qkv = b.alloc(NQKV * H * 2), *w_o = b.alloc(H * QD * 2), *w_g = b.alloc(F * H * 2), *w_u = b.alloc(F * H * 2);
     void *w_d = b.alloc(H * F * 2), *n1 = b.alloc(H * 2), *n2 = b.alloc(H * 2);
     void *x = b.alloc(M * H * 2), *h = b.alloc(M * H * 2), *qkv = b.alloc(M * NQKV * 2), *x1 = b.alloc(M * H * 2);
     void *act = b.alloc(M * F * 2), *y = b.alloc(M * H * 2), *flush = b.alloc(flush_bytes);
-    const size_t skb = size_t(160) * 128 * 1024;  // split-K scratch: tiles x slices never exceeds the SM count
+    const size_t skb = kGemmTableSplitK;
     void *sk = b.alloc(skb);
-    if (!sk) return SA_ERR_CUDA;
-    if (!w_qkv || !w_o || !w_g || !w_u || !w_d || !n1 || !n2 || !x || !h || !qkv || !x1 || !act || !y || !flush) return SA_ERR_CUDA;
     if (cudaEventCreate(&b.e0) != cudaSuccess || cudaEventCreate(&b.e1) != cudaSuccess) return SA_ERR_CUDA;
     struct { void *p; size_t n; float amp; } fills[] = {
         {w_qkv, NQKV * H, 0.05f}, {w_o, H * QD, 0.05f}, {w_g, F * H, 0.05f}, {w_u, F * H, 0.05f}, {w_d, H * F, 0.05f},

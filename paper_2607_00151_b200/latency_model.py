@@ -106,6 +106,87 @@ def fig15_design(pool: sa.Pool, model: sa.LatencyModel, token_model, cached=(102
     return rows
 
 
+def time_layer_batch(pool: sa.Pool, lw: "sa.LayerWeights", hidden: int, decode_L, chunks, iters=7, warmup=3, seed=0):
+    """Median CUDA-event time (ms) of ONE sa_layer_forward call (RMSNorm, fused QKV + RoPE + append, mixed attention, output
+    projection, SwiGLU FFN) on a batch of decode requests whose caches reach decode_L tokens and prefill chunks (q, prefix).
+    Every iteration first drops the tokens the previous one appended (host bookkeeping, outside the event pair)."""
+    cfg = pool.cfg
+    dev = torch.device("cuda:%d" % cfg.device)
+    g = torch.Generator(device=dev)
+    g.manual_seed(seed)
+    before = [int(L) - 1 for L in decode_L] + [int(p) for _, p in chunks]   # cached tokens before the call
+    qs = [1] * len(decode_L) + [int(q) for q, _ in chunks]
+    sids = [sa.sa_kv_session_open(pool) for _ in before]
+    src_n = 4096
+    k = ((torch.rand((src_n, cfg.num_kv_heads, cfg.head_dim), generator=g, device=dev) - 0.5) * 0.3).to(torch.bfloat16)
+    v = ((torch.rand((src_n, cfg.num_kv_heads, cfg.head_dim), generator=g, device=dev) - 0.5) * 0.3).to(torch.bfloat16)
+    try:
+        for sid, n in zip(sids, before):
+            done = 0
+            while done < n:
+                m = min(src_n, n - done)
+                sa.sa_rope_kv_append(pool, [sid], [0, m], k[:m], v[:m], None)
+                done += m
+        indptr = np.concatenate([[0], np.cumsum(qs)]).astype(np.int32)
+        T = int(indptr[-1])
+        x = torch.randn((T, hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+        y = torch.empty_like(x)
+        ws = torch.empty(sa.sa_layer_workspace_bytes(pool, lw, sids, indptr), dtype=torch.uint8, device=dev)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        st = torch.cuda.current_stream()
+        ts = []
+        for i in range(warmup + iters):
+            for sid, n in zip(sids, before):
+                sa.sa_kv_session_truncate(pool, sid, n)
+            flush.fill_(i & 1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            sa.sa_layer_forward(pool, lw, sids, indptr, x, y, ws)
+            e1.record(st)
+            torch.cuda.synchronize()
+            if i >= warmup:
+                ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+    finally:
+        for sid in sids:
+            sa.sa_kv_session_close(pool, sid)
+
+
+def fig15_layer_design(pool: sa.Pool, attn_model: sa.LatencyModel, hidden=4096, ffn=14336,
+                       cached=(1024, 4096, 16384, 32768), n_chunks=(2, 4), chunk_tokens=256, n_decode=4, seed=21):
+    """The FULL Eq. 1 that Algorithms 1 and 2 admit batches with (L349-353): c0 and the attention coefficients from the
+    latency-table fit plus T_GEMM(M) from sa_gemm_table (L299-303), against the measured time of sa_layer_forward on
+    Figure 15's batches (the whole layer, as in the paper: attention AND the dense operators).  What the sum can miss or
+    count twice -- launch gaps between the seven operators, the fixed cost c0 that both profiles contain -- shows up here
+    as relative error."""
+    cfg = pool.cfg
+    dev = torch.device("cuda:%d" % cfg.device)
+    g = torch.Generator(device=dev)
+    g.manual_seed(seed)
+    rnd = lambda *sh, sc=0.02: (torch.randn(*sh, device=dev, generator=g, dtype=torch.float32) * sc).to(torch.bfloat16)
+    nqkv = (cfg.num_q_heads + 2 * cfg.num_kv_heads) * cfg.head_dim
+    lw = sa.LayerWeights(rnd(hidden, sc=1.0), rnd(nqkv, hidden), rnd(hidden, cfg.num_q_heads * cfg.head_dim), rnd(hidden, sc=1.0),
+                         rnd(ffn, hidden), rnd(ffn, hidden), rnd(hidden, ffn), 1e-5)
+    m_list = sorted({1, 16, 64, 128, 256, 512, 1024, 2048} | {n_decode + nc * chunk_tokens for nc in n_chunks})
+    gemm_ms = sa.sa_gemm_table(hidden, ffn, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, m_list, warmup=3, iters=9)
+    full = sa.LatencyModel(attn_model.c0_ms, attn_model.alpha_d_ms, attn_model.alpha_p_ms, [(m, float(t)) for m, t in zip(m_list, gemm_ms)])
+    tok_only = []   # the token-budget view of the same batches: T_GEMM(M) + c0 alone (no KV terms)
+    rows = []
+    for nc in n_chunks:
+        for c in cached:
+            dec = [c] * n_decode
+            chunks = [(chunk_tokens, c)] * nc
+            meas = time_layer_batch(pool, lw, hidden, dec, chunks, seed=nc * 100003 + c)
+            est = sa.sa_est_batch_latency(full, dec, chunks)
+            tok = sa.sa_est_batch_latency(sa.LatencyModel(attn_model.c0_ms, 0.0, 0.0, full.gemm), dec, chunks)
+            rows.append({"prefill_chunks": nc, "cached_tokens": c, "M": n_decode + nc * chunk_tokens, "measured_ms": meas,
+                         "eq1_ms": est, "gemm_only_ms": tok, "eq1_rel_err": abs(est - meas) / meas,
+                         "gemm_only_rel_err": abs(tok - meas) / meas})
+            tok_only.append(tok)
+    return {"t_gemm_table": {"M": m_list, "ms": [float(t) for t in gemm_ms]}, "rows": rows,
+            "max_rel_err": {"eq1": max(r["eq1_rel_err"] for r in rows), "gemm_only": max(r["gemm_only_rel_err"] for r in rows)}}
+
+
 def run(device: int = 0, num_pages: int = 65536, verbose: bool = False):
     cfg = sa.PoolConfig(num_pages=num_pages, max_sessions=96, max_session_tokens=40960, device=device, **LLAMA8B)
     pool = sa.sa_kv_pool_create(cfg)
@@ -117,6 +198,7 @@ def run(device: int = 0, num_pages: int = 65536, verbose: bool = False):
         tb, *_ = np.linalg.lstsq(A, ms.astype(np.float64), rcond=None)
         tok_fit_err = float(np.max(np.abs(A @ tb - ms) / ms))
         rows = fig15_design(pool, model, tb)
+        layer = fig15_layer_design(pool, model)
     finally:
         sa.sa_kv_pool_destroy(pool)
     res = {
@@ -128,6 +210,7 @@ def run(device: int = 0, num_pages: int = 65536, verbose: bool = False):
         "prefill_tflops_implied": 4.0 * 128 * 32 / model.alpha_p_ms / 1e9 if model.alpha_p_ms > 0 else None,
         "fig15_design": rows,
         "fig15_max_rel_err": {"eq1": max(r["eq1_rel_err"] for r in rows), "token_only": max(r["token_only_rel_err"] for r in rows)},
+        "fig15_layer": layer,
         "paper_fig15_max_rel_err": {"eq1": 0.137, "token_only": 0.415, "cite": "PAPER.md L476 (H100, whole-model forward; context only)"},
     }
     if verbose:

@@ -182,3 +182,84 @@ def test_errors_change_nothing():
     sa.sa_kv_session_import(pool, sid, 0, img, 2, 0)
     assert sa.sa_kv_session_query(pool, sid)[0] == 40
     sa.sa_kv_pool_destroy(pool)
+
+
+@pytest.mark.parametrize("n_sessions", [5, 70])
+def test_many_sessions_in_one_call_equal_one_call_per_session(n_sessions):
+    """sa_kv_sessions_export / sa_kv_sessions_import (one launch for every session of a batch; 5 sessions ride in the kernel
+    parameters, 70 go through the metadata slab) against the per-session calls: images and imported pages bit for bit,
+    ragged lengths incl. an empty range, two ranges of one session, sentinel slots untouched, all-or-nothing page demand."""
+    L = Layer(32, 8, 128, 64, 500000.0)
+    rng = np.random.default_rng(100 + n_sessions)
+    lens = [int(x) for x in rng.integers(1, 400, size=n_sessions)]
+    lens[1] = 64      # ends on a page boundary
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(7)
+    pages = sum((n + 63) // 64 for n in lens) + 8
+    cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, pages, n_sessions + 2, 1024, L.rope_base, 0)
+
+    def mk(seed):
+        nbytes = sa.sa_kv_pool_storage_bytes(cfg)
+        storage = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        storage.view(torch.int16)[: nbytes // 2].fill_(np.array(SENT, dtype=np.uint16).view(np.int16).item())
+        return sa.sa_kv_pool_create(cfg, storage, np.random.default_rng(seed).permutation(pages).astype(np.int32))
+    src = mk(1)
+    sids = [sa.sa_kv_session_open(src) for _ in lens]
+    for sid, n in zip(sids, lens):
+        sa.sa_rope_kv_append(src, [sid], [0, n], _rand(n, 8, 128, gen, 0.1), _rand(n, 8, 128, gen, 0.1), None)
+    # ranges: every session whole, except session 0 in two pieces and session 2 as an empty range plus the whole
+    ranges = [(sids[0], 0, lens[0] // 2), (sids[0], lens[0] // 2, lens[0] - lens[0] // 2), (sids[2], 3 if lens[2] > 3 else 0, 0)]
+    ranges += [(sid, 0, n) for sid, n in zip(sids[1:], lens[1:])]
+    new_img = lambda n: torch.full((2, 8, n, 128), float("nan"), dtype=torch.bfloat16, device="cuda")
+    one = [new_img(n) for _, _, n in ranges]
+    for (sid, t0, n), im in zip(ranges, one):
+        sa.sa_kv_session_export(src, sid, t0, n, im)
+    many = [new_img(n) for _, _, n in ranges]
+    sa.sa_kv_sessions_export(src, [r[0] for r in ranges], [r[1] for r in ranges], [r[2] for r in ranges], many)
+    assert sa.sa_last_launch_count(src) == (1 if len(ranges) <= 64 else 2)
+    torch.cuda.synchronize()
+    for a, b in zip(one, many):
+        assert torch.equal(_bits(a), _bits(b))
+    # import: whole sessions (session 0 from its two pieces joined along tokens), one call vs one call per session
+    whole = [torch.cat([many[0], many[1]], dim=2).contiguous()] + many[3:]
+    assert [w_.shape[2] for w_ in whole] == lens
+    dst_a, dst_b = mk(2), mk(2)
+    sa_ids = [sa.sa_kv_session_open(dst_a) for _ in lens]
+    sb_ids = [sa.sa_kv_session_open(dst_b) for _ in lens]
+    for sid, n, im in zip(sa_ids, lens, whole):
+        sa.sa_kv_session_import(dst_a, sid, n, im, 8, 0)
+    # the joint call first fails for want of pages without touching anything ...
+    free0 = sa.sa_kv_pool_free_pages(dst_b)
+    hog = sa.sa_kv_session_open(dst_b)
+    sa.sa_rope_kv_append(dst_b, [hog], [0, 9 * 64], _rand(9 * 64, 8, 128, gen, 0.1), _rand(9 * 64, 8, 128, gen, 0.1), None)
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_kv_sessions_import(dst_b, sb_ids, lens, whole, 8, 0)
+    assert e.value.status == sa.SA_ERR_OUT_OF_PAGES and all(sa.sa_kv_session_query(dst_b, s)[0] == 0 for s in sb_ids)
+    hog_pages = set(int(x) for x in sa.sa_kv_session_query(dst_b, hog)[1])   # these lose their sentinel to the hog's own data
+    sa.sa_kv_session_close(dst_b, hog)
+    assert sa.sa_kv_pool_free_pages(dst_b) == free0
+    # ... and then does everything in one launch (plus the metadata uploads of a batch too large for the kernel parameters)
+    sa.sa_kv_sessions_import(dst_b, sb_ids, lens, whole, 8, 0)
+    assert sa.sa_last_launch_count(dst_b) <= (1 if n_sessions <= 64 else 4)
+    torch.cuda.synchronize()
+    for s_a, s_b, n in zip(sa_ids, sb_ids, lens):
+        la, pa = sa.sa_kv_session_query(dst_a, s_a)
+        lb, pb = sa.sa_kv_session_query(dst_b, s_b)
+        assert la == lb == n
+        ka, va = gather_kv(dst_a, list(pa), n)
+        kb, vb = gather_kv(dst_b, list(pb), n)
+        assert torch.equal(_bits(ka), _bits(kb)) and torch.equal(_bits(va), _bits(vb))
+    # sentinel: every slot no session owns is untouched in the jointly imported pool
+    kp, vp = pool_views(dst_b)
+    owned = {}
+    for s_b, n in zip(sb_ids, lens):
+        pg = sa.sa_kv_session_query(dst_b, s_b)[1]
+        for i, p_ in enumerate(pg):
+            owned[int(p_)] = min(64, n - 64 * i)
+    sent = np.array(SENT, dtype=np.uint16).view(np.int16).item()
+    for pg in range(pages):
+        lo = owned.get(pg, 0)
+        if lo < 64 and pg not in hog_pages:
+            assert (_bits(kp[pg, :, lo:, :]) == sent).all() and (_bits(vp[pg, :, lo:, :]) == sent).all()
+    for p_ in (src, dst_a, dst_b):
+        sa.sa_kv_pool_destroy(p_)

@@ -322,3 +322,16 @@ def test_two_appenders_of_one_shared_partial_page_need_one_copy():
     with pytest.raises(sa.SAError):
         sa.sa_rope_kv_append(p, [a, d], [0, 1, 2], None, None)  # holders 3 (b keeps it), appenders 2: two copies, one page
     assert sa.sa_kv_session_query(p, a)[0] == 8 and sa.sa_kv_session_query(p, d)[0] == 8 and sa.sa_kv_pool_free_pages(p) == 1
+
+
+def test_latency_table_workspace_is_sized_on_a_host_only_twin():
+    """sa_latency_table_workspace_bytes replays the run's sessions on a host-only twin of the pool: it needs no device, and
+    the figure grows with the decode batch (split partials) on top of the fixed buffers (sources, queries, L2 flush)."""
+    p = _pool(num_pages=4096, page_size=64, max_sessions=40, max_tokens=8192, Hq=32, Hkv=8, D=128)
+    a = sa.sa_latency_table_workspace_bytes(p, [0, 512], [1], 1024, 512, 2048, 3)
+    b = sa.sa_latency_table_workspace_bytes(p, [0, 512], [1, 32], 1024, 512, 2048, 3)
+    assert (256 << 20) < a < b < (300 << 20)
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_latency_table_workspace_bytes(p, [0], [64], 1024, 512, 2048, 3)   # more scratch sessions than the pool has
+    assert e.value.status == sa.SA_ERR_OUT_OF_SESSIONS
+    assert sa.sa_kv_pool_free_pages(p) == 4096
