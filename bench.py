@@ -377,7 +377,7 @@ def measure_parts(local: int, peaks, iters: int = 10):
     dec_bytes = float(kappa) * kv_tok + 2.0 * q.numel() * 2
     decode = {"bound": "hbm", "achieved": dec_bytes / (ms_dec * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
               "frac": dec_bytes / (ms_dec * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": load_traffic().get("flash_mma_decode_cfg4"),
-              "kernel": "flash_mma_kernel<128> (split-KV decode) + merge_splits_kernel on config 4's %d decode rows, "
+              "kernel": "flash_mma_kernel<128> (split-KV decode, the last split of a row merges) on config 4's %d decode rows, "
                         "%d cached tokens; 4 calls back to back per event pair (5.8 GB each: nothing is served from L2)" % (len(dec), kv_tok),
               "bytes_per_launch": dec_bytes, "ms": ms_dec, "ms_min": ms_dec_min, "peak_source": peaks["source"],
               "frac_of_nominal_7700": dec_bytes / (ms_dec * 1e-3) / 1e9 / 7700.0,
@@ -507,6 +507,85 @@ def measure_config(cfg_id: int, local: int, peaks, iters: int):
     r.close()
     sa.sa_kv_pool_destroy(pool)
     return res
+
+
+def measure_decode_step(local: int, peaks, batches=(1, 4, 16, 64), ctx: int = 21504, rounds: int = 10):
+    """The latency-critical decode iteration at small batch: sa_decode_step_prepare (host) + ONE captured
+    CUDA graph per step object of sa_decode_step_enqueue (append of the new token + split-KV attention with the merge
+    inside), replayed per iteration.  n_sets step objects on DISJOINT sets of sessions (a lone 21 K-token cache is 88 MB and
+    would otherwise be served from the 126 MB L2) are prepared on the host, then their graphs are replayed back to back inside
+    one event pair that is queued behind a short spin kernel: the figure is device time per iteration in a stream of
+    iterations (an event pair around a single trivial kernel reads ~5 us on this box, which is not the iteration's)."""
+    from paper_2607_00151_b200 import binding as sa
+    L = get_workload(4).layer
+    dev = torch.device("cuda:%d" % local)
+    kappa = 2 * L.num_kv_heads * L.head_dim * 2
+    out = {"ctx_tokens": ctx, "rows": {}}
+    for d in batches:
+        n_sets = max(2, min(8, int(np.ceil(400e6 / (d * ctx * kappa))) + 1))   # >= 400 MB of distinct K/V between two uses of a set
+        n_sess = d * n_sets
+        pages = n_sess * ((ctx + rounds * 4 + L.page_size) // L.page_size + 1) + 8
+        cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, pages, n_sess + 1, ctx + 1024, L.rope_base, local)
+        pool = sa.sa_kv_pool_create(cfg)
+        try:
+            g = torch.Generator(device=dev)
+            g.manual_seed(99 + d)
+            src = (torch.randn((ctx, L.num_kv_heads, L.head_dim), generator=g, device=dev) * L.head_dim ** -0.5).to(torch.bfloat16)
+            sids = [sa.sa_kv_session_open(pool) for _ in range(n_sess)]
+            for sid in sids:
+                sa.sa_rope_kv_append(pool, [sid], [0, ctx], src, src, None)
+            k = (torch.randn((d, L.num_kv_heads, L.head_dim), generator=g, device=dev) * L.head_dim ** -0.5).to(torch.bfloat16)
+            v = k.clone()
+            q = (torch.randn((d, L.num_q_heads, L.head_dim), generator=g, device=dev) * L.head_dim ** -0.5).to(torch.bfloat16)
+            o = torch.empty_like(q)
+            sets = [sids[i * d:(i + 1) * d] for i in range(n_sets)]
+            steps, graphs = [], []
+            for ss in sets:
+                stp = sa.sa_decode_step_create(pool, d, ctx + 1024)
+                sa.sa_decode_step_prepare(stp, ss)
+                sa.sa_decode_step_enqueue(stp, k, v, q, o, None)
+                torch.cuda.synchronize()
+                gr = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gr):
+                    sa.sa_decode_step_enqueue(stp, k, v, q, o, None)
+                steps.append(stp)
+                graphs.append(gr)
+            st = torch.cuda.current_stream()
+            ts, host_prep, host_launch = [], [], []
+            for it in range(rounds + 3):
+                t0 = time.perf_counter()
+                for stp, ss in zip(steps, sets):
+                    sa.sa_decode_step_prepare(stp, ss)
+                t1 = time.perf_counter()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda._sleep(200000)   # ~100 us of device time: the events and the graphs are all queued when it ends
+                e0.record(st)
+                t2 = time.perf_counter()
+                for gr in graphs:
+                    gr.replay()
+                t3 = time.perf_counter()
+                e1.record(st)
+                torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(e0.elapsed_time(e1) / n_sets)
+                    host_prep.append(1e6 * (t1 - t0) / n_sets)
+                    host_launch.append(1e6 * (t3 - t2) / n_sets)
+            ms = float(np.median(ts))
+            nbytes = float(kappa) * d * (ctx + rounds) + 2.0 * q.numel() * 2
+            out["rows"][str(d)] = {"ms": ms, "ms_min": float(min(ts)), "gbs": nbytes / (ms * 1e-3) / 1e9,
+                                   "frac": nbytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "bytes": nbytes,
+                                   "host_prepare_us": float(np.median(host_prep)), "host_graph_launch_us": float(np.median(host_launch)),
+                                   "steps_per_event_pair": n_sets}
+            del graphs
+            for stp in steps:
+                sa.sa_decode_step_destroy(stp)
+        finally:
+            sa.sa_kv_pool_destroy(pool)
+        torch.cuda.empty_cache()
+    out["note"] = ("device time per decode iteration: n graph replays (2 kernels each: append of the new token, split-KV attention "
+                   "with the merge inside) on disjoint session sets per event pair, queued behind a spin kernel; bytes = K/V of the "
+                   "rows' caches + q + out; host_* = wall time of sa_decode_step_prepare and of the graph launch per iteration")
+    return out
 
 
 def measure_latency_table(local: int, peaks):
@@ -795,13 +874,21 @@ def run_ours(args, world, rank, local):
         # the two HBM-bound kernels of the path (decode and append against the HBM peak), nested so that the
         # whole roofline story sits in one object; timed on config 4, where they move enough bytes for a bandwidth claim
         line["roofline"]["parts"] = {
-            "decode": short(dec_roof) | {"kernel": "flash_mma_kernel<128> + merge_splits_kernel, cfg4's 64 decode rows (read-only stream; "
+            "decode": short(dec_roof) | {"kernel": "flash_mma_kernel<128> (merge inside), cfg4's 64 decode rows (read-only stream; "
                                                    "%.3f of the 7.7 TB/s datasheet figure)" % dec_roof["frac_of_nominal_7700"]},
             "append": short(app_roof) | {"kernel": "rope_append_kernel, cfg4's 1.5 M-token prefix fill in one call"},
             "mixed_cfg4": {"ms": round(mixed["ms"], 4), "ms_decode_rows_done": round(mixed.get("ms_decode_done", 0.0), 4),
                            "bound_sum_ms": round(mixed["bound_sum_ms"], 4), "bound_max_ms": round(mixed["bound_max_ms"], 4)},
         }
         line["host_us_per_call"] = {k: round(v, 1) for k, v in host.items() if k.endswith("_us")}
+        try:
+            ds = measure_decode_step(local, peaks)
+            detail["decode_step_graph"] = ds
+            line["roofline"]["parts"]["decode_step_graph_21k"] = {
+                d: {"us": round(r_["ms"] * 1e3, 1), "frac": round(r_["frac"], 3), "host_us": round(r_["host_prepare_us"] + r_["host_graph_launch_us"], 1)}
+                for d, r_ in ds["rows"].items()}
+        except Exception as e:   # noqa: BLE001 - a side measurement never takes the line down
+            detail["decode_step_graph"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
         layer = measure_layer(local, peaks)
         detail["layer"] = layer
         torch.cuda.empty_cache()
@@ -857,6 +944,7 @@ def main():
     ap.add_argument("--other-configs-only", action="store_true", help="only the config 3 / config 5 measurements")
     ap.add_argument("--parts-only", action="store_true", help="only the decode / append measurements (for profiling them)")
     ap.add_argument("--layer-only", action="store_true", help="only the whole-layer measurement (for profiling the GEMMs)")
+    ap.add_argument("--decode-step-only", action="store_true", help="only the captured decode iteration at small batch")
     args = ap.parse_args()
     if args.layer_only:
         import __graft_entry__
@@ -872,6 +960,11 @@ def main():
         import __graft_entry__
         __graft_entry__.build()
         print(json.dumps({"other_configs": measure_other_configs(0, load_peaks())}))
+        return
+    if args.decode_step_only:
+        import __graft_entry__
+        __graft_entry__.build()
+        print(json.dumps({"decode_step_graph": measure_decode_step(0, load_peaks())}))
         return
     if args.parts_only:
         import __graft_entry__

@@ -24,7 +24,8 @@
  *     device memory and never synchronise the device.  All hot calls on one pool must be
  *     issued on one stream (or on streams the caller orders).  A pool is not thread-safe.
  *     They may wait on the host for a metadata slot of an earlier call and change host-side
- *     session state when called, so they must not be issued under CUDA stream capture.
+ *     session state when called, so they must not be issued under CUDA stream capture; the capturable form of a
+ *     decode iteration is sa_decode_step_prepare (host) + sa_decode_step_enqueue (device).
  *   - A call that fails with SA_ERR_INVALID_ARG, SA_ERR_OUT_OF_PAGES, SA_ERR_OUT_OF_SESSIONS, SA_ERR_UNSUPPORTED or
  *     SA_ERR_WORKSPACE_TOO_SMALL leaves the pool, its block tables and session lengths unchanged: everything is
  *     validated and sized before any state is touched.  SA_ERR_CUDA means the CUDA runtime refused a launch, copy or
@@ -203,6 +204,44 @@ SA_API int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req, co
 SA_API int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                     const int32_t *qo_indptr, int32_t *out_parts, int32_t cap,
                                     int64_t *out_summary);
+
+/* ---- sa_decode_step_*: one decode iteration, capturable in a CUDA graph (steps a1-a2, a5-a6) -----------------------
+ * The latency-critical class of the runtime is the decode iteration (its time is the TBT that
+ * Algorithm 2 protects, L392-398): every request appends ONE token and its query row attends to the whole cache, own
+ * token included.  sa_rope_kv_append + sa_mixed_attention compute that, but plan on the host inside the call, so
+ * they cannot be recorded once and replayed.  A decode step separates the two halves:
+ *   sa_decode_step_prepare   HOST ONLY (no device work, nothing enqueued).  For each request: the host half of
+ *       appending one token to sids[r] (a page is taken when the session's last page is full; the session grows by
+ *       one) and the attention plan of its row.  Everything the kernels need is written to a pinned slab the step
+ *       owns.  Must not be called while an earlier enqueue / graph replay of this step can still be running (the
+ *       kernels read the slab when they execute).  Errors leave the pool and the step unchanged: SA_ERR_INVALID_ARG
+ *       (n_req > max_requests, unknown / closed / repeated session, cache would exceed max_kv_tokens),
+ *       SA_ERR_OUT_OF_PAGES, SA_ERR_UNSUPPORTED (a session whose partly filled last page is shared with a fork: the
+ *       copy-on-write needs sa_rope_kv_append).
+ *   sa_decode_step_enqueue   DEVICE ONLY.  Enqueues two launches with fixed grids on `stream` and changes no host
+ *       state: (1) slab -> device twin, RoPE + placement of the new tokens (K rotated at the token's position, V bit
+ *       copy, q_inout rotated in place, block-table entry written), (2) split-KV attention of the rows, the actual
+ *       counts read on the device, the last split of a row merging them.  Legal under CUDA stream capture; the captured graph is
+ *       replayed after each prepare (same k / v / q_inout / out / lse addresses, new contents).  Calling it again
+ *       without a new prepare re-places the same tokens and recomputes the same rows (idempotent).
+ * Results are bit-equal to sa_rope_kv_append + sa_mixed_attention on the same batch (same device code per row).
+ *   max_requests   : capacity of a step (<= cfg.max_sessions); max_kv_tokens: longest cache a row may attend to
+ *   dev_mem        : device, 256-byte aligned, >= sa_decode_step_device_bytes(...): metadata twin + split partials;
+ *                    the caller's, and must outlive the step (NULL for a host-only pool)
+ *   k, v           : device bf16 [n_req, Hkv, D], pre-RoPE; q_inout: device bf16 [n_req, Hq, D]
+ *   out            : device bf16 [n_req, Hq, D]; lse: device f32 [n_req, Hq], nullable
+ *   sa_decode_step_stats: host int64[6] = {requests, work items, CTAs of the attention grid, launches of the last
+ *                    enqueue, partial rows the workspace holds, capacity} */
+typedef struct sa_decode_step sa_decode_step; /* opaque */
+SA_API int32_t sa_decode_step_device_bytes(const sa_kv_pool *pool, int32_t max_requests, int64_t max_kv_tokens,
+                                           size_t *out_bytes);
+SA_API int32_t sa_decode_step_create(sa_kv_pool *pool, int32_t max_requests, int64_t max_kv_tokens, void *dev_mem,
+                                     size_t dev_bytes, sa_decode_step **out_step);
+SA_API int32_t sa_decode_step_destroy(sa_decode_step *step);
+SA_API int32_t sa_decode_step_prepare(sa_decode_step *step, int32_t n_req, const int32_t *sids);
+SA_API int32_t sa_decode_step_enqueue(sa_decode_step *step, const void *k, const void *v, void *q_inout, void *out,
+                                      float *lse, float sm_scale, void *stream);
+SA_API int32_t sa_decode_step_stats(const sa_decode_step *step, int64_t *out_stats);
 
 /* Number of kernel launches the last successful sa_mixed_attention / sa_rope_kv_append on this
  * pool enqueued (for launch accounting in benchmarks). */

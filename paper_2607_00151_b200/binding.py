@@ -151,6 +151,12 @@ PROTOTYPES = {
                                                ctypes.POINTER(ctypes.c_size_t), _vp]),
     "sa_kv_sessions_import": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p, _i64p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int32,
                                                ctypes.c_int32, _vp]),
+    "sa_decode_step_device_bytes": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, ctypes.POINTER(ctypes.c_size_t)]),
+    "sa_decode_step_create": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, _vp, ctypes.c_size_t, ctypes.POINTER(_vp)]),
+    "sa_decode_step_destroy": (ctypes.c_int32, [_vp]),
+    "sa_decode_step_prepare": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p]),
+    "sa_decode_step_enqueue": (ctypes.c_int32, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp]),
+    "sa_decode_step_stats": (ctypes.c_int32, [_vp, _i64p]),
 }
 
 _lib = None
@@ -565,6 +571,70 @@ def sa_kv_sessions_import(pool: Pool, sids, n_tokens, images, src_heads: int, he
     ptrs = (ctypes.c_void_p * max(n, 1))(*[_ptr(im) for im in images])
     sp = None if pool.storage is None else _stream_ptr(stream, pool)
     _check(load_library().sa_kv_sessions_import(pool.handle, n, s_ptr, n_ptr, ptrs, src_heads, head_begin, sp), "sa_kv_sessions_import")
+
+# ---------------------------------------------------------------- capturable decode step
+class DecodeStep:
+    """Handle of an sa_decode_step plus the torch tensor that owns its device memory."""
+
+    def __init__(self, handle: int, pool: Pool, mem, max_requests: int, max_kv_tokens: int):
+        self.handle = handle
+        self.pool = pool
+        self.mem = mem
+        self.max_requests = max_requests
+        self.max_kv_tokens = max_kv_tokens
+
+    def __del__(self):
+        try:
+            if self.handle:
+                sa_decode_step_destroy(self)
+        except Exception:
+            pass
+
+
+def sa_decode_step_device_bytes(pool: Pool, max_requests: int, max_kv_tokens: int) -> int:
+    out = ctypes.c_size_t(0)
+    _check(load_library().sa_decode_step_device_bytes(pool.handle, max_requests, max_kv_tokens, ctypes.byref(out)),
+           "sa_decode_step_device_bytes")
+    return int(out.value)
+
+
+def sa_decode_step_create(pool: Pool, max_requests: int, max_kv_tokens: int, mem=None) -> DecodeStep:
+    """mem: a uint8 CUDA tensor of >= sa_decode_step_device_bytes(...) bytes (allocated here if None; None stays None
+    for a host-only pool)."""
+    nbytes = sa_decode_step_device_bytes(pool, max_requests, max_kv_tokens)
+    if pool.storage is not None and mem is None:
+        import torch
+        mem = torch.empty(nbytes, dtype=torch.uint8, device="cuda:%d" % pool.cfg.device)
+    out = _vp()
+    _check(load_library().sa_decode_step_create(pool.handle, max_requests, max_kv_tokens, _ptr(mem), _nbytes(mem), ctypes.byref(out)),
+           "sa_decode_step_create")
+    return DecodeStep(out.value, pool, mem, max_requests, max_kv_tokens)
+
+
+def sa_decode_step_destroy(step: DecodeStep) -> None:
+    h, step.handle = step.handle, None
+    if h:
+        _check(load_library().sa_decode_step_destroy(h), "sa_decode_step_destroy")
+
+
+def sa_decode_step_prepare(step: DecodeStep, sids) -> None:
+    """Host half of one decode iteration: every session grows by one token, the step's metadata is rewritten."""
+    keep, ptr = _i32(sids)
+    _check(load_library().sa_decode_step_prepare(step.handle, keep.shape[0], ptr), "sa_decode_step_prepare")
+
+
+def sa_decode_step_enqueue(step: DecodeStep, k, v, q_inout, out, lse=None, sm_scale: float = 0.0, stream=None) -> None:
+    """Device half (two launches, capturable): RoPE + placement of the new tokens, split-KV attention of the rows."""
+    _check(load_library().sa_decode_step_enqueue(step.handle, _ptr(k), _ptr(v), _ptr(q_inout), _ptr(out), _ptr(lse),
+                                                 float(sm_scale), _stream_ptr(stream, step.pool)), "sa_decode_step_enqueue")
+
+
+def sa_decode_step_stats(step: DecodeStep) -> dict:
+    out = np.zeros(6, dtype=np.int64)
+    _check(load_library().sa_decode_step_stats(step.handle, out.ctypes.data_as(_i64p)), "sa_decode_step_stats")
+    return {"requests": int(out[0]), "items": int(out[1]), "grid_ctas": int(out[2]), "launches": int(out[3]),
+            "max_part_rows": int(out[4]), "capacity": int(out[5])}
+
 
 # ---------------------------------------------------------------- dense operators of the layer (N3)
 def _nbytes(t) -> int:

@@ -41,53 +41,17 @@ __global__ void block_table_update_kernel(const ReqMeta *__restrict__ reqs, cons
     for (int i = threadIdx.x; i < r.n_splits; i += blockDim.x) row[i] = new_pages[r.item_begin + i];
 }
 
-// Per token: (2*Hkv + Hq) heads, each D/16 "units" of two 16-byte vectors (dims [8j, 8j+8) and
-// [D/2+8j, D/2+8j+8)): K and Q units are rotated, V units are copied bit for bit.
-// INLINE: the call's metadata (requests, new page ids) rides in the kernel parameters instead of the slab: no upload
-// launch, no block-table launch -- the thread that places a token in a page this call allocated also writes that
-// page's block-table entry (every new page receives at least one new token; equal values from several threads).
-template <int D, bool INLINE>
-__global__ void __launch_bounds__(kAppendThreads)
-rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *__restrict__ reqs_slab, int32_t n_req_slab, int64_t total_rows,
-                   const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
-                   __nv_bfloat16 *__restrict__ q, __nv_bfloat16 *__restrict__ k_base,
-                   __nv_bfloat16 *__restrict__ v_base, int32_t *block_table, int64_t mpps,
-                   int32_t log2_page, int64_t stride_page, int64_t stride_head,
-                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
-    const ReqMeta *reqs = INLINE ? im.reqs : reqs_slab;
-    const int32_t n_req = INLINE ? im.n_req : n_req_slab;
+// RoPE tables of the CTA's tokens, then the copy itself.  s_pos / s_dst: position and destination (element offset of
+// the token's slot inside a (page, head 0) block) of each of the CTA's n_tok tokens, filled by the caller.
+template <int D>
+__device__ __forceinline__ void append_rows(int64_t t0, int n_tok, const int32_t *s_pos, const int64_t *s_dst,
+                                            float2 (*s_cs)[D / 2], const __nv_bfloat16 *__restrict__ k,
+                                            const __nv_bfloat16 *__restrict__ v, __nv_bfloat16 *__restrict__ q,
+                                            __nv_bfloat16 *__restrict__ k_base, __nv_bfloat16 *__restrict__ v_base,
+                                            int64_t stride_head, const float2 *__restrict__ rope_tab, int32_t Hq,
+                                            int32_t Hkv, int tid) {
     constexpr int HALF = D / 2;
     constexpr int UPH = D / 16;  // units per head
-    __shared__ int64_t s_dst[kAppendTok];
-    __shared__ float2 s_cs[kAppendTok][HALF];
-    __shared__ int32_t s_pos[kAppendTok];
-
-    const int64_t t0 = int64_t(blockIdx.x) * kAppendTok;
-    const int n_tok = int(min(int64_t(kAppendTok), total_rows - t0));
-    const int tid = threadIdx.x;
-
-    if (tid < n_tok) {
-        const int64_t t = t0 + tid;
-        int lo = 0, hi = n_req - 1;  // last request with q_start <= t (empty requests never match last)
-        while (lo < hi) {
-            int mid = (lo + hi + 1) >> 1;
-            if (reqs[mid].q_start <= t) lo = mid; else hi = mid - 1;
-        }
-        const ReqMeta r = reqs[lo];
-        const int32_t pos = r.kv_len + int32_t(t - r.q_start);
-        const int32_t pi = pos >> log2_page;
-        int32_t page;
-        if (INLINE && pi >= r.part_begin && pi - r.part_begin < r.n_splits) {
-            page = im.pages[r.item_begin + pi - r.part_begin];       // allocated (or copied on write) by this call
-            block_table[int64_t(r.sid) * mpps + pi] = page;
-        } else {
-            page = block_table[int64_t(r.sid) * mpps + pi];
-        }
-        const int32_t slot = pos & ((1 << log2_page) - 1);
-        s_pos[tid] = pos;
-        s_dst[tid] = int64_t(page) * stride_page + int64_t(slot) * D;
-    }
-    __syncthreads();
     for (int e = tid; e < n_tok * HALF; e += kAppendThreads) {
         const int tl = e / HALF, m = e % HALF;
         s_cs[tl][m] = rope_cos_sin(s_pos[tl], rope_tab[m]);
@@ -153,6 +117,106 @@ rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *_
     }
 }
 
+// Per token: (2*Hkv + Hq) heads, each D/16 "units" of two 16-byte vectors (dims [8j, 8j+8) and
+// [D/2+8j, D/2+8j+8)): K and Q units are rotated, V units are copied bit for bit.
+// INLINE: the call's metadata (requests, new page ids) rides in the kernel parameters instead of the slab: no upload
+// launch, no block-table launch -- the thread that places a token in a page this call allocated also writes that
+// page's block-table entry (every new page receives at least one new token; equal values from several threads).
+template <int D, bool INLINE>
+__global__ void __launch_bounds__(kAppendThreads)
+rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *__restrict__ reqs_slab, int32_t n_req_slab, int64_t total_rows,
+                   const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
+                   __nv_bfloat16 *__restrict__ q, __nv_bfloat16 *__restrict__ k_base,
+                   __nv_bfloat16 *__restrict__ v_base, int32_t *block_table, int64_t mpps,
+                   int32_t log2_page, int64_t stride_page, int64_t stride_head,
+                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
+    const ReqMeta *reqs = INLINE ? im.reqs : reqs_slab;
+    const int32_t n_req = INLINE ? im.n_req : n_req_slab;
+    constexpr int HALF = D / 2;
+    constexpr int UPH = D / 16;  // units per head
+    __shared__ int64_t s_dst[kAppendTok];
+    __shared__ float2 s_cs[kAppendTok][HALF];
+    __shared__ int32_t s_pos[kAppendTok];
+
+    const int64_t t0 = int64_t(blockIdx.x) * kAppendTok;
+    const int n_tok = int(min(int64_t(kAppendTok), total_rows - t0));
+    const int tid = threadIdx.x;
+
+    if (tid < n_tok) {
+        const int64_t t = t0 + tid;
+        int lo = 0, hi = n_req - 1;  // last request with q_start <= t (empty requests never match last)
+        while (lo < hi) {
+            int mid = (lo + hi + 1) >> 1;
+            if (reqs[mid].q_start <= t) lo = mid; else hi = mid - 1;
+        }
+        const ReqMeta r = reqs[lo];
+        const int32_t pos = r.kv_len + int32_t(t - r.q_start);
+        const int32_t pi = pos >> log2_page;
+        int32_t page;
+        if (INLINE && pi >= r.part_begin && pi - r.part_begin < r.n_splits) {
+            page = im.pages[r.item_begin + pi - r.part_begin];       // allocated (or copied on write) by this call
+            block_table[int64_t(r.sid) * mpps + pi] = page;
+        } else {
+            page = block_table[int64_t(r.sid) * mpps + pi];
+        }
+        const int32_t slot = pos & ((1 << log2_page) - 1);
+        s_pos[tid] = pos;
+        s_dst[tid] = int64_t(page) * stride_page + int64_t(slot) * D;
+    }
+    __syncthreads();
+    append_rows<D>(t0, n_tok, s_pos, s_dst, s_cs, k, v, q, k_base, v_base, stride_head, rope_tab, Hq, Hkv, tid);
+}
+
+// The new token of every request of a captured decode step (sa_decode_step_enqueue).  The step's metadata sits in a
+// pinned host slab that sa_decode_step_prepare rewrites between replays: this kernel copies it to its device twin
+// (the attention kernels behind it read that) and places the tokens from the host copy directly -- position and page
+// of every token are decided on the host, so the block table is only written here, never read.  Same arithmetic as
+// rope_append_kernel (append_rows), so the stored bits are those of sa_rope_kv_append.
+template <int D>
+__global__ void __launch_bounds__(kAppendThreads)
+step_append_kernel(const uint32_t *__restrict__ slab_host, uint32_t *__restrict__ slab_dev, int32_t words, int32_t cap,
+                   const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v, __nv_bfloat16 *__restrict__ q,
+                   __nv_bfloat16 *__restrict__ k_base, __nv_bfloat16 *__restrict__ v_base, int32_t *block_table,
+                   int64_t mpps, int32_t log2_page, int64_t stride_page, int64_t stride_head,
+                   const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
+    __shared__ int64_t s_dst[kAppendTok];
+    __shared__ float2 s_cs[kAppendTok][D / 2];
+    __shared__ int32_t s_pos[kAppendTok];
+    const int tid = threadIdx.x;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the attention grid may be staged behind this one
+    // the CTA's own records and the request count come straight from the pinned slab, all reads issued together (one
+    // PCIe round trip); the copy to the device twin rides along
+    const StepHeader *hd = reinterpret_cast<const StepHeader *>(slab_host);
+    const StepAppend *ap = reinterpret_cast<const StepAppend *>(reinterpret_cast<const char *>(slab_host) + step_append_offset(cap));
+    const int64_t t0 = int64_t(blockIdx.x) * kAppendTok;
+    StepAppend x = {0, 0, 0, 0};
+    if (tid < kAppendTok && t0 + tid < cap) x = ap[t0 + tid];
+    {   // while the slab crosses PCIe: pull the rows this CTA may place (and the RoPE table) into L2
+        const int64_t n_max = min(int64_t(kAppendTok), int64_t(cap) - t0);
+        const char *kp = reinterpret_cast<const char *>(k + t0 * Hkv * D), *vp = reinterpret_cast<const char *>(v + t0 * Hkv * D);
+        const char *qp = reinterpret_cast<const char *>(q + t0 * Hq * D);
+        const int64_t kv_bytes = n_max * Hkv * D * 2, q_bytes = n_max * Hq * D * 2;
+        for (int64_t o = int64_t(tid) * 128; o < kv_bytes; o += int64_t(kAppendThreads) * 128) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(kp + o));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(vp + o));
+        }
+        for (int64_t o = int64_t(tid) * 128; o < q_bytes; o += int64_t(kAppendThreads) * 128)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(qp + o));
+        if (tid * 128 < int(D / 2 * sizeof(float2)))
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(rope_tab) + tid * 128));
+    }
+    const int n_req = hd->n_req;
+    for (int i = blockIdx.x * kAppendThreads + tid; i < words; i += gridDim.x * kAppendThreads) slab_dev[i] = slab_host[i];
+    const int n_tok = int(max(int64_t(0), min(int64_t(kAppendTok), int64_t(n_req) - t0)));
+    if (tid < n_tok) {
+        block_table[int64_t(x.sid) * mpps + (x.pos >> log2_page)] = x.page;
+        s_pos[tid] = x.pos;
+        s_dst[tid] = int64_t(x.page) * stride_page + int64_t(x.pos & ((1 << log2_page) - 1)) * D;
+    }
+    __syncthreads();
+    if (n_tok > 0) append_rows<D>(t0, n_tok, s_pos, s_dst, s_cs, k, v, q, k_base, v_base, stride_head, rope_tab, Hq, Hkv, tid);
+}
+
 template <bool INLINE>
 static cudaError_t launch_rope_append_t(const sa_kv_pool *pool, const InlineAppendMeta &im, const ReqMeta *reqs_dev,
                                         int32_t n_req, int64_t total_rows, const void *k, const void *v, void *q,
@@ -173,6 +237,28 @@ static cudaError_t launch_rope_append_t(const sa_kv_pool *pool, const InlineAppe
             static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
             pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
             pool->cfg.num_kv_heads);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step_append(const sa_kv_pool *pool, const void *slab_host, void *slab_dev, int32_t cap, const void *k,
+                               const void *v, void *q, cudaStream_t stream, int32_t *launches) {
+    const unsigned grid = unsigned((cap + kAppendTok - 1) / kAppendTok);
+    const int32_t words = int32_t(step_slab_bytes(cap) / 4);
+    auto kb = static_cast<__nv_bfloat16 *>(pool->k_base);
+    auto vb = static_cast<__nv_bfloat16 *>(pool->v_base);
+    if (pool->cfg.head_dim == 128)
+        step_append_kernel<128><<<grid, kAppendThreads, 0, stream>>>(
+            static_cast<const uint32_t *>(slab_host), static_cast<uint32_t *>(slab_dev), words, cap,
+            static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v), static_cast<__nv_bfloat16 *>(q), kb, vb,
+            pool->block_table, pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head,
+            pool->rope_tab, pool->cfg.num_q_heads, pool->cfg.num_kv_heads);
+    else
+        step_append_kernel<64><<<grid, kAppendThreads, 0, stream>>>(
+            static_cast<const uint32_t *>(slab_host), static_cast<uint32_t *>(slab_dev), words, cap,
+            static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v), static_cast<__nv_bfloat16 *>(q), kb, vb,
+            pool->block_table, pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head,
+            pool->rope_tab, pool->cfg.num_q_heads, pool->cfg.num_kv_heads);
     ++*launches;
     return cudaGetLastError();
 }

@@ -1,8 +1,9 @@
 // sa_flash_mma.cu -- decode attention over paged KV on the warp-level tensor path (mma.sync m16n8k16):
 // decode-like rows (q_len * G <= 16), split-KV, HBM-bound.  One CTA per (request, kv head, 1024-key
-// split); the G query heads of the group are the M rows of the MMA so K/V are read once per group;
+// split); the G query heads of the group are the N columns of the MMA (keys are its M rows: S^T = K Q^T,
+// O^T += V^T P^T) so K/V are read once per group and no tensor work is spent on padding rows;
 // 4 warps take 16 keys each of every 64-key tile; cp.async 3-stage ring of page-gathered tiles;
-// deterministic merge of the splits ("a single query token that attends to its full
+// deterministic merge of the splits by the last of them to finish ("a single query token that attends to its full
 // KV cache of length L_j ... memory-bandwidth bound").  Prefill chunks run on the tcgen05 kernel
 // (sa_prefill_tc5.cu) for every supported head_dim.
 // Packed rows: row rho of a (request, kv head g) pair is (token rho / G, q head g*G + rho % G).
@@ -19,6 +20,7 @@ namespace {
 constexpr int kThreads = 128;
 constexpr int kBN = 64;      // keys per tile
 constexpr int kStages = 3;   // cp.async ring depth (64 KiB of K/V in flight per CTA)
+constexpr int kMaxSplitPages = kDecodeSplitKeys / 16;  // pages a split can span at the smallest page size
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -55,9 +57,17 @@ __device__ __forceinline__ uint32_t tile_off(int row, int chunk) {
     return uint32_t(row * (D * 2) + ((chunk ^ (row & 7)) << 4));
 }
 
+constexpr int kLoopReqCache = 128;  // requests a captured step keeps in shared memory (4 KiB)
+// shared memory of one 128-thread group: the K/V ring, the Q tile, the page ids of the split
+template <int D>
+constexpr size_t group_smem() {
+    return size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2 + kMaxSplitPages * 4 + 16;
+}
+
 struct KvView {
     const __nv_bfloat16 *k_base, *v_base;
-    const int32_t *bt_row;  // block table row of the session
+    const int32_t *pages;   // shared memory: the page ids of the item's split, pages[0] = page of key k_begin
+    int32_t page0;          // k_begin >> log2_page
     int64_t stride_page;
     int64_t head_off;  // g * stride_head
     int32_t log2_page;
@@ -65,9 +75,10 @@ struct KvView {
 
 // Gather one 64-key tile of K and V (logical keys kt .. kt+63, kt a multiple of 64 and < kv_len) into
 // swizzled smem; rows at or beyond kv_len are zero-filled (src-size 0: nothing is read), so slots the
-// session does not own never reach the math.  The block-table reads come first and are branch-free:
-// with pages of >= 64 slots a tile lies in one page (one read per thread); smaller pages read one entry
-// per row, all independent, so their latencies overlap instead of adding up row by row.
+// session does not own never reach the math.  The page ids come from shared memory (decode_item reads the split's
+// slice of the block table once, before the ring starts): a block-table read from global memory in front of every
+// tile's copies stalled the issuing warp for an L2 or DRAM round trip per tile, in program order before the tile's
+// arithmetic -- with one warp per scheduler nothing hid it, and a lone CTA took 0.64 us per tile.
 template <int D>
 __device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_len, uint32_t sK, uint32_t sV, int tid) {
     constexpr int CPR = D / 8;               // 16-byte chunks per row
@@ -77,7 +88,7 @@ __device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_le
     const int r0 = tid / CPR;
     const int last = kv_len - 1;
     if (kv.log2_page >= 6) {
-        const int32_t page = __ldg(kv.bt_row + (kt >> kv.log2_page));
+        const int32_t page = kv.pages[(kt >> kv.log2_page) - kv.page0];
         const int slot0 = (kt & ((1 << kv.log2_page) - 1)) + r0;
         const int64_t base = int64_t(page) * kv.stride_page + kv.head_off + int64_t(slot0) * D + chunk * 8;
         const __nv_bfloat16 *kp = kv.k_base + base, *vp = kv.v_base + base;
@@ -94,7 +105,7 @@ __device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_le
     const int pmask = (1 << kv.log2_page) - 1;
     int32_t page[NP];
 #pragma unroll
-    for (int i = 0; i < NP; ++i) page[i] = __ldg(kv.bt_row + (min(kt + r0 + i * RPP, last) >> kv.log2_page));
+    for (int i = 0; i < NP; ++i) page[i] = kv.pages[(min(kt + r0 + i * RPP, last) >> kv.log2_page) - kv.page0];
 #pragma unroll
     for (int i = 0; i < NP; ++i) {
         const int row = r0 + i * RPP;
@@ -107,82 +118,191 @@ __device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_le
     }
 }
 
-// One online-softmax step of a warp over NKG groups of 16 keys starting at tile row key_off.
-template <int D, int NKG>
-__device__ __forceinline__ void warp_step(const uint32_t (&qf)[D / 16][4], uint32_t sK, uint32_t sV, int key_off,
-                                          int kt_abs, int lim0, int lim1, bool need_mask, float scale_log2,
-                                          float (&o)[D / 8][4], float &m0, float &m1, float &l0, float &l1, int lane) {
-    float s[NKG * 2][4];
+// barrier over one 128-thread group of the CTA (id 0 with 128 threads is __syncthreads of a 128-thread CTA)
+__device__ __forceinline__ void group_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+
+__device__ __forceinline__ uint32_t movmatrix_t(uint32_t x) {  // transpose of an 8x8 b16 matrix held one row pair per lane
+    uint32_t y;
+    asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;\n" : "=r"(y) : "r"(x));
+    return y;
+}
+
+// Running state of a warp for its NT * 8 query rows.  Everything is held TRANSPOSED: the 16 keys of a step are the M
+// rows of the MMA and the query rows its N columns, S^T = K Q^T and O^T += V^T P^T.  A decode batch has G (<= 8) live
+// rows per kv head, so one n8 column tile carries them and a step costs D/16 + D/16 HMMAs instead of twice that with
+// the rows as M (16 rows, most of them padding) -- on sm_100a the warp-level HMMA pipe retires one m16n8k16 per ~30
+// cycles per scheduler, which, not HBM, bounded a lone warp (d = 1) and co-limited the full-batch stream at G = 4.
+// A thread holds query rows qa = nt*8 + 2*(lane%4) and qa + 1 (C-fragment columns); keys / dims run over lane/4.
+template <int D, int NT>
+struct WarpState {
+    float o[D / 16][NT][4];  // O^T: [0],[1] dim = np*16 + lane/4, rows qa, qa+1; [2],[3] dim + 8
+    float m[NT][2], l[NT][2];
+};
+
+// One online-softmax step of a warp over 16 keys starting at tile row key_off (absolute position kt_abs + key_off).
+template <int D, int NT>
+__device__ __forceinline__ void warp_step(const uint32_t (&qf)[D / 16][4], uint32_t sK, uint32_t sV, int key_off, int kt_abs,
+                                          const int (&lim)[NT][2], bool need_mask, float scale_log2, WarpState<D, NT> &w,
+                                          int lane) {
+    float s[NT][4];
 #pragma unroll
-    for (int i = 0; i < NKG * 2; ++i) s[i][0] = s[i][1] = s[i][2] = s[i][3] = 0.f;
+    for (int nt = 0; nt < NT; ++nt) s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f;
     const int mi = lane >> 3, rr = lane & 7;
 #pragma unroll
     for (int ks = 0; ks < D / 16; ++ks) {
+        uint32_t ka[4];  // A = K: keys x dims, row-major as stored
+        ldsm_x4(ka, sK + tile_off<D>(key_off + (mi & 1) * 8 + rr, ks * 2 + (mi >> 1)));
 #pragma unroll
-        for (int kg = 0; kg < NKG; ++kg) {
-            const int krow = key_off + kg * 16 + (mi >> 1) * 8 + rr;
-            uint32_t b[4];
-            ldsm_x4(b, sK + tile_off<D>(krow, ks * 2 + (mi & 1)));
-            mma16816(s[kg * 2], qf[ks], b[0], b[1]);
-            mma16816(s[kg * 2 + 1], qf[ks], b[2], b[3]);
-        }
+        for (int nt = 0; nt < NT; ++nt) mma16816(s[nt], ka, qf[ks][2 * nt], qf[ks][2 * nt + 1]);
     }
-    float mx0 = -INFINITY, mx1 = -INFINITY;
+    const int key_lo = kt_abs + key_off + (lane >> 2);  // this thread's keys: key_lo ([0],[1]) and key_lo + 8 ([2],[3])
+    float c[NT][2], b[NT][2];
+    bool moved = false;
 #pragma unroll
-    for (int nt = 0; nt < NKG * 2; ++nt) {
+    for (int nt = 0; nt < NT; ++nt) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             float v = s[nt][e] * scale_log2;
-            if (need_mask) {
-                const int pos = kt_abs + key_off + nt * 8 + 2 * (lane & 3) + (e & 1);
-                if (pos > (e < 2 ? lim0 : lim1)) v = -INFINITY;
-            }
+            if (need_mask && key_lo + (e >> 1) * 8 > lim[nt][e & 1]) v = -INFINITY;
             s[nt][e] = v;
-            if (e < 2) mx0 = fmaxf(mx0, v); else mx1 = fmaxf(mx1, v);
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            float mx = fmaxf(s[nt][j], s[nt][2 + j]);
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
+            const float mn = fmaxf(w.m[nt][j], mx);
+            b[nt][j] = (mn == -INFINITY) ? 0.f : mn;
+            c[nt][j] = exp2f(w.m[nt][j] - b[nt][j]);
+            moved = moved || c[nt][j] != 1.f;
+            w.m[nt][j] = mn;
         }
     }
-    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
-    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
-    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
-    const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
-    const float b0 = (mn0 == -INFINITY) ? 0.f : mn0, b1 = (mn1 == -INFINITY) ? 0.f : mn1;
-    const float c0 = exp2f(m0 - b0), c1 = exp2f(m1 - b1);
-    m0 = mn0;
-    m1 = mn1;
-    float rs0 = 0.f, rs1 = 0.f;
+    uint32_t pb[NT][2];  // B = P^T: keys x rows
 #pragma unroll
-    for (int nt = 0; nt < NKG * 2; ++nt) {
-        s[nt][0] = exp2f(s[nt][0] - b0);
-        s[nt][1] = exp2f(s[nt][1] - b0);
-        s[nt][2] = exp2f(s[nt][2] - b1);
-        s[nt][3] = exp2f(s[nt][3] - b1);
-        rs0 += s[nt][0] + s[nt][1];
-        rs1 += s[nt][2] + s[nt][3];
+    for (int nt = 0; nt < NT; ++nt) {
+        s[nt][0] = exp2f(s[nt][0] - b[nt][0]);
+        s[nt][1] = exp2f(s[nt][1] - b[nt][1]);
+        s[nt][2] = exp2f(s[nt][2] - b[nt][0]);
+        s[nt][3] = exp2f(s[nt][3] - b[nt][1]);
+        // per-thread partial row sums (this thread's two keys); reduced over lane/4 at the end of the item
+        w.l[nt][0] = w.l[nt][0] * c[nt][0] + (s[nt][0] + s[nt][2]);
+        w.l[nt][1] = w.l[nt][1] * c[nt][1] + (s[nt][1] + s[nt][3]);
+        // C fragment (key = lane/4, rows qa, qa+1) -> B fragment (keys 2*(lane%4), +1, row = lane/4): an 8x8 transpose
+        pb[nt][0] = movmatrix_t(pack_bf16(s[nt][0], s[nt][1]));
+        pb[nt][1] = movmatrix_t(pack_bf16(s[nt][2], s[nt][3]));
     }
-    l0 = l0 * c0 + rs0;  // per-thread partial sums; reduced across the quad at the end
-    l1 = l1 * c1 + rs1;
+    // O needs rescaling only when some row max of the warp moved (c = 1 exactly otherwise: skipping changes no bit)
+    if (__any_sync(0xffffffffu, moved)) {
 #pragma unroll
-    for (int nt = 0; nt < D / 8; ++nt) {
-        o[nt][0] *= c0;
-        o[nt][1] *= c0;
-        o[nt][2] *= c1;
-        o[nt][3] *= c1;
+        for (int np = 0; np < D / 16; ++np)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                w.o[np][nt][0] *= c[nt][0];
+                w.o[np][nt][1] *= c[nt][1];
+                w.o[np][nt][2] *= c[nt][0];
+                w.o[np][nt][3] *= c[nt][1];
+            }
     }
 #pragma unroll
-    for (int kg = 0; kg < NKG; ++kg) {
-        uint32_t a[4];
-        a[0] = pack_bf16(s[kg * 2][0], s[kg * 2][1]);
-        a[1] = pack_bf16(s[kg * 2][2], s[kg * 2][3]);
-        a[2] = pack_bf16(s[kg * 2 + 1][0], s[kg * 2 + 1][1]);
-        a[3] = pack_bf16(s[kg * 2 + 1][2], s[kg * 2 + 1][3]);
-        const int vrow = key_off + kg * 16 + (mi & 1) * 8 + rr;
+    for (int np = 0; np < D / 16; ++np) {
+        uint32_t va[4];  // A = V^T: dims x keys, i.e. the stored [key][dim] tile read through the transposing ldmatrix
+        ldsm_x4_t(va, sV + tile_off<D>(key_off + (mi >> 1) * 8 + rr, np * 2 + (mi & 1)));
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) mma16816(w.o[np][nt], va, pb[nt][0], pb[nt][1]);
+    }
+}
+
+// The tile loop of one item for NT * 8 query rows; leaves the warp's (unnormalised O^T, m, l) in the merge scratch.
+template <int D, int NT>
+__device__ __forceinline__ void decode_tiles(const KvView &kv, const ReqMeta &r, int log2G, int n_rows, int k_begin, int k_end,
+                                             int n_tiles, float scale_log2, uint32_t s_base, uint32_t sQ, unsigned char *smem,
+                                             int tid, int bar_id) {
+    constexpr int TILE_BYTES = kBN * D * 2;
+    const int lane = tid & 31, warp = tid >> 5;
+    uint32_t qf[D / 16][4];  // B = Q^T: [ks][2*nt], [2*nt+1] = dims ks*16 + {0..7, 8..15} of rows nt*8 + lane/4
+    {
+        const int mi = lane >> 3, rr = lane & 7;
+#pragma unroll
+        for (int ks = 0; ks < D / 16; ++ks) ldsm_x4(qf[ks], sQ + tile_off<D>((mi >> 1) * 8 + rr, ks * 2 + (mi & 1)));
+    }
+    // causal limits (inclusive last key) of this thread's rows; rows beyond n_rows are padding whose results are
+    // never read (Q is zero there, so they stay finite): no limit, so that they never force a mask
+    const int base_lim = r.kv_len - r.q_len;
+    int lim[NT][2];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int q = nt * 8 + 2 * (lane & 3) + j;
+            lim[nt][j] = q < n_rows ? base_lim + (q >> log2G) : 0x7fffffff;
+        }
+    const int lim_min = base_lim;  // row 0's limit, the smallest: tiles entirely at or below it need no mask
+
+    WarpState<D, NT> w;
+#pragma unroll
+    for (int np = 0; np < D / 16; ++np)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) w.o[np][nt][0] = w.o[np][nt][1] = w.o[np][nt][2] = w.o[np][nt][3] = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        w.m[nt][0] = w.m[nt][1] = -INFINITY;
+        w.l[nt][0] = w.l[nt][1] = 0.f;
+    }
+
+    for (int t = 0; t < n_tiles; ++t) {
+        cp_async_wait<kStages - 2>();
+        group_sync(bar_id);
+        {
+            const int tn = t + kStages - 1;
+            if (tn < n_tiles) {
+                const int sn = tn % kStages;
+                load_kv_tile<D>(kv, k_begin + tn * kBN, r.kv_len, s_base + sn * 2 * TILE_BYTES,
+                                s_base + sn * 2 * TILE_BYTES + TILE_BYTES, tid);
+            }
+            cp_async_commit();
+        }
+        const int st = t % kStages;
+        const uint32_t sK = s_base + st * 2 * TILE_BYTES, sV = sK + TILE_BYTES;
+        const int kt = k_begin + t * kBN;
+        const int key_off = warp * 16;
+        if (kt + key_off < k_end) {  // warp-uniform: this warp's 16 keys hold at least one live key
+            const bool need_mask = kt + key_off + 15 > lim_min;
+            warp_step<D, NT>(qf, sK, sV, key_off, kt, lim, need_mask, scale_log2, w, lane);
+        }
+    }
+    cp_async_wait<0>();
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            w.l[nt][j] += __shfl_xor_sync(0xffffffffu, w.l[nt][j], 4);
+            w.l[nt][j] += __shfl_xor_sync(0xffffffffu, w.l[nt][j], 8);
+            w.l[nt][j] += __shfl_xor_sync(0xffffffffu, w.l[nt][j], 16);
+        }
+    // ---- the warp's state into the merge scratch (each warp saw a disjoint quarter of every tile)
+    group_sync(bar_id);  // everyone is done with the stage buffers
+    float *sO = reinterpret_cast<float *>(smem);             // [4][16][D]
+    float *sM = sO + 4 * 16 * D;                             // [4][16]
+    float *sL = sM + 4 * 16;                                 // [4][16]
+    float *wo = sO + warp * 16 * D;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        const int qa = nt * 8 + 2 * (lane & 3);
 #pragma unroll
         for (int np = 0; np < D / 16; ++np) {
-            uint32_t b[4];
-            ldsm_x4_t(b, sV + tile_off<D>(vrow, np * 2 + (mi >> 1)));
-            mma16816(o[np * 2], a, b[0], b[1]);
-            mma16816(o[np * 2 + 1], a, b[2], b[3]);
+            const int dim = np * 16 + (lane >> 2);
+            wo[qa * D + dim] = w.o[np][nt][0];
+            wo[(qa + 1) * D + dim] = w.o[np][nt][1];
+            wo[qa * D + dim + 8] = w.o[np][nt][2];
+            wo[(qa + 1) * D + dim + 8] = w.o[np][nt][3];
+        }
+        if ((lane >> 2) == 0) {
+            sM[warp * 16 + qa] = w.m[nt][0];
+            sM[warp * 16 + qa + 1] = w.m[nt][1];
+            sL[warp * 16 + qa] = w.l[nt][0];
+            sL[warp * 16 + qa + 1] = w.l[nt][1];
         }
     }
 }
@@ -206,16 +326,15 @@ struct AttnArgs {
     float *part_lse;
     const __nv_bfloat16 *k_base, *v_base;
     const int32_t *block_table;
+    int32_t *tickets;  // [requests of the call][Hkv] arrival counters, zero on entry and on exit
     int64_t mpps, stride_page, stride_head;
     int32_t log2_page, Hq, Hkv, log2G;
     float scale_log2;
-    // Captured launches (sa_decode_step): the grid is sized for the step's capacity and the actual counts are read on the
-    // device, dyn = {requests, decode CTAs, ...} in the step's metadata slab; nullptr: counts are the launch's own.
+    // Captured launches (sa_decode_step): the grids are fixed and the actual counts are read on the device,
+    // dyn = {requests, items} at the head of the step's metadata; nullptr: the counts are the launch's own.
     const int32_t *dyn;
 };
 
-// barrier over one 128-thread group of the CTA (id 0 with 128 threads is __syncthreads of a 128-thread CTA)
-__device__ __forceinline__ void group_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 
 // Load BM packed rows of Q (row base rho0) into swizzled smem; rows beyond n_rows are zero.
 template <int D, int BM>
@@ -235,6 +354,73 @@ __device__ __forceinline__ void load_q_tile(const AttnArgs &a, const ReqMeta &r,
     }
 }
 
+// Merge of the splits of one (request, kv head), run by the LAST of its split items to finish (arrival counter in
+// the pool): each warp takes packed rows of the group; lanes cover D with float4.  Every sum has a fixed order that
+// depends on the request's split count alone (row max and the weight total: lane-strided, then a butterfly over the
+// warp; the output: split order), so a row's bits depend neither on its batch nor on which item arrived last.  The
+// partials of 4 splits are requested together and the next 4 before those are summed: one load per loop trip made the
+// merge a chain of L2 round trips as long as the streaming of the splits itself.  Loads bypass L1 (other SMs wrote).
+template <int D>
+__device__ __forceinline__ void merge_rows(const AttnArgs &a, const ReqMeta &r, int g, int tid) {
+    const int G = 1 << a.log2G;
+    const int n_rows = r.q_len * G;
+    const int lane = tid & 31, warp = tid >> 5;
+    constexpr int LANES = D / 4;
+    constexpr int U = 4;
+    const int n = r.n_splits;
+    for (int row = warp; row < n_rows; row += 4) {
+        const int tok = row >> a.log2G, hq = (g << a.log2G) + (row & (G - 1));
+        const int64_t p0 = int64_t(r.part_begin) + int64_t(tok) * a.Hq + hq;
+        const int64_t pstride = int64_t(r.q_len) * a.Hq;
+        float4 ov[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            ov[u] = (u < n && lane < LANES) ? __ldcg(reinterpret_cast<const float4 *>(a.part_o + (p0 + u * pstride) * D + lane * 4))
+                                            : make_float4(0.f, 0.f, 0.f, 0.f);
+        float M = -INFINITY;
+        for (int s = lane; s < n; s += 32) M = fmaxf(M, __ldcg(a.part_lse + p0 + s * pstride));
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, d));
+        const float Mb = (M == -INFINITY) ? 0.f : M;
+        float W = 0.f;
+        for (int s = lane; s < n; s += 32) W += exp2f(__ldcg(a.part_lse + p0 + s * pstride) - Mb);
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) W += __shfl_xor_sync(0xffffffffu, W, d);
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int s0 = 0; s0 < n; s0 += U) {
+            float ls[U];
+            float4 nx[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                ls[u] = s0 + u < n ? __ldcg(a.part_lse + p0 + (s0 + u) * pstride) : -INFINITY;
+                nx[u] = (s0 + U + u < n && lane < LANES)
+                            ? __ldcg(reinterpret_cast<const float4 *>(a.part_o + (p0 + (s0 + U + u) * pstride) * D + lane * 4))
+                            : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {  // split order
+                if (s0 + u < n) {
+                    const float w = exp2f(ls[u] - Mb);
+                    acc.x += ov[u].x * w;
+                    acc.y += ov[u].y * w;
+                    acc.z += ov[u].z * w;
+                    acc.w += ov[u].w * w;
+                }
+                ov[u] = nx[u];
+            }
+        }
+        const float inv = W > 0.f ? 1.f / W : 0.f;
+        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
+        if (lane < LANES) {
+            uint2 pk;
+            pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+            pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+            *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
+        }
+        if (a.lse && lane == 0) a.lse[orow] = (M + log2f(W)) * 0.6931471805599453f;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // Decode-like rows: split-KV, partials out.
 // One work item = one (request, kv head, 1024-key split), computed by a group of 128 threads over its own ring in
@@ -248,6 +434,7 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
     const int lane = tid & 31, warp = tid >> 5;
     const uint32_t s_base = smem_u32(smem);
     const uint32_t sQ = s_base + kStages * 2 * TILE_BYTES;
+    int32_t *s_pages = reinterpret_cast<int32_t *>(smem + kStages * 2 * TILE_BYTES + BM * D * 2);  // [kMaxSplitPages]
 
     const int ri = find_req(reqs, n_reqs, item);
     const ReqMeta r = reqs[ri];
@@ -261,12 +448,19 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
     KvView kv;
     kv.k_base = a.k_base;
     kv.v_base = a.v_base;
-    kv.bt_row = a.block_table + int64_t(r.sid) * a.mpps;
+    kv.pages = s_pages;
+    kv.page0 = k_begin >> a.log2_page;
     kv.stride_page = a.stride_page;
     kv.head_off = int64_t(g) * a.stride_head;
     kv.log2_page = a.log2_page;
 
     const int n_tiles = (k_end - k_begin + kBN - 1) / kBN;
+    {   // the split's slice of the block table (<= 64 entries) and Q: one global round trip, then the ring starts
+        const int n_pages = ((k_end - 1) >> a.log2_page) - kv.page0 + 1;
+        if (tid < n_pages) s_pages[tid] = __ldg(a.block_table + int64_t(r.sid) * a.mpps + kv.page0 + tid);
+    }
+    load_q_tile<D, BM>(a, r, g, rho0, n_rows, sQ, tid);
+    group_sync(bar_id);
     // prologue of the cp.async ring
 #pragma unroll
     for (int s = 0; s < kStages - 1; ++s) {
@@ -275,78 +469,14 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
                             s_base + s * 2 * TILE_BYTES + TILE_BYTES, tid);
         cp_async_commit();
     }
-    load_q_tile<D, BM>(a, r, g, rho0, n_rows, sQ, tid);
-    group_sync(bar_id);
-    constexpr int row_base = 0;
-    uint32_t qf[D / 16][4];
-    {
-        const int mi = lane >> 3, rr = lane & 7;
-#pragma unroll
-        for (int ks = 0; ks < D / 16; ++ks)
-            ldsm_x4(qf[ks], sQ + tile_off<D>(row_base + (mi & 1) * 8 + rr, ks * 2 + (mi >> 1)));
-    }
-    // causal limits (inclusive last key) of this thread's two rows
-    const int rA = rho0 + row_base + (lane >> 2), rB = rA + 8;
-    const int base_lim = r.kv_len - r.q_len;
-    const int lim0 = rA < n_rows ? base_lim + (rA >> a.log2G) : -1;
-    const int lim1 = rB < n_rows ? base_lim + (rB >> a.log2G) : -1;
-    // smallest limit among this warp's rows (warp-uniform): tiles entirely at or below it need no mask
-    const int warp_rows_lo = rho0 + row_base;
-    const int lim_min = (warp_rows_lo + 15 < n_rows) ? base_lim + (warp_rows_lo >> a.log2G) : -1;
-
-    float o[D / 8][4];
-#pragma unroll
-    for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
-    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
-
-    for (int t = 0; t < n_tiles; ++t) {
-        cp_async_wait<kStages - 2>();
-        group_sync(bar_id);
-        {
-            const int tn = t + kStages - 1;
-            if (tn < n_tiles) {
-                const int sn = tn % kStages;
-                load_kv_tile<D>(kv, k_begin + tn * kBN, r.kv_len, s_base + sn * 2 * TILE_BYTES,
-                                s_base + sn * 2 * TILE_BYTES + TILE_BYTES, tid);
-            }
-            cp_async_commit();
-        }
-        const int st = t % kStages;
-        const uint32_t sK = s_base + st * 2 * TILE_BYTES, sV = sK + TILE_BYTES;
-        const int kt = k_begin + t * kBN;
-        const int key_off = warp * 16;
-        if (kt + key_off < k_end) {  // warp-uniform: this warp's 16 keys hold at least one live key
-            const bool need_mask = kt + key_off + 15 > lim_min;
-            warp_step<D, 1>(qf, sK, sV, key_off, kt, lim0, lim1, need_mask, a.scale_log2, o, m0, m1, l0, l1, lane);
-        }
-    }
-    cp_async_wait<0>();
-    l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
-    l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
-    l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
-    l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-
-    // ---- merge the four warps' states (each saw a disjoint quarter of every tile)
-    group_sync(bar_id);  // everyone is done with the stage buffers
+    // rows as MMA columns: one n8 tile when the group's rows fit (every decode batch with G <= 8), else two
+    if (n_rows <= 8)
+        decode_tiles<D, 1>(kv, r, a.log2G, n_rows, k_begin, k_end, n_tiles, a.scale_log2, s_base, sQ, smem, tid, bar_id);
+    else
+        decode_tiles<D, 2>(kv, r, a.log2G, n_rows, k_begin, k_end, n_tiles, a.scale_log2, s_base, sQ, smem, tid, bar_id);
     float *sO = reinterpret_cast<float *>(smem);             // [4][16][D]
     float *sM = sO + 4 * 16 * D;                             // [4][16]
     float *sL = sM + 4 * 16;                                 // [4][16]
-    {
-        const int r0 = lane >> 2, r1 = r0 + 8;
-        float *wo = sO + warp * 16 * D;
-#pragma unroll
-        for (int nt = 0; nt < D / 8; ++nt) {
-            const int col = nt * 8 + 2 * (lane & 3);
-            *reinterpret_cast<float2 *>(wo + r0 * D + col) = make_float2(o[nt][0], o[nt][1]);
-            *reinterpret_cast<float2 *>(wo + r1 * D + col) = make_float2(o[nt][2], o[nt][3]);
-        }
-        if ((lane & 3) == 0) {
-            sM[warp * 16 + r0] = m0;
-            sM[warp * 16 + r1] = m1;
-            sL[warp * 16 + r0] = l0;
-            sL[warp * 16 + r1] = l1;
-        }
-    }
     group_sync(bar_id);
     for (int e = tid; e < n_rows * (D / 4); e += kThreads) {
         const int row = e / (D / 4), c4 = e % (D / 4);
@@ -372,6 +502,22 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
         *reinterpret_cast<float4 *>(a.part_o + prow * D + c4 * 4) = make_float4(acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv);
         if (c4 == 0) a.part_lse[prow] = L > 0.f ? M + log2f(L) : -INFINITY;  // log2 domain
     }
+    // ---- the last split of this (request, kv head) to get here merges them all: no second kernel, no launch gap
+    int *s_last = reinterpret_cast<int *>(s_pages + kMaxSplitPages);
+    __threadfence();
+    group_sync(bar_id);
+    if (tid == 0) {
+        int *ticket = a.tickets + ri * a.Hkv + g;
+        const int arrived = r.n_splits > 1 ? atomicAdd(ticket, 1) : 0;
+        const int last = arrived == r.n_splits - 1;
+        if (last && r.n_splits > 1) *ticket = 0;  // everyone else has been here: the counter is zero again for the next kernel
+        *s_last = last;
+    }
+    group_sync(bar_id);
+    if (*s_last) {
+        __threadfence();
+        merge_rows<D>(a, r, g, tid);
+    }
 }
 
 // grid = decode CTAs of the call (one item each).  INLINE: the requests of a small decode-only call ride in the kernel
@@ -379,12 +525,31 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
 template <int D, bool INLINE>
 __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
-    int n_reqs = a.n_reqs;
-    if (!INLINE && a.dyn) {
-        n_reqs = a.dyn[0];
-        if (int(blockIdx.x) >= a.dyn[1]) return;
+    decode_item<D>(a, INLINE ? ir.reqs : a.reqs, a.n_reqs, blockIdx.x, smem, threadIdx.x, 0);
+}
+
+// Captured decode step (sa_decode_step_enqueue): the launch is recorded once and replayed on batches whose size and
+// lengths change, so the grid is fixed and the counts are read on the device (dyn = {requests, items} in the step's
+// metadata); the CTAs stride over the items.  Which CTA runs an item does not enter its arithmetic.
+template <int D>
+__global__ void __launch_bounds__(kThreads, 3) flash_mma_loop_kernel(const AttnArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    // programmatic dependent launch: this grid is staged while the step's append kernel runs and waits here for its
+    // results (the metadata twin, the new token in the cache, the rotated q)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // the step's whole request array (a.n_reqs = its capacity; entries past the count are never looked at) comes into
+    // shared memory together with the counts: one global round trip instead of a binary search of dependent ones
+    ReqMeta *s_reqs = reinterpret_cast<ReqMeta *>(smem + group_smem<D>());
+    const bool cached = a.n_reqs <= kLoopReqCache;
+    if (cached)
+        for (int i = threadIdx.x; i < a.n_reqs * int(sizeof(ReqMeta) / 16); i += kThreads)
+            reinterpret_cast<uint4 *>(s_reqs)[i] = reinterpret_cast<const uint4 *>(a.reqs)[i];
+    const int n_reqs = a.dyn[0], n_items = a.dyn[1];
+    __syncthreads();
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        decode_item<D>(a, cached ? s_reqs : a.reqs, n_reqs, item, smem, threadIdx.x, 0);
+        group_sync(0);  // the merge scratch and the page list of this item live where the next item's ring goes
     }
-    decode_item<D>(a, INLINE ? ir.reqs : a.reqs, n_reqs, blockIdx.x, smem, threadIdx.x, 0);
 }
 
 // The same items on a FIXED number of CTAs, each with two 128-thread groups that walk the item list with their own
@@ -393,58 +558,12 @@ __global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_consta
 template <int D>
 __global__ void __launch_bounds__(2 * kThreads) flash_mma_persist_kernel(const AttnArgs a, int n_items) {
     extern __shared__ __align__(128) unsigned char smem[];
-    constexpr size_t GROUP_BYTES = size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2;
+    constexpr size_t GROUP_BYTES = group_smem<D>();
     const int grp = threadIdx.x >> 7, tid = threadIdx.x & 127;
     unsigned char *my = smem + size_t(grp) * GROUP_BYTES;
     for (int item = blockIdx.x * 2 + grp; item < n_items; item += gridDim.x * 2) {
         decode_item<D>(a, a.reqs, a.n_reqs, item, my, tid, 1 + grp);
         group_sync(1 + grp);  // the merge scratch of this item lives in the ring the next item fills
-    }
-}
-
-// Merge of the split partials, fixed split order.  grid = (decode-like requests, Hkv); each warp
-// takes packed rows of the group; lanes cover D with float4.
-template <int D, bool INLINE>
-__global__ void __launch_bounds__(128) merge_splits_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
-    // launched with programmatic stream serialization: the grid is staged while the split kernel drains and waits
-    // here until that kernel has completed and its partials are visible (a no-op for an ordinary launch)
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (!INLINE && a.dyn && int(blockIdx.x) >= a.dyn[0]) return;
-    const ReqMeta r = INLINE ? ir.reqs[blockIdx.x] : a.reqs[blockIdx.x];
-    const int g = blockIdx.y;
-    const int G = 1 << a.log2G;
-    const int n_rows = r.q_len * G;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    constexpr int LANES = D / 4;
-    for (int row = warp; row < n_rows; row += 4) {
-        const int tok = row >> a.log2G, hq = (g << a.log2G) + (row & (G - 1));
-        const int64_t p0 = int64_t(r.part_begin) + int64_t(tok) * a.Hq + hq;
-        const int64_t pstride = int64_t(r.q_len) * a.Hq;
-        float M = -INFINITY;
-        for (int s = 0; s < r.n_splits; ++s) M = fmaxf(M, a.part_lse[p0 + s * pstride]);
-        const float Mb = (M == -INFINITY) ? 0.f : M;
-        float W = 0.f;
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int s = 0; s < r.n_splits; ++s) {
-            const float w = exp2f(a.part_lse[p0 + s * pstride] - Mb);
-            W += w;
-            if (lane < LANES) {
-                const float4 ov = *reinterpret_cast<const float4 *>(a.part_o + (p0 + s * pstride) * D + lane * 4);
-                acc.x += ov.x * w;
-                acc.y += ov.y * w;
-                acc.z += ov.z * w;
-                acc.w += ov.w * w;
-            }
-        }
-        const float inv = W > 0.f ? 1.f / W : 0.f;
-        const int64_t orow = int64_t(r.q_start + tok) * a.Hq + hq;
-        if (lane < LANES) {
-            uint2 pk;
-            pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-            pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-            *reinterpret_cast<uint2 *>(a.out + orow * D + lane * 4) = pk;
-        }
-        if (a.lse && lane == 0) a.lse[orow] = (M + log2f(W)) * 0.6931471805599453f;
     }
 }
 
@@ -461,6 +580,7 @@ AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const
     a.k_base = static_cast<const __nv_bfloat16 *>(pool->k_base);
     a.v_base = static_cast<const __nv_bfloat16 *>(pool->v_base);
     a.block_table = pool->block_table;
+    a.tickets = pool->tickets;
     a.mpps = pool->max_pages_per_session;
     a.stride_page = pool->stride_page;
     a.stride_head = pool->stride_head;
@@ -488,31 +608,9 @@ cudaError_t opt_in_smem(size_t smem) {
     return e;
 }
 
-template <int D>
-constexpr size_t group_smem() {
-    return size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2;
-}
-
-// The merge of the splits is launched with programmatic stream serialization: its grid is set up while the split
-// kernel still runs and starts (griddepcontrol.wait at its top) the moment that kernel has completed.
-template <int D, bool INLINE>
-cudaError_t launch_merge(const InlineReqs &ir, const AttnArgs &a, dim3 grid, cudaStream_t stream) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid;
-    cfg.blockDim = dim3(128);
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, merge_splits_kernel<D, INLINE>, ir, a);
-}
 
 template <int D, bool INLINE>
-cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, dim3 merge_grid, cudaStream_t stream,
-                         int32_t *launches) {
+cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, cudaStream_t stream, int32_t *launches) {
     constexpr size_t smem = group_smem<D>();
     static_assert(smem >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
     cudaError_t e = opt_in_smem<&flash_mma_kernel<D, INLINE>>(smem);
@@ -521,13 +619,34 @@ cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, dim
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     ++*launches;
-    e = launch_merge<D, INLINE>(ir, a, merge_grid, stream);
+    return e;
+}
+
+template <int D>
+cudaError_t launch_flash_loop(const AttnArgs &a, int n_cta, cudaStream_t stream, int32_t *launches) {
+    constexpr size_t smem = group_smem<D>() + kLoopReqCache * sizeof(ReqMeta);
+    cudaError_t e = opt_in_smem<&flash_mma_loop_kernel<D>>(smem);
+    if (e != cudaSuccess) return e;
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(unsigned(n_cta));
+        cfg.blockDim = dim3(kThreads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, flash_mma_loop_kernel<D>, a);
+    }
+    if (e != cudaSuccess) return e;
     ++*launches;
     return e;
 }
 
 template <int D>
-cudaError_t launch_flash_persist(const AttnArgs &a, int items, int n_cta, dim3 merge_grid, cudaStream_t stream, int32_t *launches) {
+cudaError_t launch_flash_persist(const AttnArgs &a, int items, int n_cta, cudaStream_t stream, int32_t *launches) {
     constexpr size_t smem = 2 * group_smem<D>();
     cudaError_t e = opt_in_smem<&flash_mma_persist_kernel<D>>(smem);
     if (e != cudaSuccess) return e;
@@ -535,38 +654,43 @@ cudaError_t launch_flash_persist(const AttnArgs &a, int items, int n_cta, dim3 m
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     ++*launches;
-    static const InlineReqs none{};
-    e = launch_merge<D, false>(none, a, merge_grid, stream);
-    ++*launches;
     return e;
 }
 
 }  // namespace
 
+cudaError_t flash_loop_prepare(const sa_kv_pool *pool) {
+    return pool->cfg.head_dim == 128 ? opt_in_smem<&flash_mma_loop_kernel<128>>(group_smem<128>() + kLoopReqCache * sizeof(ReqMeta))
+                                     : opt_in_smem<&flash_mma_loop_kernel<64>>(group_smem<64>() + kLoopReqCache * sizeof(ReqMeta));
+}
+
 // reqs_host != nullptr (and plan.n_dec <= kInlineReqs): the requests go in the kernel parameters, reqs_dev is unused.
 // persist_ctas > 0: the items run on that many two-group CTAs (one per SM) instead of one CTA each.
-// dyn != nullptr (captured step): grid sizes come from `plan` (the step's capacity), the actual counts from dyn.
+// dyn != nullptr (captured step): persist_ctas CTAs stride over the items, plan.n_dec is the capacity of the step's
+// request array, the actual counts come from dyn.
 cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
                                 const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
                                 float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches,
                                 int persist_ctas, const int32_t *dyn) {
-    if (plan.dec_items == 0) return cudaSuccess;
+    if (plan.dec_items == 0 && !dyn) return cudaSuccess;
     AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
     a.dyn = dyn;
-    const dim3 grid(unsigned(plan.n_dec), unsigned(pool->cfg.num_kv_heads));
     const bool d128 = pool->cfg.head_dim == 128;
     if (reqs_host) {
         InlineReqs ir;
         memcpy(ir.reqs, reqs_host, sizeof(ReqMeta) * size_t(plan.n_dec));
-        return d128 ? launch_flash<128, true>(ir, a, plan.dec_items, grid, stream, launches)
-                    : launch_flash<64, true>(ir, a, plan.dec_items, grid, stream, launches);
+        return d128 ? launch_flash<128, true>(ir, a, plan.dec_items, stream, launches)
+                    : launch_flash<64, true>(ir, a, plan.dec_items, stream, launches);
     }
+    if (dyn)
+        return d128 ? launch_flash_loop<128>(a, persist_ctas, stream, launches)
+                    : launch_flash_loop<64>(a, persist_ctas, stream, launches);
     if (persist_ctas > 0)
-        return d128 ? launch_flash_persist<128>(a, plan.dec_items, persist_ctas, grid, stream, launches)
-                    : launch_flash_persist<64>(a, plan.dec_items, persist_ctas, grid, stream, launches);
+        return d128 ? launch_flash_persist<128>(a, plan.dec_items, persist_ctas, stream, launches)
+                    : launch_flash_persist<64>(a, plan.dec_items, persist_ctas, stream, launches);
     static const InlineReqs none{};  // never read by the slab variants
-    return d128 ? launch_flash<128, false>(none, a, plan.dec_items, grid, stream, launches)
-                : launch_flash<64, false>(none, a, plan.dec_items, grid, stream, launches);
+    return d128 ? launch_flash<128, false>(none, a, plan.dec_items, stream, launches)
+                : launch_flash<64, false>(none, a, plan.dec_items, stream, launches);
 }
 
 }  // namespace sa

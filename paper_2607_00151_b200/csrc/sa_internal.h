@@ -47,6 +47,19 @@ struct InlineReqs {
     ReqMeta reqs[kInlineReqs];
 };
 
+// Metadata of a captured decode step (sa_decode_step_*): a pinned host slab the host rewrites between replays and a
+// device twin the step's first kernel refreshes.  Layout: [StepHeader][ReqMeta x cap][StepAppend x cap].
+struct StepHeader {
+    int32_t n_req;    // requests of this step (<= cap)
+    int32_t n_items;  // decode work items = sum over requests of Hkv * n_splits
+    int32_t pad[6];
+};
+struct StepAppend {
+    int32_t sid, pos, page, pad;  // the request's new token: position in the session, page that holds its slot
+};
+__host__ __device__ inline size_t step_append_offset(int32_t cap) { return sizeof(StepHeader) + sizeof(ReqMeta) * size_t(cap); }
+__host__ __device__ inline size_t step_slab_bytes(int32_t cap) { return step_append_offset(cap) + sizeof(StepAppend) * size_t(cap); }
+
 // tcgen05 prefill kernel: one persistent CTA per SM walks a list of parts.  An item is (request, kv
 // head, 256 packed rows); a part is the KV-tile range [u0, u1) of an item.  slot < 0: the part is the
 // whole item and writes the output directly; otherwise it writes partial slot `slot` and the merge
@@ -99,6 +112,7 @@ struct sa_kv_pool {
     void *v_base = nullptr;
     int32_t *block_table = nullptr;  // [max_sessions][max_pages_per_session]
     float2 *rope_tab = nullptr;      // [D/2] (hi, lo) of theta_m / (2 pi)
+    int32_t *tickets = nullptr;      // [max_sessions][Hkv] arrival counters of the split-KV decode kernel (zero between kernels)
     char *meta_dev = nullptr;        // [kMetaRing][meta_slab_bytes]
     size_t meta_slab_bytes = 0;
     int64_t stride_page = 0, stride_head = 0, stride_slot = 0;
@@ -197,6 +211,12 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
 cudaError_t launch_rope_append(const sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_t n_req,
                                int64_t total_rows, const void *k, const void *v, void *q,
                                cudaStream_t stream, int32_t *launches);
+
+// the step's first kernel: slab_host -> slab_dev, then RoPE + placement of one token per request (sa_append.cu)
+cudaError_t launch_step_append(const sa_kv_pool *pool, const void *slab_host, void *slab_dev, int32_t cap, const void *k,
+                               const void *v, void *q, cudaStream_t stream, int32_t *launches);
+// shared-memory opt-in of the step's decode kernel for the current device (so that nothing but launches happens later)
+cudaError_t flash_loop_prepare(const sa_kv_pool *pool);
 
 struct AttnPlan {
     int32_t n_dec = 0, n_pre = 0;        // requests per class

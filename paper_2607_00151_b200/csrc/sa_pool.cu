@@ -14,7 +14,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {
-    size_t k_off, v_off, bt_off, rope_off, meta_off, total, kv_bytes, slab;
+    size_t k_off, v_off, bt_off, rope_off, ticket_off, meta_off, total, kv_bytes, slab;
     int64_t mpps;
 };
 
@@ -49,6 +49,8 @@ Carve carve(const sa_kv_pool_config *c) {
     off = align_up(off + size_t(c->max_sessions) * r.mpps * 4, 256);
     r.rope_off = off;
     off = align_up(off + size_t(c->head_dim / 2) * sizeof(float2), 256);
+    r.ticket_off = off;  // one arrival counter per (request of a call, kv head): the last split to finish merges
+    off = align_up(off + size_t(c->max_sessions) * c->num_kv_heads * 4, 256);
     r.meta_off = off;
     off += r.slab * sa::kMetaRing;
     r.total = off;
@@ -118,6 +120,7 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
         pool->v_base = base + cv.v_off;
         pool->block_table = reinterpret_cast<int32_t *>(base + cv.bt_off);
         pool->rope_tab = reinterpret_cast<float2 *>(base + cv.rope_off);
+        pool->tickets = reinterpret_cast<int32_t *>(base + cv.ticket_off);
         pool->meta_dev = base + cv.meta_off;
         sa::DeviceGuard device_guard(cfg->device);  // the caller's current device is restored on return
         bool ok = device_guard.ok;
@@ -140,6 +143,8 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
                 tab[size_t(m)] = make_float2(hi, lo);
             }
             ok = cudaMemcpy(pool->rope_tab, tab.data(), sizeof(float2) * size_t(half), cudaMemcpyHostToDevice) == cudaSuccess;
+            // the counters start at zero and every kernel that uses them leaves them at zero
+            ok = ok && cudaMemset(pool->tickets, 0, size_t(cfg->max_sessions) * cfg->num_kv_heads * 4) == cudaSuccess;
         }
         if (ok) ok = sa::tc5_init(pool) == SA_OK;
         if (!ok) {

@@ -47,7 +47,7 @@ def profile(pool: sa.Pool, prefixes=(2048, 8192, 24576), prefill_tokens=(0, 256,
     return np.array(ms_all, dtype=np.float32), np.array(sums_all, dtype=np.int64), np.array(tok_all, dtype=np.int64)
 
 
-def time_batch(pool: sa.Pool, decode_L, chunks, iters=9, warmup=3, seed=0):
+def time_batch(pool: sa.Pool, decode_L, chunks, iters=15, warmup=4, seed=0):
     """Median CUDA-event time (ms) of ONE sa_mixed_attention call on a batch of decode requests with caches
     of decode_L tokens and prefill chunks (q, prefix); scratch sessions are filled with seeded uniform values."""
     cfg = pool.cfg

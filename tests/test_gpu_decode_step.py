@@ -1,0 +1,109 @@
+"""The capturable decode iteration (sa_decode_step_prepare + sa_decode_step_enqueue, the TBT path):
+bit-equal to sa_rope_kv_append + sa_mixed_attention on a twin pool, eagerly and as ONE captured CUDA graph replayed over
+iterations whose batch changes (sessions join and leave, caches cross page and 1024-key split boundaries), and within
+the gates of the fp64 oracle."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2607_00151_b200 import binding as sa
+from gpu_util import check_derived
+
+pytestmark = pytest.mark.gpu
+
+
+def _bits(t):
+    return t.view(torch.int16)
+
+
+def _twin_pools(Hq, Hkv, D, page, pages, max_sessions, max_tokens, base, seed):
+    order = np.random.default_rng(seed).permutation(pages).astype(np.int32)
+    cfg = sa.PoolConfig(Hq, Hkv, D, page, pages, max_sessions, max_tokens, base, 0)
+    return sa.sa_kv_pool_create(cfg, free_page_order=order), sa.sa_kv_pool_create(cfg, free_page_order=order), cfg
+
+
+@pytest.mark.parametrize("shape", [(32, 8, 128, 64, 500000.0), (8, 2, 64, 16, 1e4)])
+def test_decode_step_graph_replay_equals_eager_calls_bitwise(shape):
+    Hq, Hkv, D, page, base = shape
+    # caches that sit on and around a page end, a split end (1024 keys) and the empty session
+    lens0 = [1023, 1024, 63, 2500, 5000, 0, 64, 2047]
+    n = len(lens0)
+    iters = 5
+    pages = sum((L + iters + page - 1) // page + 1 for L in lens0) + 8
+    eager, stepped, cfg = _twin_pools(Hq, Hkv, D, page, pages, n + 1, 8192, base, 5)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(1234)
+    rnd = lambda t, h: (torch.randn((t, h, D), generator=gen, device="cuda") * 0.7).to(torch.bfloat16)
+    hist_k, hist_v = [rnd(L, Hkv) for L in lens0], [rnd(L, Hkv) for L in lens0]
+    sids_e = [sa.sa_kv_session_open(eager) for _ in range(n)]
+    sids_s = [sa.sa_kv_session_open(stepped) for _ in range(n)]
+    live = [i for i in range(n) if lens0[i] > 0]
+    indptr = np.concatenate([[0], np.cumsum([lens0[i] for i in live])]).astype(np.int32)
+    kk, vv = torch.cat([hist_k[i] for i in live]), torch.cat([hist_v[i] for i in live])
+    for pool, sids in ((eager, sids_e), (stepped, sids_s)):
+        sa.sa_rope_kv_append(pool, [sids[i] for i in live], indptr, kk, vv, None)
+    step = sa.sa_decode_step_create(stepped, n, 8192)
+    # static buffers of the captured graph
+    k_in, v_in = torch.zeros((n, Hkv, D), dtype=torch.bfloat16, device="cuda"), torch.zeros((n, Hkv, D), dtype=torch.bfloat16, device="cuda")
+    q_in, out = torch.zeros((n, Hq, D), dtype=torch.bfloat16, device="cuda"), torch.full((n, Hq, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    lse = torch.full((n, Hq), float("nan"), dtype=torch.float32, device="cuda")
+    graph = None
+    batches = [list(range(n)), [0, 3, 5], [1], list(range(n - 1, -1, -1)), [2, 4, 6, 7, 0]]
+    for it, batch in enumerate(batches):
+        b = len(batch)
+        k1, v1, q1 = rnd(b, Hkv), rnd(b, Hkv), rnd(b, Hq)
+        # ---- eager reference path on the twin pool
+        qe = q1.clone()
+        ip = np.arange(b + 1, dtype=np.int32)
+        se = [sids_e[i] for i in batch]
+        sa.sa_rope_kv_append(eager, se, ip, k1, v1, qe)
+        oe, le = torch.empty_like(qe), torch.empty((b, Hq), dtype=torch.float32, device="cuda")
+        ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(eager, se, ip), 256), dtype=torch.uint8, device="cuda")
+        sa.sa_mixed_attention(eager, se, ip, qe, oe, le, 0.0, ws)
+        # ---- the step: host half, then the device half (captured on the first iteration, replayed afterwards)
+        torch.cuda.synchronize()                      # the previous replay has consumed the slab
+        sa.sa_decode_step_prepare(step, [sids_s[i] for i in batch])
+        k_in[:b], v_in[:b], q_in[:b] = k1, v1, q1
+        out.fill_(float("nan"))
+        lse.fill_(float("nan"))
+        if it == 0:
+            sa.sa_decode_step_enqueue(step, k_in, v_in, q_in, out, lse)      # eager enqueue of the same two launches
+            torch.cuda.synchronize()
+            assert sa.sa_decode_step_stats(step)["launches"] == 2
+            assert torch.equal(_bits(out[:b]), _bits(oe)) and torch.equal(lse[:b], le) and torch.equal(_bits(q_in[:b]), _bits(qe))
+            # enqueue is idempotent for a prepared step; capture it (nothing runs during capture)
+            q_in[:b] = q1
+            out.fill_(float("nan"))
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                sa.sa_decode_step_enqueue(step, k_in, v_in, q_in, out, lse)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(_bits(out[:b]), _bits(oe)), "iteration %d: output bits differ from the eager calls" % it
+        assert torch.equal(lse[:b], le)
+        assert torch.equal(_bits(q_in[:b]), _bits(qe)), "rotated q differs"
+        assert torch.isnan(out[b:].float()).all() and torch.isnan(lse[b:]).all(), "rows beyond the step's batch were written"
+        for j, i in enumerate(batch):
+            hist_k[i] = torch.cat([hist_k[i], k1[j:j + 1]])
+            hist_v[i] = torch.cat([hist_v[i], v1[j:j + 1]])
+        if it == len(batches) - 1:
+            # the oracle on the last iteration's rows (definition: PAPER.md L305, one query over the whole cache)
+            for j, i in enumerate(batch):
+                L = hist_k[i].shape[0]
+                kr = orc.rope(hist_k[i][:L - 1].cpu(), np.arange(L - 1), base)
+                ref = orc.oracle_cached(kr, orc.widen(hist_v[i][:L - 1].cpu()), q1[j:j + 1].cpu(), hist_k[i][L - 1:].cpu(),
+                                        hist_v[i][L - 1:].cpu(), L - 1, base)
+                # gates of DESIGN.md 3a for these inputs: scores of std sm_scale * 0.7 * 0.7 * sqrt(D) = 0.49, V of std 0.7
+                check_derived(out[j:j + 1], lse[j:j + 1], ref, 0.49, 0.7, "step row s%d" % i)
+    # ---- the caches of the two pools hold the same bits
+    for i in range(n):
+        Le, Ls = sa.sa_kv_session_query(eager, sids_e[i])[0], sa.sa_kv_session_query(stepped, sids_s[i])[0]
+        assert Le == Ls == hist_k[i].shape[0]
+        ie = torch.empty((2, Hkv, Le, D), dtype=torch.bfloat16, device="cuda")
+        is_ = torch.empty_like(ie)
+        sa.sa_kv_session_export(eager, sids_e[i], 0, Le, ie)
+        sa.sa_kv_session_export(stepped, sids_s[i], 0, Ls, is_)
+        torch.cuda.synchronize()
+        assert torch.equal(_bits(ie), _bits(is_)), "session %d: stored K'/V differ" % i
+    assert sa.sa_kv_pool_free_pages(eager) == sa.sa_kv_pool_free_pages(stepped)
