@@ -6,6 +6,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <new>
 #include <vector>
 
 #include "sa_internal.h"
@@ -29,7 +30,7 @@ struct HostPlan {
 
 // The split of a request depends only on that request (never on its batch), so co-batching
 // cannot change the bits of a row.
-int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
+int32_t build_plan_uncached(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr,
                    HostPlan *hp, bool before_append = false) {
     if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
     if (n_req == 0) return SA_OK;
@@ -99,6 +100,54 @@ int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, c
     return SA_OK;
 }
 
+}  // namespace
+
+// The plan of the last batch planned on this pool.  sa_mixed_attention_workspace_bytes and the sa_mixed_attention call
+// that follows it name the same batch on unchanged sessions: the second of them takes the plan (classes, splits,
+// the stream-K schedule: 10-80 us of host time for a chunked batch) from here instead of building it again.
+struct PlanCache {
+    bool valid = false;
+    bool before_append = false;
+    std::vector<int32_t> sids, indptr;
+    std::vector<int64_t> lens;  // session lengths the plan was built on
+    HostPlan hp;
+};
+
+namespace {
+
+int32_t build_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids, const int32_t *qo_indptr, const HostPlan **out,
+                   bool before_append = false) {
+    static const HostPlan empty;
+    *out = &empty;
+    if (!pool || n_req < 0) return SA_ERR_INVALID_ARG;
+    if (n_req == 0) return SA_OK;
+    if (!sids || !qo_indptr || n_req > pool->cfg.max_sessions) return SA_ERR_INVALID_ARG;
+    PlanCache &pc = *pool->plan_cache;
+    bool hit = pc.valid && pc.before_append == before_append && pc.sids.size() == size_t(n_req);
+    for (int r = 0; hit && r < n_req; ++r) {
+        const int32_t sid = sids[r];
+        hit = sid == pc.sids[size_t(r)] && qo_indptr[r + 1] == pc.indptr[size_t(r) + 1] && sid >= 0 &&
+              size_t(sid) < pool->sessions.size() && pool->sessions[size_t(sid)].open &&
+              pool->sessions[size_t(sid)].len == pc.lens[size_t(r)];
+    }
+    if (hit && qo_indptr[0] == 0) {
+        *out = &pc.hp;
+        return SA_OK;
+    }
+    pc.valid = false;
+    pc.hp = HostPlan();
+    const int32_t st = build_plan_uncached(pool, n_req, sids, qo_indptr, &pc.hp, before_append);
+    if (st != SA_OK) return st;
+    pc.before_append = before_append;
+    pc.sids.assign(sids, sids + n_req);
+    pc.indptr.assign(qo_indptr, qo_indptr + n_req + 1);
+    pc.lens.resize(size_t(n_req));
+    for (int r = 0; r < n_req; ++r) pc.lens[size_t(r)] = pool->sessions[size_t(sids[r])].len;
+    pc.valid = true;
+    *out = &pc.hp;
+    return SA_OK;
+}
+
 // workspace: [decode partial O f32][decode partial lse f32][tcgen05 partial slots][tcgen05 schedule payload]
 struct WsLayout {
     size_t off_part_lse, off_slots, off_sched, total;
@@ -125,12 +174,15 @@ void write_sched_payload(const Tc5Schedule &sc, char *dst) {
 
 }  // namespace
 
+PlanCache *plan_cache_new() { return new (std::nothrow) PlanCache(); }
+void plan_cache_delete(PlanCache *pc) { delete pc; }
+
 int32_t attention_workspace_after_append(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                          const int32_t *qo_indptr, size_t *out_bytes) {
-    HostPlan hp;
-    const int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hp, true);
+    const HostPlan *hpp = nullptr;
+    const int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hpp, true);
     if (st != SA_OK) return st;
-    *out_bytes = workspace_need(pool, hp);
+    *out_bytes = workspace_need(pool, *hpp);
     return SA_OK;
 }
 
@@ -139,19 +191,20 @@ int32_t attention_workspace_after_append(const sa_kv_pool *pool, int32_t n_req, 
 extern "C" int32_t sa_mixed_attention_workspace_bytes(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                                       const int32_t *qo_indptr, size_t *out_bytes) {
     if (!out_bytes) return SA_ERR_INVALID_ARG;
-    sa::HostPlan hp;
-    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hp);
+    const sa::HostPlan *hpp = nullptr;
+    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hpp);
     if (st != SA_OK) return st;
-    *out_bytes = sa::workspace_need(pool, hp);
+    *out_bytes = sa::workspace_need(pool, *hpp);
     return SA_OK;
 }
 
 extern "C" int32_t sa_mixed_attention_plan(const sa_kv_pool *pool, int32_t n_req, const int32_t *sids,
                                            const int32_t *qo_indptr, int64_t *out_stats) {
     if (!out_stats) return SA_ERR_INVALID_ARG;
-    sa::HostPlan hp;
-    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hp);
+    const sa::HostPlan *hpp = nullptr;
+    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hpp);
     if (st != SA_OK) return st;
+    const sa::HostPlan &hp = *hpp;
     out_stats[0] = hp.plan.n_dec;
     out_stats[1] = hp.plan.n_pre;
     out_stats[2] = hp.plan.dec_items;
@@ -167,9 +220,10 @@ extern "C" int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n
                                                const int32_t *qo_indptr, int32_t *out_parts, int32_t cap,
                                                int64_t *out_summary) {
     if (!out_summary || cap < 0) return SA_ERR_INVALID_ARG;
-    sa::HostPlan hp;
-    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hp);
+    const sa::HostPlan *hpp = nullptr;
+    int32_t st = sa::build_plan(pool, n_req, sids, qo_indptr, &hpp);
     if (st != SA_OK) return st;
+    const sa::HostPlan &hp = *hpp;
     if (!sa::tc5_supported(pool)) return SA_ERR_UNSUPPORTED;
     const sa::Tc5Schedule &sc = hp.sched;
     out_summary[0] = pool->num_sms;
@@ -202,9 +256,10 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     sa::DeviceGuard device_guard(pool);
     if (!device_guard.ok) return SA_ERR_CUDA;
     using namespace sa;
-    HostPlan hp;
-    int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hp);
+    const HostPlan *hpp = nullptr;
+    int32_t st = build_plan(pool, n_req, sids, qo_indptr, &hpp);
     if (st != SA_OK) return st;
+    const HostPlan &hp = *hpp;
     if (pool->host_only) return SA_ERR_CUDA;
     pool->last_launches = 0;
     if (hp.plan.n_dec + hp.plan.n_pre == 0) return SA_OK;

@@ -118,7 +118,7 @@ __device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_le
     }
 }
 
-// barrier over one 128-thread group of the CTA (id 0 with 128 threads is __syncthreads of a 128-thread CTA)
+// barrier over the 128 threads that run an item (id 0 with 128 threads is __syncthreads of a 128-thread CTA)
 __device__ __forceinline__ void group_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 
 __device__ __forceinline__ uint32_t movmatrix_t(uint32_t x) {  // transpose of an 8x8 b16 matrix held one row pair per lane
@@ -552,21 +552,6 @@ __global__ void __launch_bounds__(kThreads, 3) flash_mma_loop_kernel(const AttnA
     }
 }
 
-// The same items on a FIXED number of CTAs, each with two 128-thread groups that walk the item list with their own
-// rings (2 x 100 KiB of shared memory: nothing else fits on the SM).  Used by the overlapped mixed call, where the
-// decode rows must stay on a subset of the SMs while the tensor-core prefill kernel owns the others.
-template <int D>
-__global__ void __launch_bounds__(2 * kThreads) flash_mma_persist_kernel(const AttnArgs a, int n_items) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    constexpr size_t GROUP_BYTES = group_smem<D>();
-    const int grp = threadIdx.x >> 7, tid = threadIdx.x & 127;
-    unsigned char *my = smem + size_t(grp) * GROUP_BYTES;
-    for (int item = blockIdx.x * 2 + grp; item < n_items; item += gridDim.x * 2) {
-        decode_item<D>(a, a.reqs, a.n_reqs, item, my, tid, 1 + grp);
-        group_sync(1 + grp);  // the merge scratch of this item lives in the ring the next item fills
-    }
-}
-
 AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const void *q, void *out, float *lse,
                    float sm_scale, float *part_o, float *part_lse) {
     AttnArgs a;
@@ -645,18 +630,6 @@ cudaError_t launch_flash_loop(const AttnArgs &a, int n_cta, cudaStream_t stream,
     return e;
 }
 
-template <int D>
-cudaError_t launch_flash_persist(const AttnArgs &a, int items, int n_cta, cudaStream_t stream, int32_t *launches) {
-    constexpr size_t smem = 2 * group_smem<D>();
-    cudaError_t e = opt_in_smem<&flash_mma_persist_kernel<D>>(smem);
-    if (e != cudaSuccess) return e;
-    flash_mma_persist_kernel<D><<<unsigned(n_cta), 2 * kThreads, smem, stream>>>(a, items);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    ++*launches;
-    return e;
-}
-
 }  // namespace
 
 cudaError_t flash_loop_prepare(const sa_kv_pool *pool) {
@@ -665,13 +638,12 @@ cudaError_t flash_loop_prepare(const sa_kv_pool *pool) {
 }
 
 // reqs_host != nullptr (and plan.n_dec <= kInlineReqs): the requests go in the kernel parameters, reqs_dev is unused.
-// persist_ctas > 0: the items run on that many two-group CTAs (one per SM) instead of one CTA each.
-// dyn != nullptr (captured step): persist_ctas CTAs stride over the items, plan.n_dec is the capacity of the step's
+// dyn != nullptr (captured step): loop_ctas CTAs stride over the items, plan.n_dec is the capacity of the step's
 // request array, the actual counts come from dyn.
 cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
                                 const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
                                 float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches,
-                                int persist_ctas, const int32_t *dyn) {
+                                int loop_ctas, const int32_t *dyn) {
     if (plan.dec_items == 0 && !dyn) return cudaSuccess;
     AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
     a.dyn = dyn;
@@ -683,11 +655,8 @@ cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
                     : launch_flash<64, true>(ir, a, plan.dec_items, stream, launches);
     }
     if (dyn)
-        return d128 ? launch_flash_loop<128>(a, persist_ctas, stream, launches)
-                    : launch_flash_loop<64>(a, persist_ctas, stream, launches);
-    if (persist_ctas > 0)
-        return d128 ? launch_flash_persist<128>(a, plan.dec_items, persist_ctas, stream, launches)
-                    : launch_flash_persist<64>(a, plan.dec_items, persist_ctas, stream, launches);
+        return d128 ? launch_flash_loop<128>(a, loop_ctas, stream, launches)
+                    : launch_flash_loop<64>(a, loop_ctas, stream, launches);
     static const InlineReqs none{};  // never read by the slab variants
     return d128 ? launch_flash<128, false>(none, a, plan.dec_items, stream, launches)
                 : launch_flash<64, false>(none, a, plan.dec_items, stream, launches);

@@ -90,6 +90,10 @@ struct Tc5Schedule {
 // Static schedule of the prefill items of a call over n_cta persistent CTAs (sa_tc5_schedule.cu).
 void tc5_schedule(const std::vector<ReqMeta> &pre, int G, int Hkv, int n_cta, Tc5Schedule *out);
 
+struct PlanCache;  // last attention plan of a pool (sa_attention.cu)
+PlanCache *plan_cache_new();
+void plan_cache_delete(PlanCache *pc);
+
 struct Session {
     bool open = false;
     int64_t len = 0;
@@ -131,6 +135,7 @@ struct sa_kv_pool {
     std::vector<sa::Session> sessions;
     int32_t last_launches = 0;
     int32_t num_sms = 148;
+    sa::PlanCache *plan_cache = nullptr;  // owned; the one piece of state the const planning calls update
 
     // tcgen05 prefill kernel: TMA descriptors over the K and V page arrays (filled at create)
     alignas(64) unsigned char tmap_k[128];
@@ -228,7 +233,7 @@ struct AttnPlan {
 cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev, const ReqMeta *reqs_host,
                                 const AttnPlan &plan, const void *q, void *out, float *lse, float sm_scale,
                                 float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches,
-                                int persist_ctas = 0, const int32_t *dyn = nullptr);
+                                int loop_ctas = 0, const int32_t *dyn = nullptr);
 // dense operators of the layer (sa_gemm_tc5.cu); each returns an SA_* status
 int32_t gemm_plain(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
                    void *splitk_ws, size_t splitk_bytes, cudaStream_t stream, int32_t *launches);

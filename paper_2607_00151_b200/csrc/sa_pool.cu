@@ -99,6 +99,11 @@ extern "C" int32_t sa_kv_pool_create(const sa_kv_pool_config *cfg, void *dev_sto
     sa_kv_pool *pool = new (std::nothrow) sa_kv_pool();
     if (!pool) return SA_ERR_INVALID_ARG;
     pool->cfg = *cfg;
+    pool->plan_cache = sa::plan_cache_new();
+    if (!pool->plan_cache) {
+        delete pool;
+        return SA_ERR_INVALID_ARG;
+    }
     pool->G = cfg->num_q_heads / cfg->num_kv_heads;
     pool->log2_page = cfg->page_size == 16 ? 4 : 6;
     pool->max_pages_per_session = cv.mpps;
@@ -175,6 +180,7 @@ extern "C" int32_t sa_kv_pool_destroy(sa_kv_pool *pool) {
         }
         if (pool->big_host) cudaFreeHost(pool->big_host);
     }
+    sa::plan_cache_delete(pool->plan_cache);
     delete pool;
     return SA_OK;
 }

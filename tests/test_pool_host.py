@@ -335,3 +335,25 @@ def test_latency_table_workspace_is_sized_on_a_host_only_twin():
         sa.sa_latency_table_workspace_bytes(p, [0], [64], 1024, 512, 2048, 3)   # more scratch sessions than the pool has
     assert e.value.status == sa.SA_ERR_OUT_OF_SESSIONS
     assert sa.sa_kv_pool_free_pages(p) == 4096
+
+
+def test_cached_plan_is_dropped_when_the_batch_or_a_session_changes():
+    """The planner keeps the plan of the last batch (sa_mixed_attention_workspace_bytes followed by sa_mixed_attention
+    plans once); a different batch, or the same batch after a session grew or shrank, must be planned afresh."""
+    p = _pool(num_pages=512, max_tokens=4096)
+    a, b = sa.sa_kv_session_open(p), sa.sa_kv_session_open(p)
+    sa.sa_rope_kv_append(p, [a, b], [0, 1500, 1800], None, None)
+    s1 = sa.sa_mixed_attention_plan(p, [a, b], [0, 1, 301])          # a: decode row over 1500, b: 300-token chunk over 300
+    assert s1 == sa.sa_mixed_attention_plan(p, [a, b], [0, 1, 301])  # the cached plan answers the same
+    ws1 = sa.sa_mixed_attention_workspace_bytes(p, [a, b], [0, 1, 301])
+    assert s1["sum_decode_kv"] == 1500 and s1["sum_prefill_A"] == 300 * 301 // 2
+    sa.sa_rope_kv_append(p, [a], [0, 700], None, None)               # a grows past another 1024-key split
+    s2 = sa.sa_mixed_attention_plan(p, [a, b], [0, 1, 301])
+    assert s2["sum_decode_kv"] == 2200 and s2["decode_ctas"] == 3 * 2 and s1["decode_ctas"] == 2 * 2       # decode CTAs = Hkv x splits
+    assert sa.sa_mixed_attention_workspace_bytes(p, [a, b], [0, 1, 301]) > ws1
+    s3 = sa.sa_mixed_attention_plan(p, [b, a], [0, 300, 301])        # same sessions, other order
+    assert s3["sum_decode_kv"] == 2200 and s3["sum_prefill_A"] == s1["sum_prefill_A"]
+    s4 = sa.sa_mixed_attention_plan(p, [a, b], [0, 1, 201])          # same sessions, other chunk length
+    assert s4["sum_prefill_A"] == 200 * 100 + 200 * 201 // 2
+    sa.sa_kv_session_truncate(p, a, 1500)
+    assert sa.sa_mixed_attention_plan(p, [a, b], [0, 1, 301]) == s1
