@@ -320,16 +320,24 @@ __device__ __forceinline__ int tile_index(const GemmArgs &a, int mt, int nt) {
     return g * M_GROUP * a.n_tiles + nt * gm + (mt - g * M_GROUP);
 }
 
-// sum over the k slices, in slice order, of four consecutive accumulator columns of one row
+// sum over the k slices, in slice order, of four consecutive accumulator columns of one row; the loads of eight
+// slices go out together (one load per loop trip made the sum a chain of L2 round trips: 7 us for nine slices)
 __device__ __forceinline__ float4 splitk_sum4(const GemmArgs &a, int t, int row_in_tile, int col) {
     const float4 *p = reinterpret_cast<const float4 *>(a.partial + size_t(t) * a.k_splits * kPartialFloats + size_t(row_in_tile) * GBN + col);
     float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int sl = 0; sl < a.k_splits; ++sl) {
-        const float4 v = p[size_t(sl) * (kPartialFloats / 4)];
-        s.x += v.x;
-        s.y += v.y;
-        s.z += v.z;
-        s.w += v.w;
+    for (int s0 = 0; s0 < a.k_splits; s0 += 8) {
+        float4 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            v[u] = s0 + u < a.k_splits ? p[size_t(s0 + u) * (kPartialFloats / 4)] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (s0 + u < a.k_splits) {
+                s.x += v[u].x;
+                s.y += v[u].y;
+                s.z += v[u].z;
+                s.w += v[u].w;
+            }
     }
     return s;
 }
