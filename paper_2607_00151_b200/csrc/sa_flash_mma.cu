@@ -2,16 +2,19 @@
 // decode-like rows (q_len * G <= 16), split-KV, HBM-bound.  One CTA per (request, kv head, 1024-key
 // split); the G query heads of the group are the N columns of the MMA (keys are its M rows: S^T = K Q^T,
 // O^T += V^T P^T) so K/V are read once per group and no tensor work is spent on padding rows;
-// 4 warps take 16 keys each of every 64-key tile; cp.async 3-stage ring of page-gathered tiles;
+// 4 warps take 16 keys each of every 64-key tile; 3-stage ring of page-gathered tiles filled by TMA (one thread
+// issues the page boxes of a tile, an mbarrier per stage counts the bytes);
 // deterministic merge of the splits by the last of them to finish ("a single query token that attends to its full
 // KV cache of length L_j ... memory-bandwidth bound").  Prefill chunks run on the tcgen05 kernel
 // (sa_prefill_tc5.cu) for every supported head_dim.
 // Packed rows: row rho of a (request, kv head g) pair is (token rho / G, q head g*G + rho % G).
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <math.h>
 #include <string.h>
 
 #include "sa_internal.h"
+#include "sa_tc5_ptx.cuh"
 
 namespace sa {
 
@@ -22,17 +25,7 @@ constexpr int kBN = 64;      // keys per tile
 constexpr int kStages = 3;   // cp.async ring depth (64 KiB of K/V in flight per CTA)
 constexpr int kMaxSplitPages = kDecodeSplitKeys / 16;  // pages a split can span at the smallest page size
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) {
-    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src, int src_bytes) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
-}
+using ptx::smem_u32;
 __device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
@@ -51,71 +44,75 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
     return *reinterpret_cast<uint32_t *>(&p);
 }
-// byte offset of 16-byte chunk `chunk` of row `row` in a [rows][D] bf16 tile, XOR-swizzled
-template <int D>
+// Byte offset of 16-byte chunk `chunk` of row `row` in a [ROWS][D] bf16 tile held as D/64 halves of [ROWS][128 B] in
+// the 128-byte swizzle (chunk ^ row % 8 inside a 128-byte row): what a TMA box of 64 dims x ROWS slots with
+// SWIZZLE_128B writes, and conflict-free for ldmatrix.
+template <int ROWS>
 __device__ __forceinline__ uint32_t tile_off(int row, int chunk) {
-    return uint32_t(row * (D * 2) + ((chunk ^ (row & 7)) << 4));
+    return uint32_t((chunk >> 3) * (ROWS * 128) + row * 128 + (((chunk & 7) ^ (row & 7)) << 4));
 }
 
 constexpr int kLoopReqCache = 128;  // requests a captured step keeps in shared memory (4 KiB)
-// shared memory of one 128-thread group: the K/V ring, the Q tile, the page ids of the split
+// shared memory of the 128 threads of an item: the K/V ring, the Q tile, the page ids of the split, a flag, the ring's mbarriers
 template <int D>
 constexpr size_t group_smem() {
-    return size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2 + kMaxSplitPages * 4 + 16;
+    return size_t(kStages) * 2 * kBN * D * 2 + size_t(16) * D * 2 + kMaxSplitPages * 4 + 16 + 32;
 }
+constexpr size_t kSmemAlign = 1024;  // TMA destinations in the 128-byte swizzle want 1024-byte aligned tiles
 
 struct KvView {
-    const __nv_bfloat16 *k_base, *v_base;
+    const CUtensorMap *tmap_k, *tmap_v;  // 4-D maps over the pool's pages: (64 dims, page slots, 1 head, 1 page) boxes
     const int32_t *pages;   // shared memory: the page ids of the item's split, pages[0] = page of key k_begin
     int32_t page0;          // k_begin >> log2_page
-    int64_t stride_page;
-    int64_t head_off;  // g * stride_head
+    int32_t n_pages;        // pages of the split that hold session data
+    int32_t g;              // kv head
     int32_t log2_page;
 };
 
-// Gather one 64-key tile of K and V (logical keys kt .. kt+63, kt a multiple of 64 and < kv_len) into
-// swizzled smem; rows at or beyond kv_len are zero-filled (src-size 0: nothing is read), so slots the
-// session does not own never reach the math.  The page ids come from shared memory (decode_item reads the split's
-// slice of the block table once, before the ring starts): a block-table read from global memory in front of every
-// tile's copies stalled the issuing warp for an L2 or DRAM round trip per tile, in program order before the tile's
-// arithmetic -- with one warp per scheduler nothing hid it, and a lone CTA took 0.64 us per tile.
+// One 64-key tile of K and V (logical keys kt .. kt+63, kt a multiple of 64) into a ring stage, by TMA: one elected
+// thread issues D/64 boxes per page and operand and the stage's mbarrier counts the bytes.  (Until r2 every thread
+// issued sixteen 16-byte cp.async per tile behind its own address arithmetic: ~100 of the ~400 instructions a warp
+// spent per tile, in a kernel whose lone warp per scheduler is bound by its instruction stream.)  Only pages the
+// session owns are requested; what the rest of the stage holds is dealt with by the caller (zero_v_tail).
 template <int D>
-__device__ __forceinline__ void load_kv_tile(const KvView &kv, int kt, int kv_len, uint32_t sK, uint32_t sV, int tid) {
-    constexpr int CPR = D / 8;               // 16-byte chunks per row
-    constexpr int RPP = kThreads / CPR;      // rows per pass
-    constexpr int NP = kBN / RPP;            // passes
-    const int chunk = tid % CPR;
-    const int r0 = tid / CPR;
-    const int last = kv_len - 1;
+__device__ __forceinline__ void issue_kv_tile(const KvView &kv, int kt, uint32_t sK, uint32_t sV, uint32_t bar) {
+    constexpr int DH = D / 64;
+    constexpr uint32_t HALF = kBN * 128;
     if (kv.log2_page >= 6) {
-        const int32_t page = kv.pages[(kt >> kv.log2_page) - kv.page0];
-        const int slot0 = (kt & ((1 << kv.log2_page) - 1)) + r0;
-        const int64_t base = int64_t(page) * kv.stride_page + kv.head_off + int64_t(slot0) * D + chunk * 8;
-        const __nv_bfloat16 *kp = kv.k_base + base, *vp = kv.v_base + base;
+        const int32_t pg = kv.pages[(kt >> kv.log2_page) - kv.page0];
+        ptx::mbar_expect_tx(bar, 2 * DH * HALF);
 #pragma unroll
-        for (int i = 0; i < NP; ++i) {
-            const int row = r0 + i * RPP;
-            const int nb = (kt + row <= last) ? 16 : 0;
-            const uint32_t so = tile_off<D>(row, chunk);
-            cp_async16(sK + so, kp + i * (RPP * D), nb);
-            cp_async16(sV + so, vp + i * (RPP * D), nb);
+        for (int h = 0; h < DH; ++h) {
+            ptx::tma_load_4d(sK + h * HALF, kv.tmap_k, bar, h * 64, 0, kv.g, pg);
+            ptx::tma_load_4d(sV + h * HALF, kv.tmap_v, bar, h * 64, 0, kv.g, pg);
         }
         return;
     }
-    const int pmask = (1 << kv.log2_page) - 1;
-    int32_t page[NP];
+    const int p0 = (kt >> kv.log2_page) - kv.page0;
+    const int np = min(kBN >> kv.log2_page, kv.n_pages - p0);
+    const uint32_t page_bytes = 128u << kv.log2_page;  // one page, one 64-dim half
+    ptx::mbar_expect_tx(bar, uint32_t(np) * 2 * DH * page_bytes);
+    for (int u = 0; u < np; ++u) {
+        const int32_t pg = kv.pages[p0 + u];
 #pragma unroll
-    for (int i = 0; i < NP; ++i) page[i] = kv.pages[(min(kt + r0 + i * RPP, last) >> kv.log2_page) - kv.page0];
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
-        const int row = r0 + i * RPP;
-        const int key = kt + row;
-        const int64_t off = int64_t(page[i]) * kv.stride_page + kv.head_off + int64_t(min(key, last) & pmask) * D + chunk * 8;
-        const uint32_t so = tile_off<D>(row, chunk);
-        const int nb = key <= last ? 16 : 0;
-        cp_async16(sK + so, kv.k_base + off, nb);
-        cp_async16(sV + so, kv.v_base + off, nb);
+        for (int h = 0; h < DH; ++h) {
+            ptx::tma_load_4d(sK + h * HALF + u * page_bytes, kv.tmap_k, bar, h * 64, 0, kv.g, pg);
+            ptx::tma_load_4d(sV + h * HALF + u * page_bytes, kv.tmap_v, bar, h * 64, 0, kv.g, pg);
+        }
     }
+}
+
+// Rows [valid, 64) of a V stage hold no session data (slots past the end of the session, pages never requested):
+// they must be exactly zero, because P is 0 there and 0 * NaN = NaN.  (K rows past the end only produce scores that
+// the mask replaces.)  Generic-proxy stores into a buffer the async proxy writes next: fenced.
+template <int D>
+__device__ __forceinline__ void zero_v_tail(uint32_t sV, int valid, int tid) {
+    constexpr int CPR = D / 8;
+    for (int e = valid * CPR + tid; e < kBN * CPR; e += kThreads) {
+        const int row = e / CPR, chunk = e % CPR;
+        asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(sV + tile_off<kBN>(row, chunk)), "r"(0) : "memory");
+    }
+    ptx::fence_proxy_async_smem();
 }
 
 // barrier over the 128 threads that run an item (id 0 with 128 threads is __syncthreads of a 128-thread CTA)
@@ -151,7 +148,7 @@ __device__ __forceinline__ void warp_step(const uint32_t (&qf)[D / 16][4], uint3
 #pragma unroll
     for (int ks = 0; ks < D / 16; ++ks) {
         uint32_t ka[4];  // A = K: keys x dims, row-major as stored
-        ldsm_x4(ka, sK + tile_off<D>(key_off + (mi & 1) * 8 + rr, ks * 2 + (mi >> 1)));
+        ldsm_x4(ka, sK + tile_off<kBN>(key_off + (mi & 1) * 8 + rr, ks * 2 + (mi >> 1)));
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) mma16816(s[nt], ka, qf[ks][2 * nt], qf[ks][2 * nt + 1]);
     }
@@ -208,7 +205,7 @@ __device__ __forceinline__ void warp_step(const uint32_t (&qf)[D / 16][4], uint3
 #pragma unroll
     for (int np = 0; np < D / 16; ++np) {
         uint32_t va[4];  // A = V^T: dims x keys, i.e. the stored [key][dim] tile read through the transposing ldmatrix
-        ldsm_x4_t(va, sV + tile_off<D>(key_off + (mi >> 1) * 8 + rr, np * 2 + (mi & 1)));
+        ldsm_x4_t(va, sV + tile_off<kBN>(key_off + (mi >> 1) * 8 + rr, np * 2 + (mi & 1)));
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) mma16816(w.o[np][nt], va, pb[nt][0], pb[nt][1]);
     }
@@ -218,14 +215,14 @@ __device__ __forceinline__ void warp_step(const uint32_t (&qf)[D / 16][4], uint3
 template <int D, int NT>
 __device__ __forceinline__ void decode_tiles(const KvView &kv, const ReqMeta &r, int log2G, int n_rows, int k_begin, int k_end,
                                              int n_tiles, float scale_log2, uint32_t s_base, uint32_t sQ, unsigned char *smem,
-                                             int tid, int bar_id) {
+                                             uint32_t bars, uint32_t &phase, int tid, int bar_id) {
     constexpr int TILE_BYTES = kBN * D * 2;
     const int lane = tid & 31, warp = tid >> 5;
     uint32_t qf[D / 16][4];  // B = Q^T: [ks][2*nt], [2*nt+1] = dims ks*16 + {0..7, 8..15} of rows nt*8 + lane/4
     {
         const int mi = lane >> 3, rr = lane & 7;
 #pragma unroll
-        for (int ks = 0; ks < D / 16; ++ks) ldsm_x4(qf[ks], sQ + tile_off<D>((mi >> 1) * 8 + rr, ks * 2 + (mi & 1)));
+        for (int ks = 0; ks < D / 16; ++ks) ldsm_x4(qf[ks], sQ + tile_off<16>((mi >> 1) * 8 + rr, ks * 2 + (mi & 1)));
     }
     // causal limits (inclusive last key) of this thread's rows; rows beyond n_rows are padding whose results are
     // never read (Q is zero there, so they stay finite): no limit, so that they never force a mask
@@ -252,27 +249,30 @@ __device__ __forceinline__ void decode_tiles(const KvView &kv, const ReqMeta &r,
     }
 
     for (int t = 0; t < n_tiles; ++t) {
-        cp_async_wait<kStages - 2>();
-        group_sync(bar_id);
+        const int st = t % kStages;
+        ptx::mbar_wait(bars + 8 * st, (phase >> st) & 1u);  // tile t has landed (acquire: its bytes are visible)
+        phase ^= 1u << st;
+        group_sync(bar_id);                                 // ... and everyone is done with tile t - 1: its stage is free
         {
             const int tn = t + kStages - 1;
-            if (tn < n_tiles) {
+            if (tid == 0 && tn < n_tiles) {
                 const int sn = tn % kStages;
-                load_kv_tile<D>(kv, k_begin + tn * kBN, r.kv_len, s_base + sn * 2 * TILE_BYTES,
-                                s_base + sn * 2 * TILE_BYTES + TILE_BYTES, tid);
+                issue_kv_tile<D>(kv, k_begin + tn * kBN, s_base + sn * 2 * TILE_BYTES, s_base + sn * 2 * TILE_BYTES + TILE_BYTES,
+                                 bars + 8 * sn);
             }
-            cp_async_commit();
         }
-        const int st = t % kStages;
         const uint32_t sK = s_base + st * 2 * TILE_BYTES, sV = sK + TILE_BYTES;
         const int kt = k_begin + t * kBN;
+        if (k_end - kt < kBN) {  // the session ends inside this tile (uniform over the item; its last tile only)
+            zero_v_tail<D>(sV, k_end - kt, tid);
+            group_sync(bar_id);
+        }
         const int key_off = warp * 16;
         if (kt + key_off < k_end) {  // warp-uniform: this warp's 16 keys hold at least one live key
             const bool need_mask = kt + key_off + 15 > lim_min;
             warp_step<D, NT>(qf, sK, sV, key_off, kt, lim, need_mask, scale_log2, w, lane);
         }
     }
-    cp_async_wait<0>();
 #pragma unroll
     for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
@@ -324,10 +324,9 @@ struct AttnArgs {
     float *lse;
     float *part_o;
     float *part_lse;
-    const __nv_bfloat16 *k_base, *v_base;
     const int32_t *block_table;
     int32_t *tickets;  // [requests of the call][Hkv] arrival counters, zero on entry and on exit
-    int64_t mpps, stride_page, stride_head;
+    int64_t mpps;
     int32_t log2_page, Hq, Hkv, log2G;
     float scale_log2;
     // Captured launches (sa_decode_step): the grids are fixed and the actual counts are read on the device,
@@ -349,7 +348,7 @@ __device__ __forceinline__ void load_q_tile(const AttnArgs &a, const ReqMeta &r,
             const int tok = rho >> a.log2G, hq = (g << a.log2G) + (rho & ((1 << a.log2G) - 1));
             val = *reinterpret_cast<const uint4 *>(a.q + (int64_t(r.q_start + tok) * a.Hq + hq) * D + chunk * 8);
         }
-        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(sQ + tile_off<D>(row, chunk)), "r"(val.x),
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(sQ + tile_off<BM>(row, chunk)), "r"(val.x),
                      "r"(val.y), "r"(val.z), "r"(val.w) : "memory");
     }
 }
@@ -427,7 +426,8 @@ __device__ __forceinline__ void merge_rows(const AttnArgs &a, const ReqMeta &r, 
 // shared memory.  The arithmetic (and so every bit of the result) depends on the item alone: which kernel, CTA or
 // group runs it does not matter.
 template <int D>
-__device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *reqs, int n_reqs, int item, unsigned char *smem,
+__device__ __forceinline__ void decode_item(const AttnArgs &a, const CUtensorMap *tmap_k, const CUtensorMap *tmap_v,
+                                            const ReqMeta *reqs, int n_reqs, int item, unsigned char *smem, uint32_t &phase,
                                             int tid, int bar_id) {
     constexpr int BM = 16;
     constexpr int TILE_BYTES = kBN * D * 2;
@@ -435,6 +435,7 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
     const uint32_t s_base = smem_u32(smem);
     const uint32_t sQ = s_base + kStages * 2 * TILE_BYTES;
     int32_t *s_pages = reinterpret_cast<int32_t *>(smem + kStages * 2 * TILE_BYTES + BM * D * 2);  // [kMaxSplitPages]
+    const uint32_t bars = smem_u32(s_pages + kMaxSplitPages + 4);  // [kStages] mbarriers of the ring (after the flag)
 
     const int ri = find_req(reqs, n_reqs, item);
     const ReqMeta r = reqs[ri];
@@ -446,34 +447,30 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
     const int k_begin = split * kDecodeSplitKeys;
     const int k_end = min(r.kv_len, k_begin + kDecodeSplitKeys);
     KvView kv;
-    kv.k_base = a.k_base;
-    kv.v_base = a.v_base;
+    kv.tmap_k = tmap_k;
+    kv.tmap_v = tmap_v;
     kv.pages = s_pages;
     kv.page0 = k_begin >> a.log2_page;
-    kv.stride_page = a.stride_page;
-    kv.head_off = int64_t(g) * a.stride_head;
+    kv.n_pages = ((k_end - 1) >> a.log2_page) - kv.page0 + 1;
+    kv.g = g;
     kv.log2_page = a.log2_page;
 
     const int n_tiles = (k_end - k_begin + kBN - 1) / kBN;
-    {   // the split's slice of the block table (<= 64 entries) and Q: one global round trip, then the ring starts
-        const int n_pages = ((k_end - 1) >> a.log2_page) - kv.page0 + 1;
-        if (tid < n_pages) s_pages[tid] = __ldg(a.block_table + int64_t(r.sid) * a.mpps + kv.page0 + tid);
-    }
+    // the split's slice of the block table (<= 64 entries) and Q: one global round trip, then the ring starts
+    if (tid < kv.n_pages) s_pages[tid] = __ldg(a.block_table + int64_t(r.sid) * a.mpps + kv.page0 + tid);
     load_q_tile<D, BM>(a, r, g, rho0, n_rows, sQ, tid);
     group_sync(bar_id);
-    // prologue of the cp.async ring
+    if (tid == 0) {  // prologue of the ring
 #pragma unroll
-    for (int s = 0; s < kStages - 1; ++s) {
-        if (s < n_tiles)
-            load_kv_tile<D>(kv, k_begin + s * kBN, r.kv_len, s_base + s * 2 * TILE_BYTES,
-                            s_base + s * 2 * TILE_BYTES + TILE_BYTES, tid);
-        cp_async_commit();
+        for (int s = 0; s < kStages - 1; ++s)
+            if (s < n_tiles)
+                issue_kv_tile<D>(kv, k_begin + s * kBN, s_base + s * 2 * TILE_BYTES, s_base + s * 2 * TILE_BYTES + TILE_BYTES, bars + 8 * s);
     }
     // rows as MMA columns: one n8 tile when the group's rows fit (every decode batch with G <= 8), else two
     if (n_rows <= 8)
-        decode_tiles<D, 1>(kv, r, a.log2G, n_rows, k_begin, k_end, n_tiles, a.scale_log2, s_base, sQ, smem, tid, bar_id);
+        decode_tiles<D, 1>(kv, r, a.log2G, n_rows, k_begin, k_end, n_tiles, a.scale_log2, s_base, sQ, smem, bars, phase, tid, bar_id);
     else
-        decode_tiles<D, 2>(kv, r, a.log2G, n_rows, k_begin, k_end, n_tiles, a.scale_log2, s_base, sQ, smem, tid, bar_id);
+        decode_tiles<D, 2>(kv, r, a.log2G, n_rows, k_begin, k_end, n_tiles, a.scale_log2, s_base, sQ, smem, bars, phase, tid, bar_id);
     float *sO = reinterpret_cast<float *>(smem);             // [4][16][D]
     float *sM = sO + 4 * 16 * D;                             // [4][16]
     float *sL = sM + 4 * 16;                                 // [4][16]
@@ -522,18 +519,43 @@ __device__ __forceinline__ void decode_item(const AttnArgs &a, const ReqMeta *re
 
 // grid = decode CTAs of the call (one item each).  INLINE: the requests of a small decode-only call ride in the kernel
 // parameters (no metadata upload launch).
+// The 1024-byte aligned start of the dynamic shared memory, with the ring's mbarriers initialised (count 1: the
+// issuing thread's arrive.expect_tx) by the time every thread returns.
+template <int D>
+__device__ __forceinline__ unsigned char *ring_setup(unsigned char *smem_raw, const CUtensorMap *tmap_k, const CUtensorMap *tmap_v) {
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + kSmemAlign - 1) & ~uintptr_t(kSmemAlign - 1));
+    if (threadIdx.x == 0) {
+        const uint32_t bars = smem_u32(smem + group_smem<D>() - 32);
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) ptx::mbar_init(bars + 8 * s, 1);
+        ptx::fence_mbar_init();
+        ptx::prefetch_tmap(tmap_k);
+        ptx::prefetch_tmap(tmap_v);
+    }
+    __syncthreads();
+    return smem;
+}
+
+// grid = decode CTAs of the call (one item each).  INLINE: the requests of a small decode-only call ride in the kernel
+// parameters (no metadata upload launch).
 template <int D, bool INLINE>
-__global__ void __launch_bounds__(kThreads) flash_mma_kernel(const __grid_constant__ InlineReqs ir, const AttnArgs a) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    decode_item<D>(a, INLINE ? ir.reqs : a.reqs, a.n_reqs, blockIdx.x, smem, threadIdx.x, 0);
+__global__ void __launch_bounds__(kThreads)
+flash_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
+                 const __grid_constant__ InlineReqs ir, const AttnArgs a) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = ring_setup<D>(smem_raw, &tmap_k, &tmap_v);
+    uint32_t phase = 0;
+    decode_item<D>(a, &tmap_k, &tmap_v, INLINE ? ir.reqs : a.reqs, a.n_reqs, blockIdx.x, smem, phase, threadIdx.x, 0);
 }
 
 // Captured decode step (sa_decode_step_enqueue): the launch is recorded once and replayed on batches whose size and
 // lengths change, so the grid is fixed and the counts are read on the device (dyn = {requests, items} in the step's
 // metadata); the CTAs stride over the items.  Which CTA runs an item does not enter its arithmetic.
 template <int D>
-__global__ void __launch_bounds__(kThreads, 3) flash_mma_loop_kernel(const AttnArgs a) {
-    extern __shared__ __align__(128) unsigned char smem[];
+__global__ void __launch_bounds__(kThreads, 3)
+flash_mma_loop_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v, const AttnArgs a) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = ring_setup<D>(smem_raw, &tmap_k, &tmap_v);
     // programmatic dependent launch: this grid is staged while the step's append kernel runs and waits here for its
     // results (the metadata twin, the new token in the cache, the rotated q)
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -546,9 +568,13 @@ __global__ void __launch_bounds__(kThreads, 3) flash_mma_loop_kernel(const AttnA
             reinterpret_cast<uint4 *>(s_reqs)[i] = reinterpret_cast<const uint4 *>(a.reqs)[i];
     const int n_reqs = a.dyn[0], n_items = a.dyn[1];
     __syncthreads();
+    uint32_t phase = 0;  // parity each ring stage's mbarrier completes with next; carried from item to item
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        decode_item<D>(a, cached ? s_reqs : a.reqs, n_reqs, item, smem, threadIdx.x, 0);
-        group_sync(0);  // the merge scratch and the page list of this item live where the next item's ring goes
+        decode_item<D>(a, &tmap_k, &tmap_v, cached ? s_reqs : a.reqs, n_reqs, item, smem, phase, threadIdx.x, 0);
+        // the merge scratch, the page list and the zeroed V rows of this item live where the next item's ring goes:
+        // generic-proxy stores before the async proxy's
+        ptx::fence_proxy_async_smem();
+        group_sync(0);
     }
 }
 
@@ -562,13 +588,9 @@ AttnArgs make_args(const sa_kv_pool *pool, const ReqMeta *reqs, int32_t n, const
     a.lse = lse;
     a.part_o = part_o;
     a.part_lse = part_lse;
-    a.k_base = static_cast<const __nv_bfloat16 *>(pool->k_base);
-    a.v_base = static_cast<const __nv_bfloat16 *>(pool->v_base);
     a.block_table = pool->block_table;
     a.tickets = pool->tickets;
     a.mpps = pool->max_pages_per_session;
-    a.stride_page = pool->stride_page;
-    a.stride_head = pool->stride_head;
     a.log2_page = pool->log2_page;
     a.Hq = pool->cfg.num_q_heads;
     a.Hkv = pool->cfg.num_kv_heads;
@@ -595,12 +617,15 @@ cudaError_t opt_in_smem(size_t smem) {
 
 
 template <int D, bool INLINE>
-cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, cudaStream_t stream, int32_t *launches) {
-    constexpr size_t smem = group_smem<D>();
-    static_assert(smem >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
+cudaError_t launch_flash(const sa_kv_pool *pool, const InlineReqs &ir, const AttnArgs &a, int items, cudaStream_t stream,
+                         int32_t *launches) {
+    constexpr size_t smem = group_smem<D>() + kSmemAlign;
+    const CUtensorMap &tk = *reinterpret_cast<const CUtensorMap *>(pool->tmap_k);
+    const CUtensorMap &tv = *reinterpret_cast<const CUtensorMap *>(pool->tmap_v);
+    static_assert(size_t(kStages) * 2 * kBN * D * 2 >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
     cudaError_t e = opt_in_smem<&flash_mma_kernel<D, INLINE>>(smem);
     if (e != cudaSuccess) return e;
-    flash_mma_kernel<D, INLINE><<<unsigned(items), kThreads, smem, stream>>>(ir, a);
+    flash_mma_kernel<D, INLINE><<<unsigned(items), kThreads, smem, stream>>>(tk, tv, ir, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     ++*launches;
@@ -608,8 +633,10 @@ cudaError_t launch_flash(const InlineReqs &ir, const AttnArgs &a, int items, cud
 }
 
 template <int D>
-cudaError_t launch_flash_loop(const AttnArgs &a, int n_cta, cudaStream_t stream, int32_t *launches) {
-    constexpr size_t smem = group_smem<D>() + kLoopReqCache * sizeof(ReqMeta);
+cudaError_t launch_flash_loop(const sa_kv_pool *pool, const AttnArgs &a, int n_cta, cudaStream_t stream, int32_t *launches) {
+    constexpr size_t smem = group_smem<D>() + kLoopReqCache * sizeof(ReqMeta) + kSmemAlign;
+    const CUtensorMap &tk = *reinterpret_cast<const CUtensorMap *>(pool->tmap_k);
+    const CUtensorMap &tv = *reinterpret_cast<const CUtensorMap *>(pool->tmap_v);
     cudaError_t e = opt_in_smem<&flash_mma_loop_kernel<D>>(smem);
     if (e != cudaSuccess) return e;
     {
@@ -623,7 +650,7 @@ cudaError_t launch_flash_loop(const AttnArgs &a, int n_cta, cudaStream_t stream,
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        e = cudaLaunchKernelEx(&cfg, flash_mma_loop_kernel<D>, a);
+        e = cudaLaunchKernelEx(&cfg, flash_mma_loop_kernel<D>, tk, tv, a);
     }
     if (e != cudaSuccess) return e;
     ++*launches;
@@ -633,8 +660,9 @@ cudaError_t launch_flash_loop(const AttnArgs &a, int n_cta, cudaStream_t stream,
 }  // namespace
 
 cudaError_t flash_loop_prepare(const sa_kv_pool *pool) {
-    return pool->cfg.head_dim == 128 ? opt_in_smem<&flash_mma_loop_kernel<128>>(group_smem<128>() + kLoopReqCache * sizeof(ReqMeta))
-                                     : opt_in_smem<&flash_mma_loop_kernel<64>>(group_smem<64>() + kLoopReqCache * sizeof(ReqMeta));
+    return pool->cfg.head_dim == 128
+               ? opt_in_smem<&flash_mma_loop_kernel<128>>(group_smem<128>() + kLoopReqCache * sizeof(ReqMeta) + kSmemAlign)
+               : opt_in_smem<&flash_mma_loop_kernel<64>>(group_smem<64>() + kLoopReqCache * sizeof(ReqMeta) + kSmemAlign);
 }
 
 // reqs_host != nullptr (and plan.n_dec <= kInlineReqs): the requests go in the kernel parameters, reqs_dev is unused.
@@ -645,21 +673,22 @@ cudaError_t launch_flash_decode(const sa_kv_pool *pool, const ReqMeta *reqs_dev,
                                 float *part_o, float *part_lse, cudaStream_t stream, int32_t *launches,
                                 int loop_ctas, const int32_t *dyn) {
     if (plan.dec_items == 0 && !dyn) return cudaSuccess;
+    if (!pool->tc5_ready) return cudaErrorNotSupported;  // the TMA descriptors over the pages are built with the pool
     AttnArgs a = make_args(pool, reqs_dev, plan.n_dec, q, out, lse, sm_scale, part_o, part_lse);
     a.dyn = dyn;
     const bool d128 = pool->cfg.head_dim == 128;
     if (reqs_host) {
         InlineReqs ir;
         memcpy(ir.reqs, reqs_host, sizeof(ReqMeta) * size_t(plan.n_dec));
-        return d128 ? launch_flash<128, true>(ir, a, plan.dec_items, stream, launches)
-                    : launch_flash<64, true>(ir, a, plan.dec_items, stream, launches);
+        return d128 ? launch_flash<128, true>(pool, ir, a, plan.dec_items, stream, launches)
+                    : launch_flash<64, true>(pool, ir, a, plan.dec_items, stream, launches);
     }
     if (dyn)
-        return d128 ? launch_flash_loop<128>(a, loop_ctas, stream, launches)
-                    : launch_flash_loop<64>(a, loop_ctas, stream, launches);
+        return d128 ? launch_flash_loop<128>(pool, a, loop_ctas, stream, launches)
+                    : launch_flash_loop<64>(pool, a, loop_ctas, stream, launches);
     static const InlineReqs none{};  // never read by the slab variants
-    return d128 ? launch_flash<128, false>(none, a, plan.dec_items, stream, launches)
-                : launch_flash<64, false>(none, a, plan.dec_items, stream, launches);
+    return d128 ? launch_flash<128, false>(pool, none, a, plan.dec_items, stream, launches)
+                : launch_flash<64, false>(pool, none, a, plan.dec_items, stream, launches);
 }
 
 }  // namespace sa
