@@ -182,6 +182,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b0,
                 const __grid_constant__ CUtensorMap tmap_b1, const GemmArgs a) {
     extern __shared__ unsigned char smem_raw[];
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the next kernel of the stream may be staged behind this one
     unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t s0 = smem_u32(smem);
     __shared__ uint64_t bars[2 * GSTAGES + 4];
@@ -226,24 +227,36 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
             prefetch_tmap(&tmap_a);
             prefetch_tmap(&tmap_b0);
             prefetch_tmap(&tmap_b1);
-            int kc = 0;
-            for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-                int t, k0, k1, mt, nt;
-                k_range(u, t, k0, k1);
-                tile_coords(a, t, mt, nt);
-                const int m0 = mt * GBM;
-                const int r0 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN;        // rows of W (b0)
-                const int r1 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN + 128;  // rows of the second half (b1)
-                for (int ks = k0; ks < k1; ++ks, ++kc) {
-                    const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
-                    mbar_wait(bar_empty(s), ph ^ 1);
-                    const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
-                    mbar_expect_tx(bar_full(s), STAGE_BYTES);
-                    tma_load_2d(sA, &tmap_a, bar_full(s), ks * GBK, m0);
-                    tma_load_2d(sB, &tmap_b0, bar_full(s), ks * GBK, r0);
-                    tma_load_2d(sB + B_HALF, &tmap_b1, bar_full(s), ks * GBK, r1);
+            // Programmatic dependent launch: this grid may be staged while the kernel before it in the stream still runs.
+            // The weights (B) depend on nothing, so the B halves of the first GSTAGES stages are requested at once;
+            // the activations (A) are what the previous kernel wrote: they wait for it.
+            auto walk = [&](int phase) {  // 0: B of the first GSTAGES k-steps; 1: their A, then every later k-step whole
+                int kc = 0;
+                for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+                    int t, k0, k1, mt, nt;
+                    k_range(u, t, k0, k1);
+                    tile_coords(a, t, mt, nt);
+                    const int m0 = mt * GBM;
+                    const int r0 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN;        // rows of W (b0)
+                    const int r1 = EPI == EPI_SWIGLU ? nt * 128 : nt * GBN + 128;  // rows of the second half (b1)
+                    for (int ks = k0; ks < k1; ++ks, ++kc) {
+                        const bool early = kc < GSTAGES;
+                        if (phase == 0 && !early) return;
+                        const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
+                        const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
+                        if (!early) mbar_wait(bar_empty(s), ph ^ 1);
+                        if (phase == 0 || !early) {
+                            mbar_expect_tx(bar_full(s), STAGE_BYTES);
+                            tma_load_2d(sB, &tmap_b0, bar_full(s), ks * GBK, r0);
+                            tma_load_2d(sB + B_HALF, &tmap_b1, bar_full(s), ks * GBK, r1);
+                        }
+                        if (phase == 1) tma_load_2d(sA, &tmap_a, bar_full(s), ks * GBK, m0);
+                    }
                 }
-            }
+            };
+            walk(0);
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+            walk(1);
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
@@ -273,6 +286,7 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
         }
     } else if (warp >= 4) {
         // =========================== epilogue ===========================
+        asm volatile("griddepcontrol.wait;" ::: "memory");  // everything these warps read and write belongs to the stream's order
         const int q4 = warp & 3;                 // TMEM lane quarter this warp may read
         const int row_in_tile = q4 * 32 + lane;
         const uint32_t lane_addr = uint32_t(q4 * 32) << 16;
@@ -349,6 +363,8 @@ __device__ __forceinline__ uint2 pack4(float a, float b, float c, float d) { ret
 // fixed, so the bits do not depend on which CTA ran which slice.
 template <int EPI>
 __global__ void __launch_bounds__(256) gemm_splitk_reduce_kernel(const GemmArgs a, int64_t n_items, int32_t items_per_row) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (e >= n_items) return;
     const int64_t row = e / items_per_row;
@@ -430,34 +446,55 @@ qkv_token_table_kernel(const ReqMeta *__restrict__ reqs, int32_t n_req, int64_t 
     if (t0 + tl < total_rows) cs[(t0 + tl) * 64 + m] = rope_cos_sin(s_pos[tl], rope_tab[m]);
 }
 
-// RMSNorm (reading R22): one warp per row, fp32, the row is read twice (the second pass hits L1).
+// RMSNorm (reading R22): one CTA per row, fp32; the row is read once (up to 8192 columns stay in registers: every
+// load of a thread is in flight at the same time; a row per warp with a 16-trip load loop made the kernel a chain of
+// sixteen memory round trips, 10 us for 64 rows) and the eight warps' sums of squares are combined in a fixed order.
 __global__ void __launch_bounds__(256)
 rmsnorm_kernel(const __nv_bfloat16 *__restrict__ x, const __nv_bfloat16 *__restrict__ w, float eps,
                __nv_bfloat16 *__restrict__ y, int64_t M, int32_t H) {
-    const int64_t row = int64_t(blockIdx.x) * 8 + (threadIdx.x >> 5);
-    if (row >= M) return;
-    const int lane = threadIdx.x & 31;
-    const uint4 *xr = reinterpret_cast<const uint4 *>(x + row * H);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    __shared__ float s_part[8];
+    const int64_t row = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint4 *wr = reinterpret_cast<const uint4 *>(w);
-    uint4 *yr = reinterpret_cast<uint4 *>(y + row * H);
     const int nv = H / 8;
-    float ss = 0.f;
-    for (int i = lane; i < nv; i += 32) {
-        const uint4 u = xr[i];
-        const uint32_t v[4] = {u.x, u.y, u.z, u.w};
+    constexpr int R = 4;  // 16-byte vectors a thread keeps (R * 256 * 8 = 8192 columns)
+    uint4 g[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if (tid + i * 256 < nv) g[i] = __ldg(wr + tid + i * 256);  // the weight depends on no earlier kernel
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const uint4 *xr = reinterpret_cast<const uint4 *>(x + row * H);
+    uint4 *yr = reinterpret_cast<uint4 *>(y + row * H);
+    uint4 u[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if (tid + i * 256 < nv) u[i] = xr[tid + i * 256];
+    auto sq = [](const uint4 &q, float ss) {
+        const uint32_t v[4] = {q.x, q.y, q.z, q.w};
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const float a0 = __uint_as_float(v[j] << 16), a1 = __uint_as_float(v[j] & 0xffff0000u);
             ss = fmaf(a0, a0, ss);
             ss = fmaf(a1, a1, ss);
         }
-    }
+        return ss;
+    };
+    float ss = 0.f;
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if (tid + i * 256 < nv) ss = sq(u[i], ss);
+    for (int i = tid + R * 256; i < nv; i += 256) ss = sq(xr[i], ss);  // rows longer than 8192 columns
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-    const float inv = rsqrtf(ss / float(H) + eps);
-    for (int i = lane; i < nv; i += 32) {
-        const uint4 u = xr[i], g = wr[i];
-        const uint32_t v[4] = {u.x, u.y, u.z, u.w}, gw[4] = {g.x, g.y, g.z, g.w};
+    if (lane == 0) s_part[warp] = ss;
+    __syncthreads();
+    float tot = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tot += s_part[i];
+    const float inv = rsqrtf(tot / float(H) + eps);
+    auto scale = [inv](const uint4 &q, const uint4 &gq) {
+        const uint32_t v[4] = {q.x, q.y, q.z, q.w}, gw[4] = {gq.x, gq.y, gq.z, gq.w};
         uint32_t o[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -465,8 +502,12 @@ rmsnorm_kernel(const __nv_bfloat16 *__restrict__ x, const __nv_bfloat16 *__restr
             const float a1 = __uint_as_float(v[j] & 0xffff0000u) * inv * __uint_as_float(gw[j] & 0xffff0000u);
             o[j] = pack_bf16x2(a0, a1);
         }
-        yr[i] = make_uint4(o[0], o[1], o[2], o[3]);
-    }
+        return make_uint4(o[0], o[1], o[2], o[3]);
+    };
+#pragma unroll
+    for (int i = 0; i < R; ++i)
+        if (tid + i * 256 < nv) yr[tid + i * 256] = scale(u[i], g[i]);
+    for (int i = tid + R * 256; i < nv; i += 256) yr[i] = scale(xr[i], wr[i]);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -528,16 +569,16 @@ cudaError_t launch_gemm(const CUtensorMap &ta, const CUtensorMap &tb0, const CUt
     if (ks > 1 && (!splitk_ws || splitk_bytes < need)) ks = 1;  // no scratch: the unsplit kernel is always correct
     a.k_splits = ks;
     a.partial = ks > 1 ? reinterpret_cast<float *>(w) : nullptr;
-    gemm_tc5_kernel<EPI><<<unsigned(std::min(tiles * ks, sms)), kGemmThreads, kSmemGemm, stream>>>(ta, tb0, tb1, a);
+    cudaError_t e = launch_pdl(gemm_tc5_kernel<EPI>, dim3(unsigned(std::min(tiles * ks, sms))), dim3(kGemmThreads), kSmemGemm, stream,
+                               ta, tb0, tb1, a);
     if (launches) ++*launches;
-    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || ks == 1) return e;
     // items of four output columns per row: PLAIN N/4 (N is a multiple of 8), SWIGLU F/4, QKV 16 per head
     const int32_t per_row = EPI == EPI_QKV ? (a.Hq + 2 * a.Hkv) * 16 : a.N / 4;
     const int64_t n_items = a.M * per_row;
-    gemm_splitk_reduce_kernel<EPI><<<unsigned((n_items + 255) / 256), 256, 0, stream>>>(a, n_items, per_row);
+    e = launch_pdl(gemm_splitk_reduce_kernel<EPI>, dim3(unsigned((n_items + 255) / 256)), dim3(256), 0, stream, a, n_items, per_row);
     if (launches) ++*launches;
-    return cudaGetLastError();
+    return e;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
@@ -602,10 +643,9 @@ int32_t rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int
     if (H % 8 != 0) return SA_ERR_UNSUPPORTED;
     if (M == 0) return SA_OK;
     if (!x || !w || !y || !aligned16(x) || !aligned16(w) || !aligned16(y)) return SA_ERR_INVALID_ARG;
-    rmsnorm_kernel<<<unsigned((M + 7) / 8), 256, 0, stream>>>(static_cast<const __nv_bfloat16 *>(x),
-                                                              static_cast<const __nv_bfloat16 *>(w), eps,
-                                                              static_cast<__nv_bfloat16 *>(y), M, H);
-    return cudaGetLastError() == cudaSuccess ? SA_OK : SA_ERR_CUDA;
+    const cudaError_t e = launch_pdl(rmsnorm_kernel, dim3(unsigned(M)), dim3(256), 0, stream, static_cast<const __nv_bfloat16 *>(x),
+                                     static_cast<const __nv_bfloat16 *>(w), eps, static_cast<__nv_bfloat16 *>(y), M, H);
+    return e == cudaSuccess ? SA_OK : SA_ERR_CUDA;
 }
 
 static size_t qkv_tables_bytes(int64_t total) {

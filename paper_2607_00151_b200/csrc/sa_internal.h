@@ -190,6 +190,24 @@ int32_t acquire_big_meta(sa_kv_pool *pool, size_t bytes, char **host);
 int32_t commit_big_meta(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream);
 
 #ifdef __CUDACC__
+// Launch with programmatic stream serialization: the grid may be staged (and run whatever precedes its
+// griddepcontrol.wait) while the kernel before it in the stream is still running.  Every kernel launched this way
+// executes griddepcontrol.wait before it reads or writes anything that is ordered by the stream.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // (cos, sin) of pos * theta_m from the pool's table u = (hi, lo) of theta_m / (2 pi) (reading R9):
 // the position is an exact fp32 integer (< 2^24), the product pos * u is formed error-free, whole
 // turns are dropped and sincospif evaluates the fraction.
