@@ -693,6 +693,16 @@ def measure_layer(local: int, peaks, iters: int = 10):
            "launches_per_step": launches, "note": "whole decoder layer per chunk (7 operators), L2 flushed between steps"}
     r.close()
     sa.sa_kv_pool_destroy(pool)
+    # T_GEMM(M) of PAPER.md L299-303 (the dense operators of the layer alone) at decode sizes, where it is the larger part
+    # of a decode iteration; the floor is every weight once at the HBM copy peak
+    try:
+        m_list = [1, 16, 64, 128]
+        t = sa.sa_gemm_table(H, F, L.num_q_heads, L.num_kv_heads, L.head_dim, m_list, warmup=3, iters=15)
+        w_bytes = 2.0 * ((L.num_q_heads + 2 * L.num_kv_heads) * L.head_dim * H + H * L.num_q_heads * L.head_dim + 3 * F * H)
+        out["t_gemm_ms"] = {str(m): round(float(x), 4) for m, x in zip(m_list, t)}
+        out["t_gemm_floor_ms"] = round(w_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3, 4)
+    except Exception as e:   # noqa: BLE001 - a side measurement
+        out["t_gemm_ms"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:120])}
     return out
 
 
@@ -775,7 +785,7 @@ def run_ours(args, world, rank, local):
         achieved = flops_step * args.steps / (attn_ms * 1e-3) / 1e12
         peak = peaks["bf16_tflops"]
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": load_traffic().get("prefill_tc5_kernel_cfg2_avg_per_launch_est") if args.config == 2 else None, "peak_source": peaks["source"] + " (burst; sustained %.1f)" % peaks["bf16_tflops_sustained"],
+                "traffic": load_traffic().get("prefill_tc5_kernel_cfg2_avg_per_launch") if args.config == 2 else None, "peak_source": peaks["source"] + " (burst; sustained %.1f)" % peaks["bf16_tflops_sustained"],
                 "kernel": "prefill attention inside sa_mixed_attention (%d calls timed, avg %.3f ms; decode rows of the same "
                           "call included in the time when the workload has them)" % (n_attn, attn_ms / max(n_attn, 1)),
                 "algorithmic_flops_per_step": flops_step}
@@ -892,7 +902,8 @@ def run_ours(args, world, rank, local):
         layer = measure_layer(local, peaks)
         detail["layer"] = layer
         torch.cuda.empty_cache()
-        summary = {"layer_cfg2": {"tflops": round(layer["achieved"], 1), "frac": round(layer["frac"], 4), "ms": round(layer["ms_per_step"], 3)},
+        summary = {"layer_cfg2": {"tflops": round(layer["achieved"], 1), "frac": round(layer["frac"], 4), "ms": round(layer["ms_per_step"], 3),
+                                  "t_gemm_ms": layer.get("t_gemm_ms"), "t_gemm_floor_ms": layer.get("t_gemm_floor_ms")},
                    "transfer_cfg4": {"export_gbs": round(xfer["export_gbs"], 1), "import_gbs": round(xfer["import_gbs"], 1), "frac": round(xfer["frac"], 4)}}
         if not args.no_other_configs:
             other = measure_other_configs(local, peaks)
@@ -945,6 +956,7 @@ def main():
     ap.add_argument("--parts-only", action="store_true", help="only the decode / append measurements (for profiling them)")
     ap.add_argument("--layer-only", action="store_true", help="only the whole-layer measurement (for profiling the GEMMs)")
     ap.add_argument("--decode-step-only", action="store_true", help="only the captured decode iteration at small batch")
+    ap.add_argument("--gemm-table-only", action="store_true", help="only T_GEMM(M) of the layer's dense operators at decode sizes")
     args = ap.parse_args()
     if args.layer_only:
         import __graft_entry__
@@ -960,6 +972,15 @@ def main():
         import __graft_entry__
         __graft_entry__.build()
         print(json.dumps({"other_configs": measure_other_configs(0, load_peaks())}))
+        return
+    if args.gemm_table_only:
+        import __graft_entry__
+        __graft_entry__.build()
+        from paper_2607_00151_b200 import binding as sa
+        Lr = get_workload(2).layer
+        m_list = [1, 16, 64, 128]
+        t = sa.sa_gemm_table(4096, 14336, Lr.num_q_heads, Lr.num_kv_heads, Lr.head_dim, m_list, warmup=3, iters=15)
+        print(json.dumps({"t_gemm_ms": {str(m): round(float(x), 4) for m, x in zip(m_list, t)}}))
         return
     if args.decode_step_only:
         import __graft_entry__
