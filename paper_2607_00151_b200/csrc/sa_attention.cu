@@ -314,7 +314,7 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
 
     // Latency-critical rows first (Alg. 2 lines 3-6: decode requests are admitted before any prefill
     // chunk because they are the latency-critical class): the decode rows' outputs are complete after the HBM-bound
-    // decode + merge kernels, before the best-effort lookahead chunks' tensor-bound kernel has started.  The two
+    // decode kernel (whose last splits merge), before the best-effort lookahead chunks' tensor-bound kernel has started.  The two
     // classes write disjoint rows and disjoint workspace regions, so the order does not change any bit.
     cudaError_t e;
     e = launch_flash_decode(pool, dec_dev, nullptr, hp.plan, q, out, lse, sm_scale, part_o, part_lse, stream, &pool->last_launches);

@@ -22,7 +22,7 @@ namespace {
 
 constexpr int kThreads = 128;
 constexpr int kBN = 64;      // keys per tile
-constexpr int kStages = 3;   // cp.async ring depth (64 KiB of K/V in flight per CTA)
+constexpr int kStages = 3;   // depth of the TMA-filled K/V ring (64 KiB in flight per item)
 constexpr int kMaxSplitPages = kDecodeSplitKeys / 16;  // pages a split can span at the smallest page size
 
 using ptx::smem_u32;
@@ -70,9 +70,9 @@ struct KvView {
 };
 
 // One 64-key tile of K and V (logical keys kt .. kt+63, kt a multiple of 64) into a ring stage, by TMA: one elected
-// thread issues D/64 boxes per page and operand and the stage's mbarrier counts the bytes.  (Until r2 every thread
-// issued sixteen 16-byte cp.async per tile behind its own address arithmetic: ~100 of the ~400 instructions a warp
-// spent per tile, in a kernel whose lone warp per scheduler is bound by its instruction stream.)  Only pages the
+// thread issues D/64 boxes per page and operand and the stage's mbarrier counts the bytes.  (Until round 2 every
+// thread issued sixteen 16-byte cp.async per tile behind its own address arithmetic, ~100 of the ~400 instructions a warp
+// spent per tile; with this and the transposed MMAs the kernel executes 38 % fewer instructions for the same time.)  Only pages the
 // session owns are requested; what the rest of the stage holds is dealt with by the caller (zero_v_tail).
 template <int D>
 __device__ __forceinline__ void issue_kv_tile(const KvView &kv, int kt, uint32_t sK, uint32_t sV, uint32_t bar) {
@@ -127,8 +127,10 @@ __device__ __forceinline__ uint32_t movmatrix_t(uint32_t x) {  // transpose of a
 // Running state of a warp for its NT * 8 query rows.  Everything is held TRANSPOSED: the 16 keys of a step are the M
 // rows of the MMA and the query rows its N columns, S^T = K Q^T and O^T += V^T P^T.  A decode batch has G (<= 8) live
 // rows per kv head, so one n8 column tile carries them and a step costs D/16 + D/16 HMMAs instead of twice that with
-// the rows as M (16 rows, most of them padding) -- on sm_100a the warp-level HMMA pipe retires one m16n8k16 per ~30
-// cycles per scheduler, which, not HBM, bounded a lone warp (d = 1) and co-limited the full-batch stream at G = 4.
+// the rows as M (16 rows, most of them padding); on sm_100a the warp-level HMMA pipe retires one m16n8k16 per ~30 cycles
+// per scheduler, and with the rows as M it was busy for two thirds of a lone item's time.  (Measured: the pipe's
+// active time halved, issue slots 32 -> 19 % busy on a full batch; the time of a call is set elsewhere -- HBM on a
+// full batch, fixed costs at one row -- and did not move.)
 // A thread holds query rows qa = nt*8 + 2*(lane%4) and qa + 1 (C-fragment columns); keys / dims run over lane/4.
 template <int D, int NT>
 struct WarpState {
