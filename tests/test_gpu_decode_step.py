@@ -107,3 +107,66 @@ def test_decode_step_graph_replay_equals_eager_calls_bitwise(shape):
         torch.cuda.synchronize()
         assert torch.equal(_bits(ie), _bits(is_)), "session %d: stored K'/V differ" % i
     assert sa.sa_kv_pool_free_pages(eager) == sa.sa_kv_pool_free_pages(stepped)
+
+
+def test_decode_step_at_config4_scale_equals_the_eager_call_bitwise():
+    """64 decode rows on 8 K - 32 K contexts (BASELINE.json config 4's decode set, lengths from the same seed): the
+    captured step strides 2368 CTAs over ~11 000 items where the eager call launches one CTA per item; every output
+    bit and lse must agree, over two replays, and sampled rows must meet the oracle."""
+    Hq, Hkv, D, page, base = 32, 8, 128, 64, 500000.0
+    rng = np.random.default_rng(4)
+    lens = [int(x) for x in rng.integers(8192, 32768, size=64)]
+    n = len(lens)
+    pages = sum(L // page + 2 for L in lens) + 8
+    eager, stepped, cfg = _twin_pools(Hq, Hkv, D, page, pages, n + 1, 32768 + 64, base, 9)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(4321)
+    rnd = lambda t, h: (torch.randn((t, h, D), generator=gen, device="cuda") * D ** -0.5).to(torch.bfloat16)
+    src_k, src_v = rnd(32768, Hkv), rnd(32768, Hkv)
+    sids_e = [sa.sa_kv_session_open(eager) for _ in range(n)]
+    sids_s = [sa.sa_kv_session_open(stepped) for _ in range(n)]
+    offs = [int(x) for x in rng.integers(0, 32768 - max(lens), size=n)] if max(lens) < 32768 else [0] * n
+    for i, L in enumerate(lens):   # every session a different window of the source
+        for pool, sids in ((eager, sids_e), (stepped, sids_s)):
+            sa.sa_rope_kv_append(pool, [sids[i]], [0, L], src_k[offs[i]:offs[i] + L], src_v[offs[i]:offs[i] + L], None)
+    step = sa.sa_decode_step_create(stepped, n, 32768 + 64)
+    k_in, v_in, q_in = rnd(n, Hkv), rnd(n, Hkv), rnd(n, Hq)
+    out = torch.empty((n, Hq, D), dtype=torch.bfloat16, device="cuda")
+    lse = torch.empty((n, Hq), dtype=torch.float32, device="cuda")
+    ip = np.arange(n + 1, dtype=np.int32)
+    graph = None
+    for it in range(2):
+        k1, v1, q1 = rnd(n, Hkv), rnd(n, Hkv), rnd(n, Hq)
+        qe = q1.clone()
+        sa.sa_rope_kv_append(eager, sids_e, ip, k1, v1, qe)
+        oe, le = torch.empty_like(qe), torch.empty((n, Hq), dtype=torch.float32, device="cuda")
+        ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(eager, sids_e, ip), 256), dtype=torch.uint8, device="cuda")
+        sa.sa_mixed_attention(eager, sids_e, ip, qe, oe, le, 0.0, ws)
+        torch.cuda.synchronize()
+        sa.sa_decode_step_prepare(step, sids_s)
+        k_in.copy_(k1), v_in.copy_(v1), q_in.copy_(q1)
+        if graph is None:
+            sa.sa_decode_step_enqueue(step, k_in, v_in, q_in, out, lse)
+            torch.cuda.synchronize()
+            assert torch.equal(_bits(out), _bits(oe)) and torch.equal(lse, le)
+            q_in.copy_(q1)
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                sa.sa_decode_step_enqueue(step, k_in, v_in, q_in, out, lse)
+        out.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        st = sa.sa_decode_step_stats(step)
+        assert st["items"] == sum(Hkv * ((L + it + 1 + 1023) // 1024) for L in lens) and st["grid_ctas"] == 16 * torch.cuda.get_device_properties(0).multi_processor_count
+        assert torch.equal(_bits(out), _bits(oe)), "replay %d differs from the eager call" % it
+        assert torch.equal(lse, le)
+        if it == 1:
+            for i in (0, 17, 63):   # the oracle on three rows of the last iteration
+                L = lens[i] + 2
+                kk = torch.cat([src_k[offs[i]:offs[i] + lens[i]], kprev[i:i + 1], k1[i:i + 1]]).cpu()
+                vv = torch.cat([src_v[offs[i]:offs[i] + lens[i]], vprev[i:i + 1], v1[i:i + 1]]).cpu()
+                kr = orc.rope(kk[:L - 1], np.arange(L - 1), base)
+                ref = orc.oracle_cached(kr, orc.widen(vv[:L - 1]), q1[i:i + 1].cpu(), kk[L - 1:], vv[L - 1:], L - 1, base)
+                # BASELINE.json's distribution (values N(0,1)/sqrt(128)): its own gates apply (derived terms are far below)
+                check_derived(out[i:i + 1], lse[i:i + 1], ref, 128 ** -0.5, 128 ** -0.5, "cfg4-scale step row %d" % i)
+        kprev, vprev = k1, v1
