@@ -359,7 +359,13 @@ SA_API int32_t sa_dynamic_chunk(const sa_latency_model *model, const int64_t *de
  * accumulation is fp32 on the tensor cores (tcgen05, TMEM accumulators), every stored tensor is
  * rounded once to bf16 (round to nearest even).  All calls enqueue on `stream`, never allocate and
  * never synchronise (sa_gemm_table excepted).  Shape limits of the tcgen05 GEMM: in_features a
- * multiple of 64, out_features a multiple of 8, every pointer 16-byte aligned, M >= 0 arbitrary. */
+ * multiple of 64, out_features a multiple of 8, every pointer 16-byte aligned, M >= 0 arbitrary.
+ * Stream order: activations, residuals, outputs and workspaces are read and written in stream order.  WEIGHTS (w,
+ * w_gate, w_up, w_qkv, the norm weights) are read AHEAD of it: the kernels are launched with programmatic stream
+ * serialization and request their first weight tiles while the kernel before them in the stream may still be running
+ * (they wait for it only before touching anything else).  A weight tensor must therefore not be written by work that
+ * can still be in flight on the stream when the call is enqueued -- weights loaded once at start-up, the normal case,
+ * are fine; a kernel that rewrites a weight matrix right before the call needs a synchronisation (or an event) first. */
 
 /* y[M, N] = x[M, K] W[N, K]^T (+ residual[M, N] if non-null; y may alias residual). */
 SA_API int32_t sa_linear(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N,
