@@ -170,3 +170,50 @@ def test_decode_step_at_config4_scale_equals_the_eager_call_bitwise():
                 # BASELINE.json's distribution (values N(0,1)/sqrt(128)): its own gates apply (derived terms are far below)
                 check_derived(out[i:i + 1], lse[i:i + 1], ref, 128 ** -0.5, 128 ** -0.5, "cfg4-scale step row %d" % i)
         kprev, vprev = k1, v1
+
+
+def test_decode_step_errors_on_a_device_pool_change_nothing():
+    """Error behaviour of the pair on a device pool (include/smoothagent.h): enqueue before any prepare is refused; a
+    failed prepare leaves sessions, pages and the step's prepared batch as they were, and a replay after it still
+    recomputes the last prepared batch bit for bit."""
+    Hq, Hkv, D, page, base = 8, 2, 64, 16, 1e4
+    cfg = sa.PoolConfig(Hq, Hkv, D, page, 6, 3, 64, base, 0)
+    pool = sa.sa_kv_pool_create(cfg)
+    a, b = sa.sa_kv_session_open(pool), sa.sa_kv_session_open(pool)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    rnd = lambda t, h: torch.randn((t, h, D), generator=gen, device="cuda").to(torch.bfloat16)
+    sa.sa_rope_kv_append(pool, [a, b], [0, 32, 64], rnd(64, Hkv), rnd(64, Hkv), None)   # 2 + 2 pages, 2 left
+    step = sa.sa_decode_step_create(pool, 2, 40)
+    k, v, q = rnd(2, Hkv), rnd(2, Hkv), rnd(2, Hq)
+    out = torch.full((2, Hq, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    lse = torch.full((2, Hq), float("nan"), dtype=torch.float32, device="cuda")
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_decode_step_enqueue(step, k, v, q, out, lse)
+    assert e.value.status == sa.SA_ERR_INVALID_ARG
+    sa.sa_decode_step_prepare(step, [a, b])            # takes the two free pages
+    q0 = q.clone()
+    sa.sa_decode_step_enqueue(step, k, v, q, out, lse)
+    torch.cuda.synchronize()
+    first = out.clone(), lse.clone()
+    assert torch.isfinite(out.float()).all() and sa.sa_kv_pool_free_pages(pool) == 0
+    state = [sa.sa_kv_session_query(pool, s) for s in (a, b)], sa.sa_decode_step_stats(step)["items"]
+    c = sa.sa_kv_session_open(pool)
+    for bad, status in (([c], sa.SA_ERR_OUT_OF_PAGES), ([a, a], sa.SA_ERR_INVALID_ARG), ([a, b, c], sa.SA_ERR_INVALID_ARG)):
+        with pytest.raises(sa.SAError) as e:
+            sa.sa_decode_step_prepare(step, bad)
+        assert e.value.status == status
+        assert ([sa.sa_kv_session_query(pool, s) for s in (a, b)], sa.sa_decode_step_stats(step)["items"]) == state
+    # the step still holds its last prepared batch: enqueue again re-places the same tokens and recomputes the same rows
+    q.copy_(q0)
+    out.fill_(float("nan"))
+    sa.sa_decode_step_enqueue(step, k, v, q, out, lse)
+    torch.cuda.synchronize()
+    assert torch.equal(_bits(out), _bits(first[0])) and torch.equal(lse, first[1])
+    # a cache longer than the step was created for
+    for _ in range(7):
+        sa.sa_decode_step_prepare(step, [a])
+    assert sa.sa_kv_session_query(pool, a)[0] == 40
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_decode_step_prepare(step, [a])
+    assert e.value.status == sa.SA_ERR_INVALID_ARG and sa.sa_kv_session_query(pool, a)[0] == 40
