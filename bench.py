@@ -588,6 +588,41 @@ def measure_decode_step(local: int, peaks, batches=(1, 4, 16, 64), ctx: int = 21
     return out
 
 
+def measure_gemm_ops(local: int, M: int = 64, iters: int = 15):
+    """The layer's three plain GEMMs at a decode batch, one operator per event pair with the L2 evicted before it, ours
+    (sa_linear_ws: split-K + reduction) beside cuBLAS (torch.matmul) on the same tensors: context for T_GEMM(M), not a
+    path of the product.  Both sides carry the same ~5 us of event-pair overhead."""
+    from paper_2607_00151_b200 import binding as sa
+    dev = torch.device("cuda:%d" % local)
+    g = torch.Generator(device=dev)
+    g.manual_seed(64)
+    rnd = lambda *sh: (torch.randn(*sh, device=dev, generator=g, dtype=torch.float32) * 0.02).to(torch.bfloat16)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    st = torch.cuda.current_stream()
+
+    def timed(fn):
+        ts = []
+        for i in range(iters + 3):
+            flush.fill_(i & 1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            fn()
+            e1.record(st)
+            torch.cuda.synchronize()
+            if i >= 3:
+                ts.append(e0.elapsed_time(e1) * 1e3)
+        return round(float(np.median(ts)), 1)
+    out = {"M": M, "note": "us per call, L2 evicted before each, one call per event pair"}
+    for name, N, K in (("qkv_proj", 6144, 4096), ("o_proj", 4096, 4096), ("down_proj", 4096, 14336)):
+        x, w = rnd(M, K), rnd(N, K)
+        y = torch.empty((M, N), dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(max(sa.sa_linear_workspace_bytes(M, N, K), 256), dtype=torch.uint8, device=dev)
+        wt = w.t()
+        out[name] = {"ours_us": timed(lambda: sa.sa_linear_ws(x, w, y, ws, None)), "cublas_us": timed(lambda: torch.matmul(x, wt, out=y)),
+                     "weight_mb": round(N * K * 2 / 1e6, 1)}
+    return out
+
+
 def measure_latency_table(local: int, peaks):
     """BASELINE.json config 4's sweep: sa_latency_table over prefill tokens {0, 512, 1K, 2K, 4K} (as 2048-token
     chunks on a 20K-token prefix) x decode batch {1, 16, 64, 256} (contexts uniform in [8K, 32K]), and the
@@ -701,6 +736,7 @@ def measure_layer(local: int, peaks, iters: int = 10):
         w_bytes = 2.0 * ((L.num_q_heads + 2 * L.num_kv_heads) * L.head_dim * H + H * L.num_q_heads * L.head_dim + 3 * F * H)
         out["t_gemm_ms"] = {str(m): round(float(x), 4) for m, x in zip(m_list, t)}
         out["t_gemm_floor_ms"] = round(w_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3, 4)
+        out["gemm_operators_m64"] = measure_gemm_ops(local)
     except Exception as e:   # noqa: BLE001 - a side measurement
         out["t_gemm_ms"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:120])}
     return out
@@ -980,7 +1016,7 @@ def main():
         Lr = get_workload(2).layer
         m_list = [1, 16, 64, 128]
         t = sa.sa_gemm_table(4096, 14336, Lr.num_q_heads, Lr.num_kv_heads, Lr.head_dim, m_list, warmup=3, iters=15)
-        print(json.dumps({"t_gemm_ms": {str(m): round(float(x), 4) for m, x in zip(m_list, t)}}))
+        print(json.dumps({"t_gemm_ms": {str(m): round(float(x), 4) for m, x in zip(m_list, t)}, "operators": measure_gemm_ops(0)}))
         return
     if args.decode_step_only:
         import __graft_entry__
