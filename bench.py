@@ -912,6 +912,11 @@ def run_ours(args, world, rank, local):
         sa.sa_kv_pool_destroy(pool)
         del r, pool, flush
         torch.cuda.empty_cache()
+        # (the layer first: it is the other tensor-bound figure, and is measured before the HBM-bound parts and the 120 GB
+        # config have heated the box)
+        layer = measure_layer(local, peaks)
+        detail["layer"] = layer
+        torch.cuda.empty_cache()
         dec_roof, app_roof, mixed, xfer, host = measure_parts(local, peaks)
         detail.update({"roofline_decode": dec_roof, "roofline_append": app_roof, "mixed_config4": mixed, "transfer_config4": xfer,
                        "host_cost": host})
@@ -935,9 +940,6 @@ def run_ours(args, world, rank, local):
                 for d, r_ in ds["rows"].items()}
         except Exception as e:   # noqa: BLE001 - a side measurement never takes the line down
             detail["decode_step_graph"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
-        layer = measure_layer(local, peaks)
-        detail["layer"] = layer
-        torch.cuda.empty_cache()
         summary = {"layer_cfg2": {"tflops": round(layer["achieved"], 1), "frac": round(layer["frac"], 4), "ms": round(layer["ms_per_step"], 3),
                                   "t_gemm_ms": layer.get("t_gemm_ms"), "t_gemm_floor_ms": layer.get("t_gemm_floor_ms")},
                    "transfer_cfg4": {"export_gbs": round(xfer["export_gbs"], 1), "import_gbs": round(xfer["import_gbs"], 1), "frac": round(xfer["frac"], 4)}}

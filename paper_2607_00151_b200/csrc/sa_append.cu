@@ -130,6 +130,10 @@ rope_append_kernel(const __grid_constant__ InlineAppendMeta im, const ReqMeta *_
                    __nv_bfloat16 *__restrict__ v_base, int32_t *block_table, int64_t mpps,
                    int32_t log2_page, int64_t stride_page, int64_t stride_head,
                    const float2 *__restrict__ rope_tab, int32_t Hq, int32_t Hkv) {
+    // staged behind the kernel before it in the stream, and the next one behind it (programmatic dependent launch);
+    // everything it reads and writes is ordered by the stream, so it waits first
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const ReqMeta *reqs = INLINE ? im.reqs : reqs_slab;
     const int32_t n_req = INLINE ? im.n_req : n_req_slab;
     constexpr int HALF = D / 2;
@@ -225,20 +229,19 @@ static cudaError_t launch_rope_append_t(const sa_kv_pool *pool, const InlineAppe
     const unsigned grid = unsigned((total_rows + kAppendTok - 1) / kAppendTok);
     auto kb = static_cast<__nv_bfloat16 *>(pool->k_base);
     auto vb = static_cast<__nv_bfloat16 *>(pool->v_base);
+    cudaError_t e;
     if (pool->cfg.head_dim == 128)
-        rope_append_kernel<128, INLINE><<<grid, kAppendThreads, 0, stream>>>(
-            im, reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
-            static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
-            pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
-            pool->cfg.num_kv_heads);
+        e = launch_pdl(rope_append_kernel<128, INLINE>, dim3(grid), dim3(kAppendThreads), 0, stream, im, reqs_dev, n_req, total_rows,
+                       static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v), static_cast<__nv_bfloat16 *>(q), kb,
+                       vb, pool->block_table, pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head,
+                       static_cast<const float2 *>(pool->rope_tab), pool->cfg.num_q_heads, pool->cfg.num_kv_heads);
     else
-        rope_append_kernel<64, INLINE><<<grid, kAppendThreads, 0, stream>>>(
-            im, reqs_dev, n_req, total_rows, static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v),
-            static_cast<__nv_bfloat16 *>(q), kb, vb, pool->block_table, pool->max_pages_per_session,
-            pool->log2_page, pool->stride_page, pool->stride_head, pool->rope_tab, pool->cfg.num_q_heads,
-            pool->cfg.num_kv_heads);
+        e = launch_pdl(rope_append_kernel<64, INLINE>, dim3(grid), dim3(kAppendThreads), 0, stream, im, reqs_dev, n_req, total_rows,
+                       static_cast<const __nv_bfloat16 *>(k), static_cast<const __nv_bfloat16 *>(v), static_cast<__nv_bfloat16 *>(q), kb,
+                       vb, pool->block_table, pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head,
+                       static_cast<const float2 *>(pool->rope_tab), pool->cfg.num_q_heads, pool->cfg.num_kv_heads);
     ++*launches;
-    return cudaGetLastError();
+    return e;
 }
 
 cudaError_t launch_step_append(const sa_kv_pool *pool, const void *slab_host, void *slab_dev, int32_t cap, const void *k,

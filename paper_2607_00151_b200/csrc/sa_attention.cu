@@ -306,7 +306,8 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
             sched_dev = dst;
         }
     }
-    if (commit_meta(pool, slab_used, stream) != SA_OK) return SA_ERR_CUDA;
+    int meta_slot = 0;
+    if (commit_meta_deferred(pool, nullptr, slab_used, stream, &meta_slot) != SA_OK) return SA_ERR_CUDA;
     const ReqMeta *dec_dev = reinterpret_cast<const ReqMeta *>(md);
     const ReqMeta *pre_dev = reinterpret_cast<const ReqMeta *>(md + dec_bytes);
 
@@ -322,5 +323,5 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     e = launch_prefill_tc5(pool, pre_dev, hp.plan, hp.sched, sched_dev, tc5_partials, hp.total_q, q, out, lse, sm_scale,
                            stream, &pool->last_launches);
     if (e != cudaSuccess) return SA_ERR_CUDA;
-    return SA_OK;
+    return meta_mark(pool, meta_slot, stream);  // the pinned slab is free again when everything above has run
 }

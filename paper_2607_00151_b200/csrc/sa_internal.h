@@ -179,6 +179,10 @@ int32_t acquire_meta(sa_kv_pool *pool, char **host, char **dev);
 int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream);
 // Same slab, but the bytes go to `dev_dst` (a block-table row) instead of the slab's device twin.
 int32_t commit_meta_to(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream);
+// commit_meta without the event that frees the slab (dev_dst nullptr: the slab's device twin); the caller records it
+// with meta_mark once the kernels that read the metadata are enqueued
+int32_t commit_meta_deferred(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream, int *slot);
+int32_t meta_mark(sa_kv_pool *pool, int slot, cudaStream_t stream);
 // Page bookkeeping: a page returns to the free list when its last holder lets go of it.
 int32_t take_page(sa_kv_pool *pool);
 void release_page(sa_kv_pool *pool, int32_t page);

@@ -379,6 +379,10 @@ int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream) {
 // another stream (there is one H2D engine), and the attention kernel behind it -- measured: +0.5 ms per
 // 25 MB upload running beside the call.  Pinned memory is device-addressable under unified addressing.
 __global__ void __launch_bounds__(256) meta_upload_kernel(uint32_t *__restrict__ dst, const uint32_t *__restrict__ src, size_t words) {
+    // staged behind the kernel before it and in front of the one after it (programmatic dependent launch); it waits
+    // before it writes: the slab's device twin may still be read by the kernels of an earlier call
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < words; i += size_t(gridDim.x) * blockDim.x) dst[i] = src[i];
 }
 
@@ -386,18 +390,33 @@ static cudaError_t meta_upload(sa_kv_pool *pool, void *dev, const void *host, si
     const size_t words = (bytes + 3) / 4;  // every metadata record is a whole number of 32-bit words
     if (words == 0) return cudaSuccess;
     const unsigned blocks = unsigned(std::min<size_t>((words + 255) / 256, 128));
-    meta_upload_kernel<<<blocks, 256, 0, stream>>>(static_cast<uint32_t *>(dev), static_cast<const uint32_t *>(host), words);
+    const cudaError_t e = sa::launch_pdl(meta_upload_kernel, dim3(blocks), dim3(256), 0, stream, static_cast<uint32_t *>(dev),
+                                         static_cast<const uint32_t *>(host), words);
     ++pool->last_launches;
-    return cudaGetLastError();
+    return e;
 }
 
 int32_t commit_meta_to(sa_kv_pool *pool, void *dev, size_t bytes, cudaStream_t stream) {
-    int i = pool->meta_next;
+    int slot = 0;
+    const int32_t st = commit_meta_deferred(pool, dev, bytes, stream, &slot);
+    return st == SA_OK ? meta_mark(pool, slot, stream) : st;
+}
+
+// The same without the event that frees the pinned slab for reuse: the caller records it (meta_mark) after the kernels
+// that follow the upload -- an event record between two kernels would keep the second from being staged behind the first.
+int32_t commit_meta_deferred(sa_kv_pool *pool, void *dev, size_t bytes, cudaStream_t stream, int *slot) {
+    const int i = pool->meta_next;
     char *host = pool->meta_host + size_t(i) * pool->meta_slab_bytes;
+    if (!dev) dev = pool->meta_dev + size_t(i) * pool->meta_slab_bytes;
     if (meta_upload(pool, dev, host, bytes, stream) != cudaSuccess) return SA_ERR_CUDA;
-    if (cudaEventRecord(pool->meta_event[i], stream) != cudaSuccess) return SA_ERR_CUDA;
-    pool->meta_event_used[i] = true;
     pool->meta_next = (i + 1) % kMetaRing;
+    *slot = i;
+    return SA_OK;
+}
+
+int32_t meta_mark(sa_kv_pool *pool, int slot, cudaStream_t stream) {
+    if (cudaEventRecord(pool->meta_event[slot], stream) != cudaSuccess) return SA_ERR_CUDA;
+    pool->meta_event_used[slot] = true;
     return SA_OK;
 }
 

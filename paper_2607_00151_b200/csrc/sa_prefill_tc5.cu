@@ -166,10 +166,10 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     constexpr int PAGES_PER_TILE = BN / B;
     constexpr uint32_t PAGE_HALF_BYTES = B * 128;  // one page, one 64-wide half: B rows x 128 B
 
-    // ---- the parts of this persistent CTA (uniform over the CTA: an idle CTA leaves at once)
-    const int pb = a.cta_begin[blockIdx.x], pe = a.cta_begin[blockIdx.x + 1];
-    if (pb == pe) return;
-
+    // Programmatic dependent launch: the grid is staged while the kernel before it in the stream (the metadata upload,
+    // or the decode rows' kernel of a mixed call) still runs; barriers and TMEM are set up, then everything that the
+    // stream orders -- the schedule, the requests, K/V, Q -- waits for that kernel.  The merge kernel is staged behind.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t sQ = smem_u32(smem);                 // 2 tiles x 32 KiB
@@ -204,6 +204,14 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = tmem_base_smem;
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+
+    // ---- the parts of this persistent CTA (uniform over the CTA: an idle CTA gives its TMEM back and leaves)
+    const int pb = a.cta_begin[blockIdx.x], pe = a.cta_begin[blockIdx.x + 1];
+    if (pb == pe) {
+        if (warp == 2) tmem_dealloc<512>(tmem);
+        return;
+    }
 
     // Phase bookkeeping shared by all roles: kc counts the KV tiles this CTA has gone through (K/V
     // ring stage kc & 1, ring phase (kc >> 1) & 1; S/P barriers complete once per tile: phase
@@ -530,6 +538,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
 // the loads of up to four parts are issued together (the kernel is latency-bound otherwise).
 template <int DH>
 __global__ void __launch_bounds__(256) tc5_merge_kernel(const Tc5Args a) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");  // staged behind the prefill kernel: its partials must be complete
     constexpr int D = DH * 64;
     const Tc5Merge mg = a.merges[blockIdx.x];
     const ReqMeta r = a.reqs[mg.req];
@@ -680,22 +689,23 @@ cudaError_t launch_prefill_tc5(const sa_kv_pool *pool, const ReqMeta *reqs_dev, 
     a.scale_log2 = sm_scale * 1.4426950408889634f;
     const CUtensorMap &tk = *reinterpret_cast<const CUtensorMap *>(pool->tmap_k);
     const CUtensorMap &tv = *reinterpret_cast<const CUtensorMap *>(pool->tmap_v);
+    cudaError_t e;
+    const dim3 grid{unsigned(n_cta), 1, 1}, block{unsigned(kThreadsTc5), 1, 1};
     if (c.page_size == 64 && c.head_dim == 128)
-        prefill_tc5_kernel<6, 2><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        e = launch_pdl(prefill_tc5_kernel<6, 2>, grid, block, kSmemTc5, stream, tq, tk, tv, a);
     else if (c.page_size == 64)
-        prefill_tc5_kernel<6, 1><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        e = launch_pdl(prefill_tc5_kernel<6, 1>, grid, block, kSmemTc5, stream, tq, tk, tv, a);
     else if (c.head_dim == 128)
-        prefill_tc5_kernel<4, 2><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        e = launch_pdl(prefill_tc5_kernel<4, 2>, grid, block, kSmemTc5, stream, tq, tk, tv, a);
     else
-        prefill_tc5_kernel<4, 1><<<unsigned(n_cta), kThreadsTc5, kSmemTc5, stream>>>(tq, tk, tv, a);
+        e = launch_pdl(prefill_tc5_kernel<4, 1>, grid, block, kSmemTc5, stream, tq, tk, tv, a);
     ++*launches;
-    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (!sched.merges.empty()) {
-        if (c.head_dim == 128) tc5_merge_kernel<2><<<dim3(unsigned(sched.merges.size()), 32), 256, 0, stream>>>(a);
-        else tc5_merge_kernel<1><<<dim3(unsigned(sched.merges.size()), 32), 256, 0, stream>>>(a);
+        const dim3 mgrid(unsigned(sched.merges.size()), 32);
+        e = c.head_dim == 128 ? launch_pdl(tc5_merge_kernel<2>, mgrid, dim3(256), 0, stream, a)
+                              : launch_pdl(tc5_merge_kernel<1>, mgrid, dim3(256), 0, stream, a);
         ++*launches;
-        e = cudaGetLastError();
     }
     return e;
 }
