@@ -545,7 +545,11 @@ __global__ void __launch_bounds__(kThreads)
 flash_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
                  const __grid_constant__ InlineReqs ir, const AttnArgs a) {
     extern __shared__ unsigned char smem_raw[];
+    // programmatic dependent launch: staged behind the kernel before it (the append, the metadata upload), with the
+    // prefill kernel of a mixed call staged behind it; the ring is set up, then everything else waits for that kernel
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     unsigned char *smem = ring_setup<D>(smem_raw, &tmap_k, &tmap_v);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     uint32_t phase = 0;
     decode_item<D>(a, &tmap_k, &tmap_v, INLINE ? ir.reqs : a.reqs, a.n_reqs, blockIdx.x, smem, phase, threadIdx.x, 0);
 }
@@ -627,8 +631,7 @@ cudaError_t launch_flash(const sa_kv_pool *pool, const InlineReqs &ir, const Att
     static_assert(size_t(kStages) * 2 * kBN * D * 2 >= 4 * 16 * D * 4 + 2 * 4 * 16 * 4, "merge scratch must fit in the stage ring");
     cudaError_t e = opt_in_smem<&flash_mma_kernel<D, INLINE>>(smem);
     if (e != cudaSuccess) return e;
-    flash_mma_kernel<D, INLINE><<<unsigned(items), kThreads, smem, stream>>>(tk, tv, ir, a);
-    e = cudaGetLastError();
+    e = launch_pdl(flash_mma_kernel<D, INLINE>, dim3(unsigned(items)), dim3(kThreads), smem, stream, tk, tv, ir, a);
     if (e != cudaSuccess) return e;
     ++*launches;
     return e;
