@@ -223,7 +223,8 @@ SA_API int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n_req
  *       copy, q_inout rotated in place, block-table entry written), (2) split-KV attention of the rows, the actual
  *       counts read on the device, the last split of a row merging them.  Legal under CUDA stream capture; the captured graph is
  *       replayed after each prepare (same k / v / q_inout / out / lse addresses, new contents).  Calling it again
- *       without a new prepare re-places the same tokens and recomputes the same rows (idempotent).
+ *       without a new prepare re-places the same tokens and recomputes the same rows, provided q_inout holds the RAW
+ *       rows again (it is rotated in place each time the kernels run).
  * Results are bit-equal to sa_rope_kv_append + sa_mixed_attention on the same batch (same device code per row).
  *   max_requests   : capacity of a step (<= cfg.max_sessions); max_kv_tokens: longest cache a row may attend to
  *   dev_mem        : device, 256-byte aligned, >= sa_decode_step_device_bytes(...): metadata twin + split partials;
