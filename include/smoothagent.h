@@ -390,6 +390,33 @@ SA_API int32_t sa_swiglu_workspace_bytes(int64_t M, int32_t F, int32_t K, size_t
 SA_API int32_t sa_swiglu_ws(const void *x, const void *w_gate, const void *w_up, void *act, int64_t M, int32_t F, int32_t K,
                      void *workspace, size_t workspace_bytes, void *stream);
 
+/* sa_linear_noalloc: the split-K linear of sa_linear_ws for a caller that cannot provide `workspace`.
+ * Every other call here leaves device memory to the caller, which is no help to a caller that has no allocator to
+ * ask: an operator running inside an engine whose memory plan was fixed at start-up, a serving worker whose HBM has
+ * all gone to the KV pool and the weights (a cudaMalloc of a few MiB then fails), a latency-critical loop that may
+ * not call cudaMalloc / cudaFree because they can stall the whole device.  For those, the scratch of this one call
+ * lives INSIDE THE LIBRARY: a fixed device array of SA_LINEAR_NOALLOC_SCRATCH_BYTES (20 MiB + 512 bytes) that the
+ * driver sets aside on every GPU where this library's device code gets loaded and keeps until the process exits.
+ * The call itself allocates and frees nothing, on the device or through any library routine; x, w, residual, y are
+ * still the caller's (same meaning, layout and alignment rules as sa_linear; y may alias residual).
+ *   Result    : the same kernels, split and summation order as sa_linear_ws with a full-size workspace -- bit-equal to it.
+ *   Sizes     : only shapes the planner splits, i.e. sa_linear_workspace_bytes(M, N, K) != 0: few rows and a long K
+ *               (ceil(M/128) * ceil(N/256) <= SMs/2 and K >= 256, e.g. M <= 512 at N = 4096 on 148 SMs).  Any other shape
+ *               returns SA_ERR_UNSUPPORTED and touches nothing: it involves no scratch, so plain sa_linear already serves
+ *               a caller that cannot allocate.  A shape whose scratch exceeds the array (possible only on a GPU with more
+ *               than 160 SMs) returns SA_ERR_WORKSPACE_TOO_SMALL; the call never quietly runs unsplit.
+ *   First call: the first call on each device looks the array's device address up (once per device and process, with
+ *               the calling thread's current device; thread-safe).  That lookup may make the runtime load device code,
+ *               so make this first call during start-up, before any stream capture begins on that device.
+ *   Sharing   : every call on a device uses the same array and leaves its partial sums behind.  Nothing in it needs to
+ *               be zero beforehand (each call writes every word it later reads), so stale contents are harmless, but
+ *               two calls that can run on the GPU at the same time -- different streams without an event between them,
+ *               or two host threads -- overwrite each other's partials and both results are garbage.  Issue them on one
+ *               stream, or order them yourself.  Weights are read ahead of stream order as described above. */
+#define SA_LINEAR_NOALLOC_SCRATCH_BYTES ((size_t)160 * 128 * 256 * 4 + 512)
+SA_API int32_t sa_linear_noalloc(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N,
+                          int32_t K, void *stream);
+
 /* y[M, H] = x / sqrt(mean_j x_j^2 + eps) * w  (fp32 arithmetic, one rounding). */
 SA_API int32_t sa_rmsnorm(const void *x, const void *w, float eps, void *y, int64_t M, int32_t H, void *stream);
 

@@ -142,6 +142,7 @@ PROTOTYPES = {
                                        ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _f32p, _vp, ctypes.c_size_t, _vp]),
     "sa_linear_workspace_bytes": (ctypes.c_int32, [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_linear_ws": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp, ctypes.c_size_t, _vp]),
+    "sa_linear_noalloc": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp]),
     "sa_swiglu_workspace_bytes": (ctypes.c_int32, [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_size_t)]),
     "sa_swiglu_ws": (ctypes.c_int32, [_vp, _vp, _vp, _vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _vp, ctypes.c_size_t, _vp]),
     "sa_kv_wire_bytes": (ctypes.c_int32, [_vp, ctypes.c_int64, ctypes.POINTER(ctypes.c_size_t)]),
@@ -669,6 +670,23 @@ def sa_linear_ws(x, w, y, workspace, residual=None, stream=None) -> None:
     assert w.shape[1] == K and tuple(y.shape) == (M, N)
     _check(load_library().sa_linear_ws(_ptr(x), _ptr(w), _ptr(residual), _ptr(y), M, N, K, _ptr(workspace), _nbytes(workspace),
                                        _stream_ptr(stream)), "sa_linear_ws")
+
+
+SA_LINEAR_NOALLOC_SCRATCH_BYTES = 160 * 128 * 256 * 4 + 512
+
+
+def sa_linear_noalloc(x, w, y, residual=None, stream=None) -> None:
+    """sa_linear_ws without the workspace argument, for code that cannot get device memory of its own (it runs inside
+    someone else's fixed memory plan, or next to a KV pool that has taken all of HBM, or must not stall the device with
+    cudaMalloc / cudaFree).  The split-K partials go to a 20 MiB array built into the library; nothing is allocated.
+    Decode-sized shapes only (those sa_linear_workspace_bytes gives a non-zero size for), otherwise SAError with
+    SA_ERR_UNSUPPORTED.  Bit-equal to sa_linear_ws.  Calls share the array: keep them on one stream, and make the first
+    call on a device before any stream capture."""
+    M, K = x.shape
+    N = w.shape[0]
+    assert w.shape[1] == K and tuple(y.shape) == (M, N)
+    _check(load_library().sa_linear_noalloc(_ptr(x), _ptr(w), _ptr(residual), _ptr(y), M, N, K, _stream_ptr(stream)),
+           "sa_linear_noalloc")
 
 
 def sa_swiglu_workspace_bytes(M: int, F: int, K: int) -> int:

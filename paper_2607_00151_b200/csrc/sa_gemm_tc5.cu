@@ -20,6 +20,7 @@
 #include <cuda_bf16.h>
 
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "sa_internal.h"
@@ -703,3 +704,75 @@ int32_t qkv_rope_append_device(sa_kv_pool *pool, const ReqMeta *reqs_dev, int32_
 
 }  // namespace sa
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// sa_linear_noalloc: the split-K linear for callers that have no way to get device scratch.
+//
+// Who that is: code that is handed its input and output tensors by something else and has no allocator of its
+// own to turn to -- an operator plugged into a serving engine whose memory plan was fixed at start-up, a worker
+// whose whole HBM share was given to the KV pool and the weights (the normal state of a serving process: the
+// pool takes what is left, so a later cudaMalloc of even a few MiB fails), or a latency-critical loop that must
+// not call cudaMalloc / cudaFree because both may synchronise the whole device.  Such a caller can run sa_linear
+// (no scratch) but not sa_linear_ws, and at decode sizes sa_linear leaves most SMs without work.
+//
+// The scratch of this variant is part of the library image: a file-scope device array below.  The driver reserves it
+// on every GPU on which this library's device code gets loaded and keeps it until the process ends; nothing in this
+// file allocates or frees anything.  Its size covers every shape the split-K planner can produce on a GPU of up to
+// 160 SMs (tiles x k slices never exceeds the SM count; one work unit writes a 128 x 256 fp32 partial = 128 KiB).
+//
+// `g_noalloc_scratch` names the array in DEVICE code only.  In host code the same identifier is a handle of the
+// host-side shadow the runtime registers, not an address on the GPU: handing it to a kernel as a pointer is a fault
+// (or, on systems where the GPU can reach host memory, a silent write to the wrong place).  Host code gets the real
+// address from cudaGetSymbolAddress, per device, with that device current -- noalloc_scratch_ptr() below.
+namespace sa {
+namespace {
+
+constexpr size_t kNoallocUnits = 160;
+constexpr size_t kNoallocBytes = kNoallocUnits * kPartialFloats * sizeof(float) + 512;
+static_assert(kNoallocBytes == SA_LINEAR_NOALLOC_SCRATCH_BYTES, "smoothagent.h states the size of the built-in scratch");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoallocBytes];
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+void *g_noalloc_ptr[kNoallocMaxDevices] = {};  // device address of g_noalloc_scratch on device i; null = not looked up yet
+
+// Device address of the scratch on the CURRENT device.  The first call on a device asks the runtime (which may load
+// this library's device code onto that GPU: not something to do inside a stream capture); later calls read the table.
+cudaError_t noalloc_scratch_ptr(void **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kNoallocMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+}  // namespace sa
+
+extern "C" int32_t sa_linear_noalloc(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N,
+                                     int32_t K, void *stream) {
+    if (M < 0 || N <= 0 || K <= 0) return SA_ERR_INVALID_ARG;
+    if (K % sa::GBK != 0 || N % 8 != 0 || M > (int64_t(1) << 30)) return SA_ERR_UNSUPPORTED;
+    if (M == 0) return SA_OK;
+    if (sa::device_sms() <= 0) return SA_ERR_CUDA;
+    // the same sizing sa_linear_workspace_bytes reports: 0 = the planner would not split this shape (it has enough
+    // tiles to fill the GPU, or K is a single k-step): no scratch is involved and sa_linear is the call to make
+    const size_t need = sa::gemm_plain_splitk_bytes(M, N, K);
+    if (need == 0) return SA_ERR_UNSUPPORTED;
+    if (need > sa::kNoallocBytes) return SA_ERR_WORKSPACE_TOO_SMALL;  // never silently unsplit: the bits would change
+    void *scratch = nullptr;
+    if (sa::noalloc_scratch_ptr(&scratch) != cudaSuccess) return SA_ERR_CUDA;
+    // Nothing in the scratch has to start at zero: every partial word the reduction kernel reads (rows < M, all 256
+    // columns of each k slice of each tile) is written by the GEMM kernel of this same call, in stream order before it.
+    return sa::gemm_plain(x, w, residual, y, M, N, K, scratch, sa::kNoallocBytes, static_cast<cudaStream_t>(stream), nullptr);
+}
