@@ -502,7 +502,9 @@ SA_API int32_t sa_kv_session_import(sa_kv_pool *pool, int32_t sid, int64_t n_tok
  * n_tokens[i]) of session sids[i] and has its own image (images[i], image_bytes[i]; any mix of local and peer addresses);
  * a session may appear in several ranges of an export.  Import: session sids[i] (each at most once) grows by n_tokens[i]
  * tokens from images[i]; page allocation is all-or-nothing over the whole call.  sids, tok_begin, n_tokens, images,
- * image_bytes are HOST arrays of n entries, copied before the call returns; at most 4 x max_sessions ranges per export. */
+ * image_bytes are HOST arrays of n entries, copied before the call returns; at most 4 x max_sessions ranges per export (a list
+ * longer than one metadata slab of the pool holds -- about 2 x max_sessions + num_pages / 8 + 2000 ranges -- is enqueued as several
+ * launches; the images do not depend on that). */
 SA_API int32_t sa_kv_sessions_export(sa_kv_pool *pool, int32_t n_ranges, const int32_t *sids, const int64_t *tok_begin,
                               const int64_t *n_tokens, void *const *images, const size_t *image_bytes, void *stream);
 SA_API int32_t sa_kv_sessions_import(sa_kv_pool *pool, int32_t n_sessions, const int32_t *sids, const int64_t *n_tokens,

@@ -330,7 +330,8 @@ int32_t append_prepare(sa_kv_pool *pool, int32_t n_req, const int32_t *sids, con
     const bool inline_meta = im && !pool->host_only && n_req <= kInlineReqs && need_pages <= kInlinePages;
     char *mh = nullptr, *md = nullptr;
     if (!pool->host_only && !inline_meta) {
-        int32_t st = acquire_meta(pool, &mh, &md);
+        // upper bound of the slab layout written below: [ReqMeta x n_req][new page ids][ReqMeta x (gained <= n_req)]
+        int32_t st = acquire_meta(pool, 2 * sizeof(ReqMeta) * size_t(n_req) + sizeof(int32_t) * size_t(need_pages + 1) + 16, &mh, &md);
         if (st != SA_OK) return st;
     }
     std::vector<ReqMeta> host_meta;  // host-only pools keep the same bookkeeping path

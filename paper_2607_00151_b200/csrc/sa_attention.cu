@@ -282,9 +282,9 @@ extern "C" int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int
     // otherwise the per-call metadata [decode ReqMeta][prefill ReqMeta][tcgen05 schedule] goes through the pinned slab
     // ring; a schedule too long for the slab goes through the pool's growable pinned buffer into the workspace
     char *mh = nullptr, *md = nullptr;
-    st = acquire_meta(pool, &mh, &md);
-    if (st != SA_OK) return st;
     const size_t dec_bytes = sizeof(ReqMeta) * hp.dec.size(), pre_bytes = sizeof(ReqMeta) * hp.pre.size();
+    st = acquire_meta(pool, dec_bytes + pre_bytes, &mh, &md);
+    if (st != SA_OK) return st;
     const size_t sched_bytes = hp.sched.parts.empty() ? 0 : hp.sched.payload_bytes();
     const size_t off_sched = align_up(dec_bytes + pre_bytes, 32);
     if (dec_bytes) memcpy(mh, hp.dec.data(), dec_bytes);

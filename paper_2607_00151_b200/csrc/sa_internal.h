@@ -175,7 +175,9 @@ struct DeviceGuard {
 
 // Reserve the next metadata slab (host pinned + device twin); waits for the slab's previous
 // copy if it is still in flight.  commit_meta enqueues the H2D copy of `bytes` bytes.
-int32_t acquire_meta(sa_kv_pool *pool, char **host, char **dev);
+// `bytes`: what the caller is about to write into the slab; more than a slab holds is refused (SA_ERR_UNSUPPORTED)
+// before anything is touched, never written past the slab's end.
+int32_t acquire_meta(sa_kv_pool *pool, size_t bytes, char **host, char **dev);
 int32_t commit_meta(sa_kv_pool *pool, size_t bytes, cudaStream_t stream);
 // Same slab, but the bytes go to `dev_dst` (a block-table row) instead of the slab's device twin.
 int32_t commit_meta_to(sa_kv_pool *pool, void *dev_dst, size_t bytes, cudaStream_t stream);

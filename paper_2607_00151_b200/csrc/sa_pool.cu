@@ -238,10 +238,10 @@ static int32_t upload_row(sa_kv_pool *pool, int32_t sid, cudaStream_t stream) {
     const sa::Session &s = pool->sessions[size_t(sid)];
     if (pool->host_only || s.pages.empty()) return SA_OK;
     char *mh = nullptr, *md = nullptr;
-    int32_t st = sa::acquire_meta(pool, &mh, &md);
+    const size_t bytes = s.pages.size() * sizeof(int32_t);  // the slab holds 4 bytes per pool page: always fits
+    int32_t st = sa::acquire_meta(pool, bytes, &mh, &md);
     if (st != SA_OK) return st;
-    const size_t bytes = s.pages.size() * sizeof(int32_t);
-    memcpy(mh, s.pages.data(), bytes);  // the slab holds 4 bytes per pool page: always fits
+    memcpy(mh, s.pages.data(), bytes);
     return sa::commit_meta_to(pool, pool->block_table + int64_t(sid) * pool->max_pages_per_session, bytes, stream);
 }
 
@@ -336,7 +336,8 @@ extern "C" int32_t sa_last_launch_count(const sa_kv_pool *pool, int32_t *out_lau
 
 namespace sa {
 
-int32_t acquire_meta(sa_kv_pool *pool, char **host, char **dev) {
+int32_t acquire_meta(sa_kv_pool *pool, size_t bytes, char **host, char **dev) {
+    if (bytes > pool->meta_slab_bytes) return SA_ERR_UNSUPPORTED;
     int i = pool->meta_next;
     if (pool->meta_event_used[i]) {
         if (cudaEventSynchronize(pool->meta_event[i]) != cudaSuccess) return SA_ERR_CUDA;

@@ -12,6 +12,7 @@
 #include <cuda_bf16.h>
 #include <string.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "sa_internal.h"
@@ -165,7 +166,7 @@ extern "C" int32_t sa_kv_sessions_export(sa_kv_pool *pool, int32_t n_ranges, con
     if (!device_guard.ok) return SA_ERR_CUDA;
     if (!pool || n_ranges < 0) return SA_ERR_INVALID_ARG;
     if (n_ranges > 0 && (!sids || !tok_begin || !n_tokens || !images || !image_bytes)) return SA_ERR_INVALID_ARG;
-    if (n_ranges > pool->cfg.max_sessions * 4) return SA_ERR_INVALID_ARG;   // the metadata slab holds this many ranges
+    if (n_ranges > int64_t(pool->cfg.max_sessions) * 4) return SA_ERR_INVALID_ARG;   // the documented limit of a call
     std::vector<sa::XferReq> reqs(static_cast<size_t>(n_ranges));
     int64_t total = 0;
     for (int i = 0; i < n_ranges; ++i) {
@@ -201,16 +202,36 @@ extern "C" int32_t sa_kv_sessions_export(sa_kv_pool *pool, int32_t n_ranges, con
             ix, nullptr, n_ranges, int32_t(total), kb, vb, pool->block_table, pool->max_pages_per_session, pool->log2_page,
             pool->stride_page, pool->stride_head, pool->cfg.num_kv_heads, pool->cfg.head_dim);
     } else {
-        char *mh = nullptr, *md = nullptr;
-        const int32_t st = sa::acquire_meta(pool, &mh, &md);
-        if (st != SA_OK) return st;
-        memcpy(mh, reqs.data(), sizeof(sa::XferReq) * size_t(n_ranges));
-        if (sa::commit_meta(pool, sizeof(sa::XferReq) * size_t(n_ranges), stream) != SA_OK) return SA_ERR_CUDA;  // counts its launch
+        // The ranges go through the pinned metadata slab, as many per launch as one slab holds (a slab is sized for a
+        // call's requests and page ids, not for 4 x max_sessions ranges: a pool with many sessions and few pages has
+        // slabs smaller than that).  Ranges are independent, so a longer list is cut into several launches, each over
+        // its own slab of the ring with its token offsets rebased; the result does not depend on where the cuts fall.
         static const sa::InlineXfer none{};
-        sa::kv_export_kernel<false><<<grid, sa::kXferThreads, 0, stream>>>(
-            none, reinterpret_cast<const sa::XferReq *>(md), n_ranges, int32_t(total), kb, vb, pool->block_table,
-            pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head, pool->cfg.num_kv_heads,
-            pool->cfg.head_dim);
+        const size_t per_slab = pool->meta_slab_bytes / sizeof(sa::XferReq);
+        if (per_slab == 0) return SA_ERR_UNSUPPORTED;
+        for (size_t i0 = 0; i0 < size_t(n_ranges); i0 += per_slab) {
+            const size_t n = std::min(per_slab, size_t(n_ranges) - i0);
+            const int32_t t_base = reqs[i0].t_start;
+            const int64_t t_end = i0 + n < size_t(n_ranges) ? int64_t(reqs[i0 + n].t_start) : total;
+            if (t_end == t_base) continue;  // nothing but empty ranges
+            char *mh = nullptr, *md = nullptr;
+            const int32_t st = sa::acquire_meta(pool, sizeof(sa::XferReq) * n, &mh, &md);
+            if (st != SA_OK) return st;
+            sa::XferReq *dst = reinterpret_cast<sa::XferReq *>(mh);
+            for (size_t i = 0; i < n; ++i) {
+                dst[i] = reqs[i0 + i];
+                dst[i].t_start -= t_base;
+            }
+            if (sa::commit_meta(pool, sizeof(sa::XferReq) * n, stream) != SA_OK) return SA_ERR_CUDA;  // counts its launch
+            const int32_t sub_total = int32_t(t_end - t_base);
+            sa::kv_export_kernel<false><<<unsigned((sub_total + sa::kXferTok - 1) / sa::kXferTok), sa::kXferThreads, 0, stream>>>(
+                none, reinterpret_cast<const sa::XferReq *>(md), int32_t(n), sub_total, kb, vb, pool->block_table,
+                pool->max_pages_per_session, pool->log2_page, pool->stride_page, pool->stride_head, pool->cfg.num_kv_heads,
+                pool->cfg.head_dim);
+            ++pool->last_launches;
+            if (cudaGetLastError() != cudaSuccess) return SA_ERR_CUDA;
+        }
+        return SA_OK;
     }
     ++pool->last_launches;
     return cudaGetLastError() == cudaSuccess ? SA_OK : SA_ERR_CUDA;
@@ -257,7 +278,7 @@ extern "C" int32_t sa_kv_sessions_import(sa_kv_pool *pool, int32_t n_sessions, c
     } else {
         // the image addresses follow the requests through a slab of their own
         char *mh = nullptr, *md = nullptr;
-        const int32_t s2 = sa::acquire_meta(pool, &mh, &md);
+        const int32_t s2 = sa::acquire_meta(pool, sizeof(uint64_t) * size_t(n_sessions), &mh, &md);
         if (s2 != SA_OK) return s2;
         memcpy(mh, images, sizeof(uint64_t) * size_t(n_sessions));
         if (sa::commit_meta(pool, sizeof(uint64_t) * size_t(n_sessions), stream) != SA_OK) return SA_ERR_CUDA;  // counts its launch

@@ -263,3 +263,56 @@ def test_many_sessions_in_one_call_equal_one_call_per_session(n_sessions):
             assert (_bits(kp[pg, :, lo:, :]) == sent).all() and (_bits(vp[pg, :, lo:, :]) == sent).all()
     for p_ in (src, dst_a, dst_b):
         sa.sa_kv_pool_destroy(p_)
+
+
+def test_export_at_the_range_limit_of_a_pool_whose_slabs_are_smaller_than_it():
+    """4 x max_sessions ranges in one sa_kv_sessions_export on a pool with many sessions and few pages: its metadata slab
+    (64 (max_sessions + 8) + 4 num_pages + 64 KiB + 64 bytes = 198 208 here) holds 6194 ranges of 32 bytes, the documented
+    limit is 8192.  The list must go out in slab-sized pieces, never past a slab's end (that used to overwrite the next
+    slab of the ring): every image equals the same tokens cut from a whole-session export made through the
+    kernel-parameter path, the bytes between and after the images keep their sentinel, and one range more is refused."""
+    L = Layer(8, 2, 64, 16, 10000.0)
+    max_sessions, pages = 2048, 256
+    cfg = sa.PoolConfig(L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size, pages, max_sessions, 256, L.rope_base, 0)
+    nbytes = sa.sa_kv_pool_storage_bytes(cfg)
+    storage = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+    pool = sa.sa_kv_pool_create(cfg, storage, np.random.default_rng(5).permutation(pages).astype(np.int32))
+    rng = np.random.default_rng(6)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(8)
+    lens = [int(x) for x in rng.integers(60, 200, size=16)]
+    sids = [sa.sa_kv_session_open(pool) for _ in lens]
+    whole = []
+    for sid, n in zip(sids, lens):
+        sa.sa_rope_kv_append(pool, [sid], [0, n], _rand(n, 2, 64, gen, 1.0), _rand(n, 2, 64, gen, 1.0), None)
+        im = torch.empty((2, 2, n, 64), dtype=torch.bfloat16, device="cuda")
+        sa.sa_kv_session_export(pool, sid, 0, n, im)
+        whole.append(im)
+    n_ranges = 4 * max_sessions
+    which = rng.integers(0, len(sids), size=n_ranges)
+    n_tok = rng.integers(0, 5, size=n_ranges)
+    n_tok[:3] = 0                      # the list starts with empty ranges
+    n_tok[6190:6200] = [0, 3, 0, 0, 4, 1, 0, 0, 2, 0]   # and has some around the cut
+    t0 = np.array([rng.integers(0, lens[w] - n + 1) for w, n in zip(which, n_tok)])
+    per_tok = 2 * 2 * 64               # bf16 elements of one token in an image
+    offs = np.concatenate([[0], np.cumsum(n_tok * per_tok + 8)])   # 16 sentinel bytes after every image
+    flat = torch.full((int(offs[-1]),), SENT, dtype=torch.int16, device="cuda")
+    images = [flat[int(o): int(o) + int(n) * per_tok].view(torch.bfloat16).view(2, 2, int(n), 64) for o, n in zip(offs[:-1], n_tok)]
+    sa.sa_kv_sessions_export(pool, [sids[w] for w in which], t0, n_tok, images)
+    assert sa.sa_last_launch_count(pool) == 4          # two pieces, each a metadata upload and a gather
+    torch.cuda.synchronize()
+    for i in range(n_ranges):
+        want = whole[which[i]][:, :, int(t0[i]): int(t0[i]) + int(n_tok[i]), :]
+        assert torch.equal(_bits(images[i]), _bits(want)), "range %d" % i
+    gaps = torch.cat([flat[int(o) - 8: int(o)] for o in offs[1:]])
+    assert (gaps == np.array(SENT, dtype=np.uint16).view(np.int16).item()).all()
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_kv_sessions_export(pool, [sids[0]] * (n_ranges + 1), [0] * (n_ranges + 1), [0] * (n_ranges + 1),
+                                 [images[0]] * (n_ranges + 1))
+    assert e.value.status == sa.SA_ERR_INVALID_ARG
+    # the pool still works: a later attention-free call on it reads the same cache
+    again = torch.empty_like(whole[3])
+    sa.sa_kv_session_export(pool, sids[3], 0, lens[3], again)
+    torch.cuda.synchronize()
+    assert torch.equal(_bits(again), _bits(whole[3]))
+    sa.sa_kv_pool_destroy(pool)
