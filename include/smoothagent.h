@@ -232,7 +232,20 @@ SA_API int32_t sa_mixed_attention_schedule(const sa_kv_pool *pool, int32_t n_req
  *   k, v           : device bf16 [n_req, Hkv, D], pre-RoPE; q_inout: device bf16 [n_req, Hq, D]
  *   out            : device bf16 [n_req, Hq, D]; lse: device f32 [n_req, Hq], nullable
  *   sa_decode_step_stats: host int64[6] = {requests, work items, CTAs of the attention grid, launches of the last
- *                    enqueue, partial rows the workspace holds, capacity} */
+ *                    enqueue, partial rows the workspace holds, capacity}
+ * One prepare, one execution.  Every successful prepare must be followed by an execution of the step -- an
+ * sa_decode_step_enqueue, or a replay of the graph it was captured into -- before the next prepare.  The library cannot see
+ * graph replays, so it cannot check this; a prepare that is never executed leaves its sessions one token longer with
+ * nothing written at that position (and, where it took a page, a device block-table entry that stays unwritten until a
+ * later step places a token in that page), and a later attention over such a session reads whatever those slots held.
+ *   sa_decode_step_cancel    HOST ONLY.  Undoes the step's last successful prepare when it will not be executed (the batch
+ *       changed, a request was aborted): the sessions get their old lengths back, pages the prepare took return to the
+ *       free list so that they are handed out again in the same order, and the step holds no batch (enqueue is refused
+ *       until the next prepare; a replay of an already captured graph does nothing).  SA_ERR_INVALID_ARG, with nothing
+ *       changed, if there is no prepare to undo (none yet, or already cancelled) or one of its sessions has been closed,
+ *       grown or truncated since.  Cancelling a prepare that HAS executed amounts to truncating its sessions by one token.
+ * Lifetime: a step refers to its pool in every call except sa_decode_step_destroy; destroy the steps of a pool before
+ * the pool, or at least never prepare / enqueue / cancel / query a step once its pool is gone. */
 typedef struct sa_decode_step sa_decode_step; /* opaque */
 SA_API int32_t sa_decode_step_device_bytes(const sa_kv_pool *pool, int32_t max_requests, int64_t max_kv_tokens,
                                            size_t *out_bytes);
@@ -240,6 +253,7 @@ SA_API int32_t sa_decode_step_create(sa_kv_pool *pool, int32_t max_requests, int
                                      size_t dev_bytes, sa_decode_step **out_step);
 SA_API int32_t sa_decode_step_destroy(sa_decode_step *step);
 SA_API int32_t sa_decode_step_prepare(sa_decode_step *step, int32_t n_req, const int32_t *sids);
+SA_API int32_t sa_decode_step_cancel(sa_decode_step *step);
 SA_API int32_t sa_decode_step_enqueue(sa_decode_step *step, const void *k, const void *v, void *q_inout, void *out,
                                       float *lse, float sm_scale, void *stream);
 SA_API int32_t sa_decode_step_stats(const sa_decode_step *step, int64_t *out_stats);

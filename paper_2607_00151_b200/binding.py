@@ -156,6 +156,7 @@ PROTOTYPES = {
     "sa_decode_step_create": (ctypes.c_int32, [_vp, ctypes.c_int32, ctypes.c_int64, _vp, ctypes.c_size_t, ctypes.POINTER(_vp)]),
     "sa_decode_step_destroy": (ctypes.c_int32, [_vp]),
     "sa_decode_step_prepare": (ctypes.c_int32, [_vp, ctypes.c_int32, _i32p]),
+    "sa_decode_step_cancel": (ctypes.c_int32, [_vp]),
     "sa_decode_step_enqueue": (ctypes.c_int32, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp]),
     "sa_decode_step_stats": (ctypes.c_int32, [_vp, _i64p]),
 }
@@ -622,6 +623,11 @@ def sa_decode_step_prepare(step: DecodeStep, sids) -> None:
     """Host half of one decode iteration: every session grows by one token, the step's metadata is rewritten."""
     keep, ptr = _i32(sids)
     _check(load_library().sa_decode_step_prepare(step.handle, keep.shape[0], ptr), "sa_decode_step_prepare")
+
+
+def sa_decode_step_cancel(step: DecodeStep) -> None:
+    """Undo the step's last prepare (one that will not be executed): lengths and pages as before it, the step empty."""
+    _check(load_library().sa_decode_step_cancel(step.handle), "sa_decode_step_cancel")
 
 
 def sa_decode_step_enqueue(step: DecodeStep, k, v, q_inout, out, lse=None, sm_scale: float = 0.0, stream=None) -> None:

@@ -26,6 +26,8 @@
 
 struct sa_decode_step {
     sa_kv_pool *pool = nullptr;
+    bool host_only = false;      // copies of the pool's, so that destroying the step never reads the pool
+    int device = 0;
     int32_t cap = 0;             // most requests a step can carry
     int64_t max_kv = 0;          // longest cache (own token included) a request of a step can have
     int64_t max_part_rows = 0;   // partial rows the workspace holds
@@ -35,6 +37,14 @@ struct sa_decode_step {
     int32_t grid_ctas = 0;
     int32_t last_launches = 0;
     bool prepared = false;
+    // what the last successful prepare did, for sa_decode_step_cancel: (session, length before it, page it took or -1)
+    struct Undo {
+        int32_t sid;
+        int64_t len_before;
+        int32_t page_taken;
+    };
+    std::vector<Undo> undo;
+    bool can_cancel = false;
 };
 
 namespace {
@@ -77,6 +87,8 @@ extern "C" int32_t sa_decode_step_create(sa_kv_pool *pool, int32_t max_requests,
     sa_decode_step *st = new (std::nothrow) sa_decode_step();
     if (!st) return SA_ERR_INVALID_ARG;
     st->pool = pool;
+    st->host_only = pool->host_only;
+    st->device = pool->cfg.device;
     st->cap = max_requests;
     st->max_kv = max_kv_tokens;
     st->max_part_rows = l.max_part_rows;
@@ -116,11 +128,11 @@ extern "C" int32_t sa_decode_step_create(sa_kv_pool *pool, int32_t max_requests,
 
 extern "C" int32_t sa_decode_step_destroy(sa_decode_step *step) {
     if (!step) return SA_ERR_INVALID_ARG;
-    if (step->slab_host) {
-        if (step->pool->host_only) {
+    if (step->slab_host) {  // the pool may be gone already: nothing of it is read here
+        if (step->host_only) {
             free(step->slab_host);
         } else {
-            sa::DeviceGuard device_guard(step->pool);
+            sa::DeviceGuard device_guard(step->device);
             cudaFreeHost(step->slab_host);
         }
     }
@@ -158,9 +170,15 @@ extern "C" int32_t sa_decode_step_prepare(sa_decode_step *step, int32_t n_req, c
     StepAppend *app = reinterpret_cast<StepAppend *>(step->slab_host + step_append_offset(step->cap));
     const int Hkv = pool->cfg.num_kv_heads, Hq = pool->cfg.num_q_heads;
     int64_t items = 0, parts = 0;
+    step->undo.clear();
     for (int r = 0; r < n_req; ++r) {
         Session &s = pool->sessions[size_t(sids[r])];
-        if (s.len % B == 0) s.pages.push_back(take_page(pool));
+        sa_decode_step::Undo u{sids[r], s.len, -1};
+        if (s.len % B == 0) {
+            s.pages.push_back(take_page(pool));
+            u.page_taken = s.pages.back();
+        }
+        step->undo.push_back(u);
         StepAppend a{};
         a.sid = sids[r];
         a.pos = int32_t(s.len);
@@ -182,6 +200,37 @@ extern "C" int32_t sa_decode_step_prepare(sa_decode_step *step, int32_t n_req, c
     hd->n_req = n_req;
     hd->n_items = int32_t(items);
     step->prepared = true;
+    step->can_cancel = true;
+    return SA_OK;
+}
+
+extern "C" int32_t sa_decode_step_cancel(sa_decode_step *step) {
+    using namespace sa;
+    if (!step || !step->can_cancel) return SA_ERR_INVALID_ARG;
+    sa_kv_pool *pool = step->pool;
+    // every session must still be as the prepare left it, or nothing is undone
+    for (const sa_decode_step::Undo &u : step->undo) {
+        if (u.sid < 0 || size_t(u.sid) >= pool->sessions.size()) return SA_ERR_INVALID_ARG;
+        const Session &s = pool->sessions[size_t(u.sid)];
+        if (!s.open || s.len != u.len_before + 1 || s.pages.empty()) return SA_ERR_INVALID_ARG;
+        if (u.page_taken >= 0 && (s.pages.back() != u.page_taken || pool->page_ref[size_t(u.page_taken)] != 1)) return SA_ERR_INVALID_ARG;
+    }
+    // in reverse, so that the free list hands the same pages out in the same order again
+    for (size_t i = step->undo.size(); i-- > 0;) {
+        const sa_decode_step::Undo &u = step->undo[i];
+        Session &s = pool->sessions[size_t(u.sid)];
+        if (u.page_taken >= 0) {
+            release_page(pool, s.pages.back());
+            s.pages.pop_back();
+        }
+        s.len = u.len_before;
+    }
+    step->undo.clear();
+    step->can_cancel = false;
+    step->prepared = false;  // the slab describes a batch that no longer exists: enqueue is refused until the next prepare
+    StepHeader *hd = reinterpret_cast<StepHeader *>(step->slab_host);
+    hd->n_req = 0;
+    hd->n_items = 0;
     return SA_OK;
 }
 

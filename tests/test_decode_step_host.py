@@ -95,3 +95,51 @@ def test_create_arguments():
         with pytest.raises(sa.SAError):
             sa.sa_decode_step_create(p, cap, mk)
     assert sa.sa_decode_step_device_bytes(p, 4, 512) > 4 * 8 * 64 * 4
+
+
+def test_cancel_undoes_the_last_prepare_and_only_that():
+    """sa_decode_step_cancel (a prepared step that will not run): lengths back, pages back so that they are handed out in
+    the same order again, the step empty; refused when there is nothing to undo or a session moved since."""
+    order = np.random.default_rng(2).permutation(256).astype(np.int32)
+    p = _pool(order=order)
+    a, b, c = (sa.sa_kv_session_open(p) for _ in range(3))
+    sa.sa_rope_kv_append(p, [a, b, c], [0, 16, 16 + 20, 16 + 20 + 32], None, None)   # a, c end on a page boundary, b inside one
+    step = sa.sa_decode_step_create(p, 4, 4096)
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_decode_step_cancel(step)                       # nothing prepared yet
+    assert e.value.status == sa.SA_ERR_INVALID_ARG
+    before = [sa.sa_kv_session_query(p, s) for s in (a, b, c)], sa.sa_kv_pool_free_pages(p)
+    sa.sa_decode_step_prepare(step, [a, b, c])
+    after = [sa.sa_kv_session_query(p, s) for s in (a, b, c)], sa.sa_kv_pool_free_pages(p)
+    assert after[1] == before[1] - 2 and [x[0] for x in after[0]] == [17, 21, 33]
+    sa.sa_decode_step_cancel(step)
+    assert ([sa.sa_kv_session_query(p, s) for s in (a, b, c)], sa.sa_kv_pool_free_pages(p)) == before
+    st = sa.sa_decode_step_stats(step)
+    assert st["requests"] == 0 and st["items"] == 0
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_decode_step_cancel(step)                       # already undone
+    assert e.value.status == sa.SA_ERR_INVALID_ARG
+    # the same prepare again takes the same pages for the same sessions
+    sa.sa_decode_step_prepare(step, [a, b, c])
+    assert ([sa.sa_kv_session_query(p, s) for s in (a, b, c)], sa.sa_kv_pool_free_pages(p)) == after
+    # a session that moved since the prepare: nothing is undone
+    sa.sa_kv_session_truncate(p, b, 5)
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_decode_step_cancel(step)
+    assert e.value.status == sa.SA_ERR_INVALID_ARG
+    assert sa.sa_kv_session_query(p, a) == after[0][0] and sa.sa_kv_session_query(p, c) == after[0][2]
+    assert sa.sa_kv_session_query(p, b)[0] == 5
+    # a failed prepare does not disturb what can be cancelled: the last SUCCESSFUL prepare stays the one that is undone
+    sa.sa_decode_step_prepare(step, [a])
+    with pytest.raises(sa.SAError):
+        sa.sa_decode_step_prepare(step, [a, a])
+    sa.sa_decode_step_cancel(step)
+    assert sa.sa_kv_session_query(p, a) == after[0][0]
+
+
+def test_step_may_be_destroyed_after_its_pool():
+    """sa_decode_step_destroy reads nothing of the pool (garbage collection may run it after sa_kv_pool_destroy)."""
+    p = _pool()
+    step = sa.sa_decode_step_create(p, 2, 64)
+    sa.sa_kv_pool_destroy(p)
+    sa.sa_decode_step_destroy(step)

@@ -211,9 +211,84 @@ def test_decode_step_errors_on_a_device_pool_change_nothing():
     torch.cuda.synchronize()
     assert torch.equal(_bits(out), _bits(first[0])) and torch.equal(lse, first[1])
     # a cache longer than the step was created for
-    for _ in range(7):
+    for _ in range(7):                                # one prepare, one execution (include/smoothagent.h)
         sa.sa_decode_step_prepare(step, [a])
+        q.copy_(q0)
+        sa.sa_decode_step_enqueue(step, k, v, q, out, lse)
     assert sa.sa_kv_session_query(pool, a)[0] == 40
     with pytest.raises(sa.SAError) as e:
         sa.sa_decode_step_prepare(step, [a])
     assert e.value.status == sa.SA_ERR_INVALID_ARG and sa.sa_kv_session_query(pool, a)[0] == 40
+
+
+def test_cancelled_prepare_leaves_no_trace_on_the_device_path():
+    """sa_decode_step_cancel on a device pool: a prepared batch that is dropped instead of executed.  A replay of the
+    captured graph after the cancel touches nothing, and the next prepared batch (other sessions, the pages the dropped
+    one had taken handed out again) equals the eager calls on a twin pool that never saw the dropped batch, bit for bit."""
+    Hq, Hkv, D, page, base = 8, 2, 64, 16, 1e4
+    lens0 = [15, 37, 1023, 47]                       # after iteration 0 sessions 0, 2, 3 end on a page boundary
+    n = len(lens0)
+    eager, stepped, cfg = _twin_pools(Hq, Hkv, D, page, 96, n + 1, 2048, base, 11)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(99)
+    rnd = lambda t, h: (torch.randn((t, h, D), generator=gen, device="cuda") * 0.7).to(torch.bfloat16)
+    sids_e = [sa.sa_kv_session_open(eager) for _ in range(n)]
+    sids_s = [sa.sa_kv_session_open(stepped) for _ in range(n)]
+    indptr = np.concatenate([[0], np.cumsum(lens0)]).astype(np.int32)
+    kk, vv = rnd(int(indptr[-1]), Hkv), rnd(int(indptr[-1]), Hkv)
+    for pool, sids in ((eager, sids_e), (stepped, sids_s)):
+        sa.sa_rope_kv_append(pool, sids, indptr, kk, vv, None)
+    step = sa.sa_decode_step_create(stepped, n, 2048)
+    k_in, v_in, q_in = rnd(n, Hkv), rnd(n, Hkv), rnd(n, Hq)
+    out = torch.full((n, Hq, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    lse = torch.full((n, Hq), float("nan"), dtype=torch.float32, device="cuda")
+
+    def eager_step(batch, k1, v1, q1):
+        b = len(batch)
+        qe, ip, se = q1.clone(), np.arange(b + 1, dtype=np.int32), [sids_e[i] for i in batch]
+        sa.sa_rope_kv_append(eager, se, ip, k1, v1, qe)
+        oe, le = torch.empty_like(qe), torch.empty((b, Hq), dtype=torch.float32, device="cuda")
+        ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(eager, se, ip), 256), dtype=torch.uint8, device="cuda")
+        sa.sa_mixed_attention(eager, se, ip, qe, oe, le, 0.0, ws)
+        torch.cuda.synchronize()
+        return oe, le
+
+    # iteration 0 on both pools, captured
+    k1, v1, q1 = k_in.clone(), v_in.clone(), q_in.clone()
+    oe, le = eager_step(list(range(n)), k1, v1, q1)
+    sa.sa_decode_step_prepare(step, sids_s)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        sa.sa_decode_step_enqueue(step, k_in, v_in, q_in, out, lse)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(_bits(out), _bits(oe)) and torch.equal(lse, le)
+    # a batch is prepared (sessions 2 and 0 each take a page for it) and dropped
+    state = [sa.sa_kv_session_query(stepped, s) for s in sids_s], sa.sa_kv_pool_free_pages(stepped)
+    pool_bits = stepped.storage.clone()
+    sa.sa_decode_step_prepare(step, [sids_s[1], sids_s[2], sids_s[0]])
+    assert sa.sa_kv_pool_free_pages(stepped) == state[1] - 2
+    sa.sa_decode_step_cancel(step)
+    assert ([sa.sa_kv_session_query(stepped, s) for s in sids_s], sa.sa_kv_pool_free_pages(stepped)) == state
+    with pytest.raises(sa.SAError) as e:
+        sa.sa_decode_step_enqueue(step, k_in, v_in, q_in, out, lse)      # the step holds no batch
+    assert e.value.status == sa.SA_ERR_INVALID_ARG
+    out.fill_(float("nan"))
+    lse.fill_(float("nan"))
+    q_keep = q_in.clone()
+    graph.replay()                                                       # an empty step: nothing is placed, no row is written
+    torch.cuda.synchronize()
+    assert torch.isnan(out.float()).all() and torch.isnan(lse).all() and torch.equal(_bits(q_in), _bits(q_keep))
+    kv_bytes = 2 * 96 * Hkv * page * D * 2                               # the K and V pages lead the pool's storage
+    assert torch.equal(stepped.storage[:kv_bytes], pool_bits[:kv_bytes]), "a cancelled step wrote into the cache"
+    # the next real batch: the twin pool never heard of the dropped one
+    batch = [3, 0, 2]
+    k1, v1, q1 = rnd(3, Hkv), rnd(3, Hkv), rnd(3, Hq)
+    oe, le = eager_step(batch, k1, v1, q1)
+    sa.sa_decode_step_prepare(step, [sids_s[i] for i in batch])
+    k_in[:3], v_in[:3], q_in[:3] = k1, v1, q1
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(_bits(out[:3]), _bits(oe)) and torch.equal(lse[:3], le)
+    for i in range(n):
+        assert sa.sa_kv_session_query(eager, sids_e[i]) == sa.sa_kv_session_query(stepped, sids_s[i])
