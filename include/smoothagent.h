@@ -182,7 +182,13 @@ SA_API int32_t sa_mixed_attention(sa_kv_pool *pool, int32_t n_req, const int32_t
                            const int32_t *qo_indptr, const void *q, void *out, float *lse,
                            float sm_scale, void *workspace, size_t workspace_bytes, void *stream);
 
-/* Host-side planner statistics of the batch sa_mixed_attention would run (no device work; works
+/* The three planning calls below take a `const sa_kv_pool *` because they change nothing a caller can observe, but
+ * they do write a per-pool cache (the plan of the last batch planned, which the sa_mixed_attention call that follows
+ * takes over instead of planning again) and sa_mixed_attention_schedule / _plan read it.  Like every call on a pool
+ * they must therefore be serialised with the other calls on that pool: a scheduler thread sizing a batch while a worker
+ * thread enqueues on the same pool is a data race.  Plan on a host-only twin pool if two threads must do both.
+ *
+ * Host-side planner statistics of the batch sa_mixed_attention would run (no device work; works
  * on host-only pools).  out_stats (host int64[8]) = { decode-like requests, prefill requests,
  * decode CTAs, prefill work items (parts of the schedule on the tcgen05 path), split partial rows, sum_j L_j over decode-like requests,
  * sum_j A_j over prefill requests (A_j = q_j*prefix_j + q_j(q_j+1)/2, L313), 1 if prefill chunks
@@ -396,7 +402,10 @@ SA_API int32_t sa_swiglu(const void *x, const void *w_gate, const void *w_up, vo
  * tile is cut into slices that run on different SMs (split-K); fp32 partials go through `workspace` and a second
  * kernel sums them IN SLICE ORDER and applies the epilogue, so the result is bit-reproducible run to run (it may
  * differ in the last bit from the unsplit call: another summation order).  *_workspace_bytes returns 0 when the
- * shape will not be split; a null or too small workspace falls back to the unsplit kernel, never to an error. */
+ * shape will not be split; a null or too small workspace falls back to the unsplit kernel, never to an error -- so the
+ * last bit of a result depends on whether the workspace was large enough: pass the same (sufficient) size every time
+ * where bit-reproducibility across calls matters.  sa_qkv_rope_append and sa_layer_forward refuse a workspace smaller
+ * than their *_workspace_bytes, which includes this scratch, so their split never varies. */
 SA_API int32_t sa_linear_workspace_bytes(int64_t M, int32_t N, int32_t K, size_t *out_bytes);
 SA_API int32_t sa_linear_ws(const void *x, const void *w, const void *residual, void *y, int64_t M, int32_t N, int32_t K,
                      void *workspace, size_t workspace_bytes, void *stream);
