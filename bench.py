@@ -506,6 +506,7 @@ def measure_config(cfg_id: int, local: int, peaks, iters: int):
            "note": "attention time is the whole sa_mixed_attention call (the decode rows of the workload included); "
                    "causal algorithmic flops only; L2 flushed between iterations"}
     res["frac"] = res["achieved"] / res["peak"]
+    res["frac_sustained"] = res["achieved"] / peaks["bf16_tflops_sustained"]
     r.close()
     sa.sa_kv_pool_destroy(pool)
     return res
@@ -727,7 +728,7 @@ def measure_layer(local: int, peaks, iters: int = 10):
     out = {"workload": "cfg2_summarize through sa_layer_forward, hidden %d ffn %d" % (H, F), "tokens_per_s": tokens / (ms * 1e-3),
            "ms_per_step": ms, "ms_min": float(min(ts)), "gemm_flops": gemm_flops, "attention_flops": attn_flops,
            "bound": "tensor", "achieved": tf, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": tf / peaks["bf16_tflops"],
-           "launches_per_step": launches, "note": "whole decoder layer per chunk (7 operators), L2 flushed between steps"}
+           "frac_sustained": tf / peaks["bf16_tflops_sustained"], "launches_per_step": launches, "note": "whole decoder layer per chunk (7 operators), L2 flushed between steps"}
     r.close()
     sa.sa_kv_pool_destroy(pool)
     # T_GEMM(M) of PAPER.md L299-303 (the dense operators of the layer alone) at decode sizes, where it is the larger part
@@ -823,6 +824,7 @@ def run_ours(args, world, rank, local):
         achieved = flops_step * args.steps / (attn_ms * 1e-3) / 1e12
         peak = peaks["bf16_tflops"]
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "peak_sustained": peaks["bf16_tflops_sustained"], "frac_sustained": achieved / peaks["bf16_tflops_sustained"],
                 "traffic": load_traffic().get("prefill_tc5_kernel_cfg2_avg_per_launch") if args.config == 2 else None, "peak_source": peaks["source"] + " (burst; sustained %.1f)" % peaks["bf16_tflops_sustained"],
                 "kernel": "prefill attention inside sa_mixed_attention (%d calls timed, avg %.3f ms; decode rows of the same "
                           "call included in the time when the workload has them)" % (n_attn, attn_ms / max(n_attn, 1)),
