@@ -252,7 +252,7 @@ __device__ __forceinline__ void decode_tiles(const KvView &kv, const ReqMeta &r,
 
     for (int t = 0; t < n_tiles; ++t) {
         const int st = t % kStages;
-        ptx::mbar_wait(bars + 8 * st, (phase >> st) & 1u);  // tile t has landed (acquire: its bytes are visible)
+        ptx::mbar_wait_watched(bars + 8 * st, (phase >> st) & 1u);  // tile t has landed (acquire: its bytes are visible)
         phase ^= 1u << st;
         group_sync(bar_id);                                 // ... and everyone is done with tile t - 1: its stage is free
         {

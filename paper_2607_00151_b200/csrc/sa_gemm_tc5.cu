@@ -245,7 +245,7 @@ gemm_tc5_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constan
                         if (phase == 0 && !early) return;
                         const int s = kc % GSTAGES, ph = (kc / GSTAGES) & 1;
                         const uint32_t sA = s0 + s * STAGE_BYTES, sB = sA + A_STAGE;
-                        if (!early) mbar_wait(bar_empty(s), ph ^ 1);
+                        if (!early) mbar_wait_watched(bar_empty(s), ph ^ 1);
                         if (phase == 0 || !early) {
                             mbar_expect_tx(bar_full(s), STAGE_BYTES);
                             tma_load_2d(sB, &tmap_b0, bar_full(s), ks * GBK, r0);

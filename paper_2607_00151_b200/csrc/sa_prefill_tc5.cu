@@ -229,7 +229,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
             for (int p = pb; p < pe; ++p) {
                 const PartGeom gm = load_part<LOG2B>(a, p);
                 // Q of this part may land once every QK product of the previous part has read its Q
-                if (p > pb) mbar_wait(bar(BAR_Q_EMPTY), (p - pb - 1) & 1);
+                if (p > pb) mbar_wait_watched(bar(BAR_Q_EMPTY), (p - pb - 1) & 1);
                 mbar_expect_tx(bar(BAR_Q_FULL), 2 * DH * HALF_BYTES);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
@@ -246,7 +246,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                     int32_t pg[PAGES_PER_TILE];
 #pragma unroll
                     for (int u = 0; u < PAGES_PER_TILE; ++u) pg[u] = u < np ? __ldg(bt + p0 + u) : 0;
-                    mbar_wait(bar(BAR_K_EMPTY + s), ph ^ 1);
+                    mbar_wait_watched(bar(BAR_K_EMPTY + s), ph ^ 1);
                     mbar_expect_tx(bar(BAR_K_FULL + s), uint32_t(np) * DH * PAGE_HALF_BYTES);
 #pragma unroll
                     for (int u = 0; u < PAGES_PER_TILE; ++u)
@@ -254,7 +254,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                             tma_load_4d(sK + s * TILE_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 0, 0, gm.g, pg[u]);
                             if (DH == 2) tma_load_4d(sK + s * TILE_BYTES + HALF_BYTES + u * PAGE_HALF_BYTES, &tmap_k, bar(BAR_K_FULL + s), 64, 0, gm.g, pg[u]);
                         }
-                    mbar_wait(bar(BAR_V_EMPTY + s), ph ^ 1);
+                    mbar_wait_watched(bar(BAR_V_EMPTY + s), ph ^ 1);
                     mbar_expect_tx(bar(BAR_V_FULL + s), uint32_t(np) * DH * PAGE_HALF_BYTES);
 #pragma unroll
                     for (int u = 0; u < PAGES_PER_TILE; ++u)
@@ -472,7 +472,7 @@ prefill_tc5_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_cons
                 l = a0 + a1;
             }
             // ---- epilogue of the part
-            mbar_wait(bar(BAR_O_FULL + t), (p - pb) & 1);
+            mbar_wait_watched(bar(BAR_O_FULL + t), (p - pb) & 1);
             tc_fence_after();
             if (gm.slot < 0) {
                 // whole item: O / l -> bf16 -> out

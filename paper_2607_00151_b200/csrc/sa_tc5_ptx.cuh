@@ -35,8 +35,34 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
+// %globaltimer in units of 2^30 ns (about 1.07 s), 32 bits
+__device__ __forceinline__ uint32_t globaltimer_s() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return uint32_t(t >> 30);
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {
+    }
+}
+// The same wait with a watchdog, for the waits that are off the tensor pipe's critical path: the TMA producers waiting for a
+// free ring slot and the epilogue / softmax warps waiting for a finished accumulator.  Every 16384th failed poll reads the
+// timer; a wait that has lasted kMbarWaitLimit (about 20 s, three orders of magnitude beyond the longest launch of this library)
+// can only mean that whatever should complete the barrier never will -- a TMA that faulted on a bad descriptor or address,
+// a miscounted arrival: the kernel traps (the launch fails with a sticky error, the calls report SA_ERR_CUDA) instead of
+// spinning on the GPU until someone resets it.  Whatever stalls inside a CTA ends up stalling one of these waits too (no
+// operands -> no MMA -> no free slot and no accumulator), so the plain waits of the MMA issuer and of the softmax inner
+// loop need no watchdog of their own: giving them one cost 1.5 % of the prefill kernel (A/B on one box, both with the
+// timer read on every poll and on every 16384th).
+constexpr uint32_t kMbarWaitLimit = 20;
+__device__ __forceinline__ void mbar_wait_watched(uint32_t bar, uint32_t parity) {
+    uint32_t polls = 0, t0 = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if ((++polls & 0x3FFFu) == 0) {
+            const uint32_t now = globaltimer_s();
+            if (polls == 0x4000u) t0 = now;
+            else if (now - t0 > kMbarWaitLimit) __trap();
+        }
     }
 }
 // generic-proxy writes to shared memory -> visible to the async proxy (TMA / tcgen05.mma operands)
