@@ -591,6 +591,95 @@ def measure_decode_step(local: int, peaks, batches=(1, 4, 16, 64), ctx: int = 21
     return out
 
 
+def measure_lookahead_loop(local: int, n_dec: int = 64, P: int = 16384, TAIL: int = 4096, SEG: int = 8192, gran: int = 256,
+                           max_chunk: int = 2048, room_chunk: int = 1024):
+    """The closed loop of Algorithm 2 on the kernels at config 4's scale: n_dec
+    latency-critical decode requests on 8 K - 32 K caches decode one token per iteration while a lookahead re-prefill of SEG
+    tokens behind a retained prefix of P tokens is streamed into a forked session, the chunk of each iteration sized by
+    sa_dynamic_chunk under delta with an Eq. 1 model fitted on an sa_latency_table of this pool, the batch admitted by
+    sa_schedule_hybrid, then RUN (one sa_rope_kv_append + one sa_mixed_attention over decode rows and chunk together) and
+    the session committed at the end.  Reported per iteration: the estimate and the measured device time of the attention
+    call (what Eq. 1 models here: this path has no GEMMs) against delta.  Synthetic lengths and values."""
+    from paper_2607_00151_b200 import binding as sa
+    L = get_workload(4).layer
+    dev = torch.device("cuda:%d" % local)
+    Hq, Hkv, D, B = L.num_q_heads, L.num_kv_heads, L.head_dim, L.page_size
+    rng = np.random.default_rng(44)
+    dec_len = [int(x) for x in rng.integers(8192, 32768, size=n_dec)]
+    pages = sum(n // B + 3 for n in dec_len) + (P + TAIL + SEG) // B + 3 * (SEG // B) + 64
+    cfg = sa.PoolConfig(Hq, Hkv, D, B, pages, n_dec + 8, 65536, L.rope_base, local)
+    pool = sa.sa_kv_pool_create(cfg)
+    try:
+        g = torch.Generator(device=dev)
+        g.manual_seed(4)
+        rnd = lambda n, h: (torch.randn((n, h, D), generator=g, device=dev) * D ** -0.5).to(torch.bfloat16)
+        pt, db = [0, 512, 1024, 2048], [0, 16, n_dec]
+        ms, sums = sa.sa_latency_table(pool, pt, db, P + SEG // 2, 8192, 32768, seed=5, warmup=2, iters=5)
+        keep = [(a, b) for a in range(len(pt)) for b in range(len(db)) if pt[a] + db[b] > 0]
+        model, fit_err = sa.sa_latency_fit([ms[a, b] for a, b in keep], [sums[a, b] for a, b in keep], True)
+        src_k, src_v = rnd(32768, Hkv), rnd(32768, Hkv)
+        main = sa.sa_kv_session_open(pool)
+        sa.sa_rope_kv_append(pool, [main], [0, P + TAIL], src_k[:P + TAIL], src_v[:P + TAIL], None)
+        dec = [sa.sa_kv_session_open(pool) for _ in dec_len]
+        for sid, n in zip(dec, dec_len):
+            sa.sa_rope_kv_append(pool, [sid], [0, n], src_k[:n], src_v[:n], None)
+        k_seg, v_seg, q_seg = rnd(SEG, Hkv), rnd(SEG, Hkv), rnd(SEG, Hq)
+        free0 = sa.sa_kv_pool_free_pages(pool)
+        delta = sa.sa_est_batch_latency(model, [n + 64 for n in dec_len], [(room_chunk, P + SEG)])
+        est_dec = sa.sa_est_batch_latency(model, [n + 1 for n in dec_len], [])
+        look = sa.sa_kv_session_fork(pool, main, P)
+        st = torch.cuda.current_stream()
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        done, it, rows = 0, 0, []
+        lens = list(dec_len)
+        while done < SEG:
+            decode_L = [n + 1 for n in lens]
+            c = sa.sa_dynamic_chunk(model, decode_L, [], P + done, SEG - done, max_chunk, gran, delta)
+            if c <= 0:
+                raise RuntimeError("delta %.3f ms leaves no room for a granule" % delta)
+            adm = sa.sa_schedule_hybrid(model, decode_L, [], [(c, P + done)], delta)
+            sids = dec + [look]
+            indptr = np.concatenate([np.arange(n_dec + 1), [n_dec + c]]).astype(np.int32)
+            k = torch.cat([rnd(n_dec, Hkv), k_seg[done:done + c]])
+            v = torch.cat([rnd(n_dec, Hkv), v_seg[done:done + c]])
+            q = torch.cat([rnd(n_dec, Hq), q_seg[done:done + c]])
+            out = torch.empty_like(q)
+            flush.fill_(it & 1)                                            # the caches are not served from L2
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            ev[0].record(st)
+            sa.sa_rope_kv_append(pool, sids, indptr, k, v, q)
+            ws = torch.empty(max(sa.sa_mixed_attention_workspace_bytes(pool, sids, indptr), 256), dtype=torch.uint8, device=dev)
+            ev[1].record(st)
+            sa.sa_mixed_attention(pool, sids, indptr, q, out, None, 0.0, ws)
+            ev[2].record(st)
+            torch.cuda.synchronize()
+            rows.append({"chunk": int(c), "prefix": int(P + done), "admitted": list(adm[:3]), "est_ms": adm[3],
+                         "attention_ms": ev[1].elapsed_time(ev[2]), "append_ms": ev[0].elapsed_time(ev[1])})
+            done += c
+            it += 1
+            lens = [n + 1 for n in lens]
+        sa.sa_kv_session_commit(pool, main, look)
+        n_main, pg_main = sa.sa_kv_session_query(pool, main)
+        grown = sum((n + it + B - 1) // B - (n + B - 1) // B for n in dec_len)
+        pages_ok = (n_main == P + SEG and sa.sa_kv_pool_free_pages(pool) == free0 + (P + TAIL + B - 1) // B - len(pg_main) - grown)
+        warm = rows[1:] if len(rows) > 1 else rows                         # the first iteration pays first-use costs
+        meas = np.array([r["attention_ms"] for r in warm])
+        est = np.array([r["est_ms"] for r in warm])
+        return {"delta_ms": delta, "est_decode_only_ms": est_dec, "iterations": len(rows), "decode_rows": n_dec, "segment_tokens": SEG,
+                "chunks": [r["chunk"] for r in rows], "fit_max_rel_err": fit_err,
+                "model": {"c0_ms": model.c0_ms, "alpha_d_ms": model.alpha_d_ms, "alpha_p_ms": model.alpha_p_ms},
+                "all_admitted_under_delta": bool(all(r["admitted"] == [n_dec, 0, 1] and r["est_ms"] <= delta for r in rows)),
+                "violations": int((meas > delta).sum()), "measured_over_delta_max": float((meas / delta).max()),
+                "measured_over_delta_mean": float((meas / delta).mean()), "est_rel_err_max": float((np.abs(est - meas) / meas).max()),
+                "committed_pages_ok": bool(pages_ok), "rows": rows,
+                "note": "delta = Eq. 1 of the decode rows at the end of the run + a %d-token chunk at the deepest prefix; violations / "
+                        "measured_over_delta count the attention call's device time (CUDA events, L2 evicted before each iteration) of "
+                        "iterations 2.. against delta; every batch ran once (its append changes the sessions)" % room_chunk}
+    finally:
+        sa.sa_kv_pool_destroy(pool)
+        torch.cuda.empty_cache()
+
+
 def measure_gemm_ops(local: int, M: int = 64, iters: int = 15):
     """The layer's three plain GEMMs at a decode batch, one operator per event pair with the L2 evicted before it, ours
     (sa_linear_ws: split-K + reduction) beside cuBLAS (torch.matmul) on the same tensors: context for T_GEMM(M), not a
@@ -944,6 +1033,16 @@ def run_ours(args, world, rank, local):
                 for d, r_ in ds["rows"].items()}
         except Exception as e:   # noqa: BLE001 - a side measurement never takes the line down
             detail["decode_step_graph"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
+        try:
+            ll = measure_lookahead_loop(local)
+            detail["lookahead_loop"] = ll
+            line["lookahead_loop"] = {k: (round(v, 4) if isinstance(v, float) else v) for k, v in ll.items()
+                                      if k in ("delta_ms", "iterations", "decode_rows", "segment_tokens", "chunks", "violations",
+                                               "measured_over_delta_max", "measured_over_delta_mean", "est_rel_err_max",
+                                               "fit_max_rel_err", "all_admitted_under_delta", "committed_pages_ok")}
+        except Exception as e:   # noqa: BLE001 - a side measurement never takes the line down
+            detail["lookahead_loop"] = {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
+            line["lookahead_loop"] = detail["lookahead_loop"]
         summary = {"layer_cfg2": {"tflops": round(layer["achieved"], 1), "frac": round(layer["frac"], 4), "ms": round(layer["ms_per_step"], 3),
                                   "t_gemm_ms": layer.get("t_gemm_ms"), "t_gemm_floor_ms": layer.get("t_gemm_floor_ms")},
                    "transfer_cfg4": {"export_gbs": round(xfer["export_gbs"], 1), "import_gbs": round(xfer["import_gbs"], 1), "frac": round(xfer["frac"], 4)}}
@@ -998,6 +1097,7 @@ def main():
     ap.add_argument("--parts-only", action="store_true", help="only the decode / append measurements (for profiling them)")
     ap.add_argument("--layer-only", action="store_true", help="only the whole-layer measurement (for profiling the GEMMs)")
     ap.add_argument("--decode-step-only", action="store_true", help="only the captured decode iteration at small batch")
+    ap.add_argument("--lookahead-loop-only", action="store_true", help="only the closed loop of Alg. 2 (decode iterations + streamed lookahead chunks under delta)")
     ap.add_argument("--gemm-table-only", action="store_true", help="only T_GEMM(M) of the layer's dense operators at decode sizes")
     args = ap.parse_args()
     if args.layer_only:
@@ -1023,6 +1123,12 @@ def main():
         m_list = [1, 16, 64, 128]
         t = sa.sa_gemm_table(4096, 14336, Lr.num_q_heads, Lr.num_kv_heads, Lr.head_dim, m_list, warmup=3, iters=15)
         print(json.dumps({"t_gemm_ms": {str(m): round(float(x), 4) for m, x in zip(m_list, t)}, "operators": measure_gemm_ops(0)}))
+        return
+    if args.lookahead_loop_only:
+        import __graft_entry__
+        __graft_entry__.build()
+        torch.cuda.set_device(0)
+        print(json.dumps({"lookahead_loop": measure_lookahead_loop(0)}))
         return
     if args.decode_step_only:
         import __graft_entry__
